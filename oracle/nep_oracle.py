@@ -1,0 +1,221 @@
+"""ctypes loader for oracle/nep_oracle.c (fp64 CPU oracle -- test infrastructure, not the product).
+
+Argument marshalling only; every number is computed by the C file.  The shared object is compiled
+with gcc on first use (and by __graft_entry__.build()).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nep_oracle.c")
+_SO = os.path.join(_HERE, "libnep_oracle.so")
+_lib = None
+
+
+class OracleHyper(C.Structure):
+    _fields_ = [("n_types", C.c_int32),
+                ("rc_radial", C.c_double), ("rc_angular", C.c_double),
+                ("n_max_radial", C.c_int32), ("n_max_angular", C.c_int32),
+                ("basis_radial", C.c_int32), ("basis_angular", C.c_int32),
+                ("l_max_3b", C.c_int32), ("l_max_4b", C.c_int32), ("l_max_5b", C.c_int32),
+                ("n_neurons", C.c_int32)]
+
+    @classmethod
+    def from_hyper(cls, h) -> "OracleHyper":
+        return cls(h.n_types, h.rc_radial, h.rc_angular, h.n_max_radial, h.n_max_angular,
+                   h.basis_radial, h.basis_angular, h.l_max_3b, h.l_max_4b, h.l_max_5b, h.n_neurons)
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp; rebuilt when the source is newer than the .so."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=gnu11",
+               _SRC, "-o", _SO, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_lp = C.POINTER(C.c_int64)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.onep_num_threads.restype = C.c_int
+        L.onep_num_descriptors.restype = C.c_int
+        L.onep_num_descriptors.argtypes = [C.POINTER(OracleHyper)]
+        L.onep_fc.restype = C.c_double
+        L.onep_fc.argtypes = [C.c_double, C.c_double]
+        L.onep_dfc.restype = C.c_double
+        L.onep_dfc.argtypes = [C.c_double, C.c_double]
+        L.onep_fk.restype = None
+        L.onep_fk.argtypes = [C.c_double, C.c_double, C.c_int, _dp, _dp]
+        L.onep_bk.restype = None
+        L.onep_bk.argtypes = [_dp, _dp]
+        L.onep_bk_grad.restype = None
+        L.onep_bk_grad.argtypes = [_dp, _dp]
+        L.onep_constants.restype = None
+        L.onep_constants.argtypes = [_dp, _dp, _dp]
+        L.onep_q_from_S.restype = None
+        L.onep_q_from_S.argtypes = [_dp, _dp, _dp]
+        L.onep_ann.restype = None
+        L.onep_ann.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.onep_neighbors.restype = C.c_int64
+        L.onep_neighbors.argtypes = [C.c_int64, _dp, _dp, _ip, C.c_double, _ip, _ip, C.c_int64]
+        L.onep_neighbors_of.restype = C.c_int64
+        L.onep_neighbors_of.argtypes = [C.c_int64, _dp, _dp, _ip, C.c_double, C.c_int64, _lp, _ip, _ip, C.c_int64]
+        L.onep_compute.restype = C.c_int
+        L.onep_compute.argtypes = [C.POINTER(OracleHyper), _dp, _dp, _dp, _dp, _dp, _dp,
+                                   C.c_int64, _dp, _ip, _dp, _ip, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.onep_md.restype = C.c_int
+        L.onep_md.argtypes = [C.POINTER(OracleHyper), _dp, _dp, _dp, _dp, _dp, _dp,
+                              C.c_int64, _dp, _dp, _ip, _dp, _dp, _ip, C.c_double, C.c_int32, _dp, _dp]
+        _lib = L
+    return _lib
+
+
+def _d(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a: Optional[np.ndarray], t=_dp):
+    return a.ctypes.data_as(t) if a is not None else None
+
+
+def num_threads() -> int:
+    return int(lib().onep_num_threads())
+
+
+def num_descriptors(hyper) -> int:
+    h = OracleHyper.from_hyper(hyper)
+    return int(lib().onep_num_descriptors(C.byref(h)))
+
+
+def fc(r: float, rc: float) -> float:
+    return float(lib().onep_fc(r, rc))
+
+
+def fk(r: float, rc: float, nbas: int):
+    f = np.zeros(nbas + 1)
+    df = np.zeros(nbas + 1)
+    lib().onep_fk(r, rc, nbas, _p(f), _p(df))
+    return f, df
+
+
+def bk(d) -> np.ndarray:
+    d = _d(d)
+    out = np.zeros(24)
+    lib().onep_bk(_p(d), _p(out))
+    return out
+
+
+def bk_grad(d) -> np.ndarray:
+    d = _d(d)
+    out = np.zeros((24, 3))
+    lib().onep_bk_grad(_p(d), _p(out))
+    return out
+
+
+def constants():
+    c3, c4, c5 = np.zeros(24), np.zeros(5), np.zeros(3)
+    lib().onep_constants(_p(c3), _p(c4), _p(c5))
+    return c3, c4, c5
+
+
+def q_from_S(S):
+    S = _d(S)
+    out = np.zeros(6)
+    dq = np.zeros((6, 24))
+    lib().onep_q_from_S(_p(S), _p(out), _p(dq))
+    return out, dq
+
+
+def ann(w0, b0, w1, b1, q):
+    w0, b0, w1, b1, q = map(_d, (w0, b0, w1, b1, q))
+    H, D = w0.shape
+    e = C.c_double(0.0)
+    fp = np.zeros(D)
+    lib().onep_ann(D, H, _p(w0), _p(b0), _p(w1), _p(b1), _p(q), C.byref(e), _p(fp))
+    return e.value, fp
+
+
+def _pbc(pbc) -> np.ndarray:
+    return np.ascontiguousarray(pbc, dtype=np.int32)
+
+
+def neighbors(pos, box, rc: float, pbc=(1, 1, 1), cap: Optional[int] = None):
+    """Brute-force neighbour sets: returns (count[n], list[n][cap]); grows cap until nothing is cut."""
+    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    n = pos.shape[0]
+    cap = cap or 64
+    while True:
+        count = np.zeros(n, dtype=np.int32)
+        lst = np.full((n, cap), -1, dtype=np.int32)
+        mx = lib().onep_neighbors(n, _p(pos), _p(box), _p(pbc, _ip), rc, _p(count, _ip), _p(lst, _ip), cap)
+        if mx <= cap:
+            return count, lst
+        cap = int(mx)
+
+
+def neighbors_of(pos, box, rc: float, sel, pbc=(1, 1, 1), cap: int = 256):
+    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    sel = np.ascontiguousarray(sel, dtype=np.int64)
+    n, ns = pos.shape[0], sel.shape[0]
+    while True:
+        count = np.zeros(ns, dtype=np.int32)
+        lst = np.full((ns, cap), -1, dtype=np.int32)
+        mx = lib().onep_neighbors_of(n, _p(pos), _p(box), _p(pbc, _ip), rc, ns, _p(sel, _lp),
+                                     _p(count, _ip), _p(lst, _ip), cap)
+        if mx <= cap:
+            return count, lst
+        cap = int(mx)
+
+
+def compute(hyper, params, pos, types, box, pbc=(1, 1, 1), want_internals: bool = False):
+    """Energy[n], force[n][3], virial[n][9] (+ q[n][D], fp[n][D], S[n][NA][24] if want_internals).
+    `params` holds fp32 arrays; they are widened to fp64 here, unchanged in value."""
+    h = OracleHyper.from_hyper(hyper)
+    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    types = np.ascontiguousarray(types, dtype=np.int32)
+    n = pos.shape[0]
+    cr, ca, w0, b0, w1, b1 = map(_d, (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1))
+    D = int(lib().onep_num_descriptors(C.byref(h)))
+    NA = hyper.n_max_angular + 1
+    e = np.zeros(n)
+    f = np.zeros((n, 3))
+    w = np.zeros((n, 9))
+    q = np.zeros((n, D)) if want_internals else None
+    fp = np.zeros((n, D)) if want_internals else None
+    S = np.zeros((n, NA, 24)) if want_internals else None
+    rc = lib().onep_compute(C.byref(h), _p(cr), _p(ca), _p(w0), _p(b0), _p(w1), _p(b1),
+                            n, _p(pos), _p(types, _ip), _p(box), _p(pbc, _ip),
+                            _p(e), _p(f), _p(w), _p(q), _p(fp), _p(S))
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return (e, f, w, q, fp, S) if want_internals else (e, f, w)
+
+
+def md(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int, pbc=(1, 1, 1)):
+    """Velocity-Verlet NVE; returns (pos, vel, e_pot[n_steps+1], e_kin[n_steps+1]) (copies)."""
+    h = OracleHyper.from_hyper(hyper)
+    pos, vel = _d(pos).copy(), _d(vel).copy()
+    box, pbc, masses = _d(box), _pbc(pbc), _d(masses)
+    types = np.ascontiguousarray(types, dtype=np.int32)
+    cr, ca, w0, b0, w1, b1 = map(_d, (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1))
+    ep = np.zeros(n_steps + 1)
+    ek = np.zeros(n_steps + 1)
+    rc = lib().onep_md(C.byref(h), _p(cr), _p(ca), _p(w0), _p(b0), _p(w1), _p(b1),
+                       pos.shape[0], _p(pos), _p(vel), _p(types, _ip), _p(masses), _p(box), _p(pbc, _ip),
+                       dt_fs, n_steps, _p(ep), _p(ek))
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return pos, vel, ep, ek
