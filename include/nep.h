@@ -1,0 +1,157 @@
+/*
+ * nep.h -- C ABI of the B200-native NEP3 hot path (arxiv 2205.10046: Fan et al., GPUMD / NEP3).
+ *
+ * One handle = one model on one GPU and one CUDA stream.  All work of every call is enqueued on the
+ * stream given to nep_create(); a call synchronises that stream only where stated.  Pointers named
+ * *_dev are caller-owned DEVICE memory (e.g. torch tensors' data_ptr()) valid for the duration of the
+ * call; pointers named *_host (and all parameter arrays of nep_create) are HOST memory.  The handle
+ * owns only its internal scratch (neighbour lists, descriptor sums, partial forces, quantised
+ * positions), sized at nep_neighbors() and reused.
+ *
+ * Units: eV, Angstrom, amu, fs.  Atom order of every output is the caller's atom order (the internal
+ * spatial sort is invisible).  Every function returns NEP_OK (0) or a negative nep_status;
+ * nep_last_error() gives a text for the last failure on that handle.  There is no CPU fallback: every
+ * step runs in the library's CUDA kernels, and every entry point except nep_num_descriptors() and
+ * nep_status_string() fails with NEP_ERR_CUDA when no CUDA device is usable.
+ *
+ * Citations are to /root/reference/PAPER.md (line numbers) and to DESIGN.md "Readings" for the places
+ * where the paper is silent or garbled.
+ */
+#ifndef NEP_B200_H_
+#define NEP_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nep_ctx nep_t;
+
+/* Hyper-parameters of a NEP3 model in the paper's notation (the keywords of nep.in).   */
+typedef struct {
+    int32_t n_types;                        /* N_typ >= 1; at most 16                   */
+    double rc_radial, rc_angular;           /* r_c^R, r_c^A in Angstrom; 0 < rc_angular <= rc_radial  */
+    int32_t n_max_radial, n_max_angular;    /* n = 0..n_max; 0..15 / 0..15       */
+    int32_t basis_radial, basis_angular;    /* N_bas: k = 0..N_bas; 0..31            */
+    int32_t l_max_3b;                       /* must be 4 (Eqs. 13-16)               */
+    int32_t l_max_4b;                       /* 0 (no 4-body block) or 2                */
+    int32_t l_max_5b;                       /* 0 (no 5-body block) or 1                */
+    int32_t n_neurons;                      /* N_neu >= 1 (Eq. 1); at most 200        */
+} nep_hyper_t;
+
+typedef enum {
+    NEP_OK = 0,
+    NEP_ERR_INVALID_ARG = -1,        /* null pointer, value out of the ranges above, n <= 0, cap too small */
+    NEP_ERR_BOX_TOO_SMALL = -2,      /* a box edge < 2 (rc_radial + skin): minimum image would break      */
+    NEP_ERR_UNSUPPORTED_BOX = -3,    /* non-orthorhombic box (off-diagonal elements != 0)                 */
+    NEP_ERR_NEIGHBOR_OVERFLOW = -4,  /* a list outgrew its storage and regrowing failed (never truncated) */
+    NEP_ERR_STATE = -5,              /* compute / md_step before nep_neighbors, or hook before compute    */
+    NEP_ERR_CUDA = -6,               /* a CUDA runtime call failed (text in nep_last_error)               */
+    NEP_ERR_NOMEM = -7               /* device or host allocation failed                                  */
+} nep_status;
+
+/* ---- model ---------------------------------------------------------------------------------------
+ * nep_create: builds a handle; copies all parameter arrays (HOST, fp32) to the device.  Synchronises.
+ *   c_radial  [T][T][NR][KR]  c^{ij}_{nk} of Eq. (3), index (t_i, t_j, n, k); t_i = type of
+ *                             the central atom i, t_j = type of the neighbour; NOT assumed symmetric.
+ *   c_angular [T][T][NA][KA]  same for the angular radial functions.
+ *   w0 [H][D] row-major ([neuron][descriptor], Listing 1), b0 [H], w1 [H], b1 [1]:
+ *             U = sum_m w1[m] tanh(sum_v w0[m][v] q_v - b0[m]) - b1   (Eq. 1).
+ *   mass_amu  [T] masses per type (used by md_step only).
+ *   NR = n_max_radial+1, KR = basis_radial+1, NA = n_max_angular+1, KA = basis_angular+1,
+ *   D = nep_num_descriptors(h), H = n_neurons.
+ *   Descriptor order (reading A2): v = n for the radial components (Eq. 2); then the blocks
+ *   l = 1,2,3,4 (Eqs. 13-16), 4-body q_n222 (Eq. 18), 5-body q_n1111 (Eq. 19): v = NR + block*NA + n.
+ *   device: CUDA device ordinal; cuda_stream: a cudaStream_t (NULL = the legacy default stream).
+ * nep_destroy: synchronises the stream and frees everything the handle owns.                          */
+int nep_create(nep_t** out, const nep_hyper_t* h,
+               const float* c_radial, const float* c_angular,
+               const float* w0, const float* b0, const float* w1, const float* b1,
+               const double* mass_amu, int device, void* cuda_stream);
+int nep_destroy(nep_t* nep);
+
+/* N_des of Eq. (20); pure host arithmetic; negative status on invalid h.           */
+int nep_num_descriptors(const nep_hyper_t* h);
+
+/* ---- (a1) neighbour construction -----------------------------------------------------------------
+ * Cell-binned construction of the radial and angular neighbour lists NN^R/NL^R, NN^A/NL^A
+ * (construction itself is not described by the paper).
+ *   pos_dev  [n][3] fp64 positions (need not be wrapped into the box);  type_dev [n] int32 in [0,T);
+ *   box      HOST, 9 doubles, row vectors a,b,c; must be orthorhombic (only box[0], box[4], box[8] != 0);
+ *   skin     >= 0: lists hold every pair with |r_ij| < r_c + skin (Verlet skin).
+ * Membership (reading A8): with d = (r_j - r_i) - L*rint((r_j - r_i)/L) per axis in IEEE fp64,
+ * j is a neighbour of i iff (dx*dx + dy*dy) + dz*dz < (r_c+skin)*(r_c+skin) -- evaluated exactly so, so
+ * the sets equal a brute-force fp64 search bit for bit.  The list order within an atom is unspecified
+ * but deterministic.  Copies the types; synchronises (reads back list sizes; regrows and rebuilds on
+ * overflow).  n <= 16,777,216.                                                                        */
+int nep_neighbors(nep_t* nep, int64_t n, const double* pos_dev, const int32_t* type_dev,
+                  const double box[9], double skin);
+
+/* Largest list length of the last build: which = 0 radial (r_c^R + skin), 1 angular (r_c^A + skin).   */
+int nep_max_neighbors(nep_t* nep, int which, int32_t* max_count_host);
+
+/* Copies the lists of the last build out in the caller's atom order and numbering:
+ * count_dev [n], list_dev [n][cap] row-major (entries m >= count are left untouched).
+ * NEP_ERR_INVALID_ARG if cap < nep_max_neighbors().  Does not synchronise.                            */
+int nep_get_neighbors(nep_t* nep, int which, int32_t* count_dev, int32_t* list_dev, int32_t cap);
+
+/* ---- (a2)-(a8) energy, force, virial -------------------------------------------------------------
+ * One evaluation with the lists of the last nep_neighbors() (valid while no atom has moved more than
+ * skin/2 since then): Chebyshev radial descriptors Eqs. (2)-(5); angular sums S_nk Eq. (12) and the
+ * 3-/4-/5-body components Eqs. (13)-(19); network Eq. (1); partial forces Eq. (21); F_i Eqs. (22)-(23);
+ * per-atom virial W_i Eq. (24).
+ *   pos_dev    [n][3] fp64;
+ *   energy_dev [n] fp64 site energies U_i (eV);  force_dev [n][3] fp64 (eV/Angstrom);
+ *   virial_dev [n][9] fp64 (eV), W[3a+b] = sum_j r_ij^a (dU_j/dr_ji)^b, r_ij = r_j - r_i (not symmetrised;
+ *              sum_i W_i = -dE/d(strain), reading A7).   Any output pointer may be NULL.
+ * Arithmetic: fp32 inside the kernels, fp64 I/O.  Does not synchronise.                */
+int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* force_dev, double* virial_dev);
+
+/* ---- (a9) velocity-Verlet NVE ---------------------------------------------------------------------
+ * n_steps steps of  v += (dt/2) F/m;  r += dt v;  [lists rebuilt when the number of steps since the
+ * last build reaches rebuild_every];  F = F(r);  v += (dt/2) F/m   (NVE; the paper prints no
+ * integrator formula, reading A11).  a[A/fs^2] = F/m * 9.648533212e-3.
+ *   pos_dev [n][3], vel_dev [n][3] (Angstrom/fs) are updated in place; positions are never wrapped.
+ *   The first call after nep_neighbors()/nep_compute() with other positions evaluates F(r) first; later
+ *   calls reuse the forces of the previous call (so positions must not be edited in between without
+ *   calling nep_neighbors() again).  rebuild_every >= 1; skin as in nep_neighbors().
+ * Synchronises once per list rebuild (overflow check), otherwise asynchronous.                        */
+int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs,
+            int32_t n_steps, int32_t rebuild_every, double skin);
+
+/* Results of the most recent internal evaluation (the one md_step ended with, or nep_compute):
+ * same layouts as nep_compute; any pointer may be NULL.  Does not synchronise.                        */
+int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* virial_dev);
+
+/* Largest displacement (Angstrom) of any atom since the last list build, measured at the most recent
+ * evaluation; the lists are valid while it is below skin/2.  Synchronises.                            */
+int nep_max_displacement(nep_t* nep, double* disp_host);
+
+/* ---- host-buffer entry points (end-to-end path: H2D copies, kernels, D2H copies) -------------------
+ * nep_compute_host: nep_neighbors + nep_compute on HOST arrays (pageable or pinned); synchronises.
+ * md_run_host: uploads pos/vel, runs nep_neighbors (first call or when n changed) and md_step, downloads
+ *   pos/vel and, if non-NULL, the final energy/force/virial; synchronises.                            */
+int nep_compute_host(nep_t* nep, int64_t n, const double* pos_host, const int32_t* type_host,
+                     const double box[9], double skin,
+                     double* energy_host, double* force_host, double* virial_host);
+int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const int32_t* type_host,
+                const double box[9], double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin,
+                double* energy_host, double* force_host, double* virial_host);
+
+/* ---- test hooks (internals of the last evaluation, caller's atom order) ---------------------------
+ * q_dev [n][D] descriptor, fp_dev [n][D] dU_i/dq_v, S_dev [n][NA][24] sums of Eq. (12).
+ * fp32; any pointer may be NULL.  Do not synchronise.                                                 */
+int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev);
+int nep_get_angular_sums(nep_t* nep, float* S_dev);
+
+/* Number of kernel launches the handle has enqueued so far (for bench.py's gpu_launches).             */
+int64_t nep_launch_count(const nep_t* nep);
+
+const char* nep_last_error(const nep_t* nep);
+const char* nep_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEP_B200_H_ */

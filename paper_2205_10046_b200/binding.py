@@ -1,0 +1,276 @@
+"""ctypes binding with the same names as include/nep.h -- argument marshalling only.
+
+PyTorch is used for device memory and the CUDA stream; all arithmetic of the path happens inside
+libnep_b200.so.  Functions raise NepError on any non-zero status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
+_lib = None
+
+# every symbol include/nep.h declares
+exported_symbols = (
+    "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
+    "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
+    "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums",
+    "nep_launch_count", "nep_last_error", "nep_status_string",
+)
+
+
+class NepError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"nep status {status}: {text}")
+        self.status = status
+
+
+class NepHyper(C.Structure):
+    _fields_ = [("n_types", C.c_int32),
+                ("rc_radial", C.c_double), ("rc_angular", C.c_double),
+                ("n_max_radial", C.c_int32), ("n_max_angular", C.c_int32),
+                ("basis_radial", C.c_int32), ("basis_angular", C.c_int32),
+                ("l_max_3b", C.c_int32), ("l_max_4b", C.c_int32), ("l_max_5b", C.c_int32),
+                ("n_neurons", C.c_int32)]
+
+    @classmethod
+    def from_hyper(cls, h) -> "NepHyper":
+        return cls(h.n_types, h.rc_radial, h.rc_angular, h.n_max_radial, h.n_max_angular,
+                   h.basis_radial, h.basis_angular, h.l_max_3b, h.l_max_4b, h.l_max_5b, h.n_neurons)
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Loads libnep_b200.so; fails loudly if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2205_10046_b200.build` "
+                          "(there is no CPU or PyTorch fallback for the NEP path)")
+    L = C.CDLL(_LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    fp = C.POINTER(C.c_float)
+    dp = C.POINTER(C.c_double)
+    ip = C.POINTER(C.c_int32)
+    L.nep_create.restype = C.c_int
+    L.nep_create.argtypes = [C.POINTER(vp), C.POINTER(NepHyper), fp, fp, fp, fp, fp, fp, dp, C.c_int, vp]
+    L.nep_destroy.restype = C.c_int
+    L.nep_destroy.argtypes = [vp]
+    L.nep_num_descriptors.restype = C.c_int
+    L.nep_num_descriptors.argtypes = [C.POINTER(NepHyper)]
+    L.nep_neighbors.restype = C.c_int
+    L.nep_neighbors.argtypes = [vp, i64, vp, vp, dp, dbl]
+    L.nep_max_neighbors.restype = C.c_int
+    L.nep_max_neighbors.argtypes = [vp, C.c_int, ip]
+    L.nep_get_neighbors.restype = C.c_int
+    L.nep_get_neighbors.argtypes = [vp, C.c_int, vp, vp, i32]
+    L.nep_compute.restype = C.c_int
+    L.nep_compute.argtypes = [vp, vp, vp, vp, vp]
+    L.md_step.restype = C.c_int
+    L.md_step.argtypes = [vp, vp, vp, dbl, i32, i32, dbl]
+    L.nep_get_last.restype = C.c_int
+    L.nep_get_last.argtypes = [vp, vp, vp, vp]
+    L.nep_max_displacement.restype = C.c_int
+    L.nep_max_displacement.argtypes = [vp, dp]
+    L.nep_compute_host.restype = C.c_int
+    L.nep_compute_host.argtypes = [vp, i64, vp, vp, dp, dbl, vp, vp, vp]
+    L.md_run_host.restype = C.c_int
+    L.md_run_host.argtypes = [vp, i64, vp, vp, vp, dp, dbl, i32, i32, dbl, vp, vp, vp]
+    L.nep_get_descriptors.restype = C.c_int
+    L.nep_get_descriptors.argtypes = [vp, vp, vp]
+    L.nep_get_angular_sums.restype = C.c_int
+    L.nep_get_angular_sums.argtypes = [vp, vp]
+    L.nep_launch_count.restype = i64
+    L.nep_launch_count.argtypes = [vp]
+    L.nep_last_error.restype = C.c_char_p
+    L.nep_last_error.argtypes = [vp]
+    L.nep_status_string.restype = C.c_char_p
+    L.nep_status_string.argtypes = [C.c_int]
+    _lib = L
+    return L
+
+
+def _box9(box) -> np.ndarray:
+    b = np.asarray(box, dtype=np.float64)
+    if b.shape == (3,):
+        b = np.diag(b)
+    return np.ascontiguousarray(b.reshape(9))
+
+
+def _f32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+class NEP:
+    """One model on one GPU/stream.  Methods mirror include/nep.h one to one."""
+
+    def __init__(self, hyper, params, masses: Sequence[float], device: int = 0, stream: Optional[int] = None):
+        import torch  # device memory + streams only
+        if not torch.cuda.is_available():
+            raise NepError(-6, "no CUDA device: the NEP path has no CPU fallback")
+        self._torch = torch
+        self._L = load_library()
+        self.hyper = hyper
+        self.device = device
+        self._h = NepHyper.from_hyper(hyper)
+        self.n_des = self._L.nep_num_descriptors(C.byref(self._h))
+        if self.n_des < 0:
+            raise NepError(self.n_des, self._L.nep_status_string(self.n_des).decode())
+        torch.cuda.set_device(device)
+        torch.cuda.init()
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        self.stream = stream
+        fp = C.POINTER(C.c_float)
+        arrs = [_f32(params.c_radial), _f32(params.c_angular), _f32(params.w0), _f32(params.b0),
+                _f32(params.w1), _f32(params.b1)]
+        m = np.ascontiguousarray(masses, dtype=np.float64)
+        h = C.c_void_p()
+        rc = self._L.nep_create(C.byref(h), C.byref(self._h), *[a.ctypes.data_as(fp) for a in arrs],
+                                m.ctypes.data_as(C.POINTER(C.c_double)), device, C.c_void_p(stream))
+        if rc != 0:
+            raise NepError(rc, self._L.nep_status_string(rc).decode())
+        self._h_ptr = h
+        self.n = 0
+
+    # ---- plumbing
+    def _check(self, rc: int):
+        if rc != 0:
+            raise NepError(rc, self._L.nep_last_error(self._h_ptr).decode() or self._L.nep_status_string(rc).decode())
+
+    def _dev(self, t, dtype, numel: Optional[int] = None):
+        torch = self._torch
+        if t is None:
+            return None
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+            raise ValueError(f"expected a contiguous CUDA tensor of dtype {dtype}")
+        if numel is not None and t.numel() != numel:
+            raise ValueError(f"expected {numel} elements, got {t.numel()}")
+        return C.c_void_p(t.data_ptr())
+
+    def close(self):
+        if getattr(self, "_h_ptr", None) is not None and self._h_ptr.value:
+            self._L.nep_destroy(self._h_ptr)
+            self._h_ptr = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- include/nep.h
+    def nep_neighbors(self, pos, types, box, skin: float):
+        torch = self._torch
+        n = pos.shape[0]
+        b = _box9(box)
+        self._check(self._L.nep_neighbors(self._h_ptr, n, self._dev(pos, torch.float64, 3 * n),
+                                          self._dev(types, torch.int32, n),
+                                          b.ctypes.data_as(C.POINTER(C.c_double)), float(skin)))
+        self.n = n
+
+    def nep_max_neighbors(self, which: int) -> int:
+        v = C.c_int32(0)
+        self._check(self._L.nep_max_neighbors(self._h_ptr, which, C.byref(v)))
+        return v.value
+
+    def nep_get_neighbors(self, which: int):
+        torch = self._torch
+        cap = max(1, self.nep_max_neighbors(which))
+        count = torch.zeros(self.n, dtype=torch.int32, device=f"cuda:{self.device}")
+        lst = torch.full((self.n, cap), -1, dtype=torch.int32, device=f"cuda:{self.device}")
+        self._check(self._L.nep_get_neighbors(self._h_ptr, which, C.c_void_p(count.data_ptr()),
+                                              C.c_void_p(lst.data_ptr()), cap))
+        return count, lst
+
+    def nep_compute(self, pos, energy=None, force=None, virial=None):
+        torch = self._torch
+        n = self.n
+        dev = f"cuda:{self.device}"
+        if energy is None:
+            energy = torch.empty(n, dtype=torch.float64, device=dev)
+        if force is None:
+            force = torch.empty((n, 3), dtype=torch.float64, device=dev)
+        if virial is None:
+            virial = torch.empty((n, 9), dtype=torch.float64, device=dev)
+        self._check(self._L.nep_compute(self._h_ptr, self._dev(pos, torch.float64, 3 * n),
+                                        self._dev(energy, torch.float64, n), self._dev(force, torch.float64, 3 * n),
+                                        self._dev(virial, torch.float64, 9 * n)))
+        return energy, force, virial
+
+    def md_step(self, pos, vel, dt_fs: float, n_steps: int, rebuild_every: int, skin: float):
+        torch = self._torch
+        n = self.n
+        self._check(self._L.md_step(self._h_ptr, self._dev(pos, torch.float64, 3 * n),
+                                    self._dev(vel, torch.float64, 3 * n), float(dt_fs), int(n_steps),
+                                    int(rebuild_every), float(skin)))
+
+    def nep_get_last(self):
+        torch = self._torch
+        n, dev = self.n, f"cuda:{self.device}"
+        e = torch.empty(n, dtype=torch.float64, device=dev)
+        f = torch.empty((n, 3), dtype=torch.float64, device=dev)
+        w = torch.empty((n, 9), dtype=torch.float64, device=dev)
+        self._check(self._L.nep_get_last(self._h_ptr, C.c_void_p(e.data_ptr()), C.c_void_p(f.data_ptr()),
+                                         C.c_void_p(w.data_ptr())))
+        return e, f, w
+
+    def nep_max_displacement(self) -> float:
+        v = C.c_double(0.0)
+        self._check(self._L.nep_max_displacement(self._h_ptr, C.byref(v)))
+        return v.value
+
+    def nep_get_descriptors(self):
+        torch = self._torch
+        n, dev = self.n, f"cuda:{self.device}"
+        q = torch.empty((n, self.n_des), dtype=torch.float32, device=dev)
+        fp = torch.empty((n, self.n_des), dtype=torch.float32, device=dev)
+        self._check(self._L.nep_get_descriptors(self._h_ptr, C.c_void_p(q.data_ptr()), C.c_void_p(fp.data_ptr())))
+        return q, fp
+
+    def nep_get_angular_sums(self):
+        torch = self._torch
+        S = torch.empty((self.n, self.hyper.n_max_angular + 1, 24), dtype=torch.float32, device=f"cuda:{self.device}")
+        self._check(self._L.nep_get_angular_sums(self._h_ptr, C.c_void_p(S.data_ptr())))
+        return S
+
+    def nep_launch_count(self) -> int:
+        return int(self._L.nep_launch_count(self._h_ptr))
+
+    # host-buffer entry points: numpy arrays or pinned CPU tensors (anything exposing a host pointer)
+    @staticmethod
+    def _host_ptr(a):
+        if a is None:
+            return None
+        if isinstance(a, np.ndarray):
+            if not a.flags["C_CONTIGUOUS"]:
+                raise ValueError("host arrays must be C-contiguous")
+            return C.c_void_p(a.ctypes.data)
+        return C.c_void_p(a.data_ptr())          # CPU torch tensor (pinned or pageable)
+
+    def nep_compute_host(self, pos, types, box, skin: float, energy=None, force=None, virial=None):
+        n = pos.shape[0]
+        b = _box9(box)
+        self._check(self._L.nep_compute_host(self._h_ptr, n, self._host_ptr(pos), self._host_ptr(types),
+                                             b.ctypes.data_as(C.POINTER(C.c_double)), float(skin),
+                                             self._host_ptr(energy), self._host_ptr(force), self._host_ptr(virial)))
+        self.n = n
+
+    def md_run_host(self, pos, vel, types, box, dt_fs: float, n_steps: int, rebuild_every: int, skin: float,
+                    energy=None, force=None, virial=None):
+        n = pos.shape[0]
+        b = _box9(box)
+        self._check(self._L.md_run_host(self._h_ptr, n, self._host_ptr(pos), self._host_ptr(vel),
+                                        self._host_ptr(types), b.ctypes.data_as(C.POINTER(C.c_double)),
+                                        float(dt_fs), int(n_steps), int(rebuild_every), float(skin),
+                                        self._host_ptr(energy), self._host_ptr(force), self._host_ptr(virial)))
+        self.n = n

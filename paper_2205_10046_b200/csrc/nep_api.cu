@@ -1,0 +1,694 @@
+// nep_api.cu -- the C ABI of include/nep.h: host-side logic, allocation and kernel dispatch.
+// Product code; never links, includes or calls anything under oracle/.
+#include <math.h>
+#include <stdlib.h>
+
+#include <new>
+#include <vector>
+
+#include "nep_common.cuh"
+#include "nep_neighbor.cuh"
+#include "nep_kernels.cuh"
+
+namespace {
+
+const double kAccConv = 9.648533212e-3;   // (eV/Angstrom/amu) -> Angstrom/fs^2 (reading A10)
+
+struct HostCoef { NepCoef c; };
+
+NepCoef make_coef()
+{
+    // Eqs. (13)-(16), (18), (19): closed forms of the pre-computed coefficients.
+    NepCoef C;
+    const double pi = 3.14159265358979323846;
+    const double c3[NEP_NUM_S] = {
+        3.0 / (4 * pi), 3.0 / (4 * pi), 3.0 / (4 * pi),
+        5.0 / (16 * pi), 15.0 / (4 * pi), 15.0 / (4 * pi), 15.0 / (16 * pi), 15.0 / (16 * pi),
+        7.0 / (16 * pi), 21.0 / (32 * pi), 21.0 / (32 * pi), 105.0 / (16 * pi), 105.0 / (16 * pi),
+        35.0 / (32 * pi), 35.0 / (32 * pi),
+        9.0 / (256 * pi), 45.0 / (32 * pi), 45.0 / (32 * pi), 45.0 / (64 * pi), 45.0 / (64 * pi),
+        315.0 / (32 * pi), 315.0 / (32 * pi), 315.0 / (256 * pi), 315.0 / (256 * pi)};
+    for (int k = 0; k < NEP_NUM_S; ++k) C.c3[k] = (float)c3[k];
+    const double y20 = 0.25 * sqrt(5.0 / pi), y21 = 0.5 * sqrt(15.0 / (2 * pi)), y22 = 0.25 * sqrt(15.0 / (2 * pi));
+    C.c4[0] = (float)(-sqrt(2.0 / 35.0) * y20 * y20 * y20);
+    C.c4[1] = (float)(-6.0 * sqrt(1.0 / 70.0) * y20 * y21 * y21);
+    C.c4[2] = (float)(6.0 * sqrt(2.0 / 35.0) * y20 * y22 * y22);
+    C.c4[3] = (float)(6.0 * sqrt(3.0 / 35.0) * y21 * y21 * y22);
+    C.c4[4] = (float)(-12.0 * sqrt(3.0 / 35.0) * y21 * y21 * y22);
+    C.c5[0] = (float)(21.0 / (80 * pi * pi));
+    C.c5[1] = (float)(21.0 / (40 * pi * pi));
+    C.c5[2] = (float)(21.0 / (80 * pi * pi));
+    return C;
+}
+
+int validate_hyper(const nep_hyper_t* h)
+{
+    if (!h) return NEP_ERR_INVALID_ARG;
+    if (h->n_types < 1 || h->n_types > NEP_MAX_TYPES) return NEP_ERR_INVALID_ARG;
+    if (!(h->rc_angular > 0.0) || !(h->rc_radial >= h->rc_angular)) return NEP_ERR_INVALID_ARG;
+    if (h->n_max_radial < 0 || h->n_max_radial > 15 || h->n_max_angular < 0 || h->n_max_angular > 15) return NEP_ERR_INVALID_ARG;
+    if (h->basis_radial < 0 || h->basis_radial > 31 || h->basis_angular < 0 || h->basis_angular > 31) return NEP_ERR_INVALID_ARG;
+    if (h->l_max_3b != 4) return NEP_ERR_INVALID_ARG;
+    if (h->l_max_4b != 0 && h->l_max_4b != 2) return NEP_ERR_INVALID_ARG;
+    if (h->l_max_5b != 0 && h->l_max_5b != 1) return NEP_ERR_INVALID_ARG;
+    if (h->n_neurons < 1 || h->n_neurons > 200) return NEP_ERR_INVALID_ARG;
+    return NEP_OK;
+}
+
+int n_des(const nep_hyper_t* h)
+{
+    const int nblk = h->l_max_3b + (h->l_max_4b >= 2 ? 1 : 0) + (h->l_max_5b >= 1 ? 1 : 0);
+    return (h->n_max_radial + 1) + (h->n_max_angular + 1) * nblk;     // Eq. (20)
+}
+
+template <typename T>
+int dev_alloc(nep_t* nep, T** p, size_t count)
+{
+    if (*p) { cudaFree(*p); *p = nullptr; }
+    if (count == 0) count = 1;
+    cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        snprintf(nep->err, sizeof(nep->err), "cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
+        cudaGetLastError();
+        return NEP_ERR_NOMEM;
+    }
+    return NEP_OK;
+}
+#define NEP_TRY(x) do { int rc_ = (x); if (rc_ != NEP_OK) return rc_; } while (0)
+
+template <typename K>
+int allow_smem(nep_t* nep, K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024) NEP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return NEP_OK;
+}
+
+// ---- allocation ----------------------------------------------------------------------------------------
+int alloc_lists(nep_t* nep, int capA, int capS)
+{
+    const size_t n = (size_t)nep->n;
+    NEP_TRY(dev_alloc(nep, &nep->listA, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->rev, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->cA, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->pf, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->listS, (size_t)capS * n));
+    NEP_TRY(dev_alloc(nep, &nep->cB, (size_t)(capA + capS) * n));
+    nep->capA = capA;
+    nep->capS = capS;
+    nep->d.capA = capA;
+    nep->d.capS = capS;
+    return NEP_OK;
+}
+
+int alloc_atoms(nep_t* nep, int64_t n)
+{
+    const size_t N = (size_t)n;
+    const NepDims& d = nep->d;
+    NEP_TRY(dev_alloc(nep, &nep->type_orig, N));
+    NEP_TRY(dev_alloc(nep, &nep->perm, N));
+    NEP_TRY(dev_alloc(nep, &nep->posq, N));
+    NEP_TRY(dev_alloc(nep, &nep->posq_build, N));
+    NEP_TRY(dev_alloc(nep, &nep->cell_of, N));
+    NEP_TRY(dev_alloc(nep, &nep->rank_in_cell, N));
+    NEP_TRY(dev_alloc(nep, &nep->cntA, N));
+    NEP_TRY(dev_alloc(nep, &nep->cntS, N));
+    NEP_TRY(dev_alloc(nep, &nep->ncA, N));
+    NEP_TRY(dev_alloc(nep, &nep->ncB, N));
+    NEP_TRY(dev_alloc(nep, &nep->q, N * d.D));
+    NEP_TRY(dev_alloc(nep, &nep->fp, N * d.D));
+    NEP_TRY(dev_alloc(nep, &nep->S, N * d.NA * NEP_NUM_S));
+    NEP_TRY(dev_alloc(nep, &nep->Et, N * d.T * d.KRP));
+    NEP_TRY(dev_alloc(nep, &nep->U, N));
+    NEP_TRY(dev_alloc(nep, &nep->e_out, N));
+    NEP_TRY(dev_alloc(nep, &nep->f_out, 3 * N));
+    NEP_TRY(dev_alloc(nep, &nep->w_out, 9 * N));
+    nep->atom_cap = n;
+    nep->capA = nep->capS = 0;      // list storage is tied to n: force a re-allocation
+    return NEP_OK;
+}
+
+// ---- neighbour build (used by nep_neighbors and by md_step rebuilds) -----------------------------------
+int build_lists(nep_t* nep, const double* pos_dev)
+{
+    const int n = (int)nep->n;
+    cudaStream_t st = nep->stream;
+    const double rcut = nep->h.rc_radial + nep->skin, acut = nep->h.rc_angular + nep->skin;
+    BuildParams P;
+    P.n = n;
+    P.ncx = nep->ncell[0]; P.ncy = nep->ncell[1]; P.ncz = nep->ncell[2];
+    P.hx = P.hy = P.hz = 2;
+    P.Lx = nep->box[0]; P.Ly = nep->box[1]; P.Lz = nep->box[2];
+    P.inv_Lx = 1.0 / P.Lx; P.inv_Ly = 1.0 / P.Ly; P.inv_Lz = 1.0 / P.Lz;
+    P.sx = nep->d.sx; P.sy = nep->d.sy; P.sz = nep->d.sz;
+    P.cutA2_d = acut * acut; P.cutR2_d = rcut * rcut;
+    P.cutA2 = (float)P.cutA2_d; P.cutR2 = (float)P.cutR2_d;
+    const double Lmax = fmax(P.Lx, fmax(P.Ly, P.Lz));
+    // fp32/quantisation error of r^2 is < 2 r (3 L 2^-32 + r 2^-22); the band is ~100x wider
+    P.guardR = (float)(1e-4 * P.cutR2_d + 64.0 * Lmax * rcut / 4294967296.0);
+    P.guardA = (float)(1e-4 * P.cutA2_d + 64.0 * Lmax * acut / 4294967296.0);
+
+    const int TB = 256;
+    NEP_CUDA(cudaMemsetAsync(nep->cell_count, 0, sizeof(unsigned) * (size_t)(nep->n_cells + 1), st));
+    k_cell_hist<<<div_up(n, TB), TB, 0, st>>>(P, pos_dev, nep->cell_of, nep->rank_in_cell, nep->cell_count);
+    NEP_LAUNCH_CHECK();
+    {
+        const int64_t m = nep->n_cells + 1;
+        const int nb = div_up(m, SCAN_THREADS * SCAN_ITEMS);
+        k_scan_blocks<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_count, nep->cell_start, nep->scan_tmp, m);
+        NEP_LAUNCH_CHECK();
+        k_scan_totals<<<1, 1024, 0, st>>>(nep->scan_tmp, nb);
+        NEP_LAUNCH_CHECK();
+        k_scan_add<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_start, nep->scan_tmp, m);
+        NEP_LAUNCH_CHECK();
+    }
+    k_scatter<<<div_up(n, TB), TB, 0, st>>>(n, nep->cell_of, nep->rank_in_cell, nep->cell_start, nep->perm);
+    NEP_LAUNCH_CHECK();
+    k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm);
+    NEP_LAUNCH_CHECK();
+    k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, P.inv_Lx, P.inv_Ly, P.inv_Lz, nep->posq);
+    NEP_LAUNCH_CHECK();
+    NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+
+    if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
+        const double rho = (double)n / (P.Lx * P.Ly * P.Lz);
+        const double vA = 4.0 / 3.0 * 3.14159265358979 * acut * acut * acut, vR = 4.0 / 3.0 * 3.14159265358979 * rcut * rcut * rcut;
+        int capA = (int)(rho * vA * 1.25) + 12, capS = (int)(rho * (vR - vA) * 1.25) + 12;
+        if (capA > 256) capA = 256;
+        NEP_TRY(alloc_lists(nep, capA, capS));
+    }
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        P.capA = nep->capA; P.capS = nep->capS;
+        NEP_CUDA(cudaMemsetAsync(nep->flags, 0, sizeof(int) * 8, st));
+        k_build_lists<<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
+                                                    nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags);
+        NEP_LAUNCH_CHECK();
+        int fl[8];
+        NEP_CUDA(cudaMemcpyAsync(fl, nep->flags, sizeof(fl), cudaMemcpyDeviceToHost, st));
+        NEP_CUDA(cudaStreamSynchronize(st));
+        nep->maxA_skin = fl[2];
+        nep->maxR_skin = fl[3];
+        if (!fl[0] && !fl[1]) break;
+        if (fl[2] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours inside rc_angular + skin");
+        if (attempt == 3) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "neighbour lists kept overflowing");
+        int capA = nep->capA, capS = nep->capS;
+        if (fl[0]) capA = fl[2] + 8 > 256 ? 256 : fl[2] + 8;
+        if (fl[1]) capS = fl[4] + 8;
+        NEP_TRY(alloc_lists(nep, capA, capS));
+    }
+    k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA, nep->listA, nep->cntA, nep->rev);
+    NEP_LAUNCH_CHECK();
+    nep->steps_since_build = 0;
+    nep->have_lists = true;
+    return NEP_OK;
+}
+
+// ---- one evaluation of (a2)-(a8) into the internal output buffers ---------------------------------------
+template <int NR>
+int launch_radial(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KR * d.NRP;
+    NEP_TRY(allow_smem(nep, k_radial<NR>, sm));
+    k_radial<NR><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_t, nep->q);
+    NEP_LAUNCH_CHECK();
+    return NEP_OK;
+}
+
+int dispatch_radial(nep_t* nep)
+{
+    switch (nep->d.NR) {
+#define CASE(N) case N: return launch_radial<N>(nep);
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+        CASE(9) CASE(10) CASE(11) CASE(12) CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "n_max_radial out of range");
+}
+
+template <int NCH>
+int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int accumulate)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KA * d.NAP;
+    if (!force_pass) {
+        NEP_TRY(allow_smem(nep, k_angular<NCH>, sm));
+        k_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q);
+    } else {
+        NEP_TRY(allow_smem(nep, k_force_angular<NCH>, sm));
+        k_force_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->posq, nep->cA, nep->ncA,
+                                                                        nep->cA_t, nep->S, nep->fp, nep->pf);
+    }
+    NEP_LAUNCH_CHECK();
+    return NEP_OK;
+}
+
+int dispatch_angular(nep_t* nep, const NepCoef& C, bool force_pass)
+{
+    const int NA = nep->d.NA;
+    const int npass = (NA + NEP_NCH_MAX - 1) / NEP_NCH_MAX;
+    const int base = NA / npass, rem = NA % npass;
+    int n0 = 0;
+    for (int p = 0; p < npass; ++p) {
+        const int nch = base + (p < rem ? 1 : 0);
+        int rc;
+        switch (nch) {
+            case 1: rc = launch_angular<1>(nep, C, n0, force_pass, p > 0); break;
+            case 2: rc = launch_angular<2>(nep, C, n0, force_pass, p > 0); break;
+            case 3: rc = launch_angular<3>(nep, C, n0, force_pass, p > 0); break;
+            case 4: rc = launch_angular<4>(nep, C, n0, force_pass, p > 0); break;
+            default: rc = launch_angular<5>(nep, C, n0, force_pass, p > 0); break;
+        }
+        if (rc != NEP_OK) return rc;
+        n0 += nch;
+    }
+    return NEP_OK;
+}
+
+template <int DP>
+int launch_ann(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H);
+    NEP_TRY(allow_smem(nep, k_ann<DP>, sm));
+    k_ann<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
+                                                        nep->cR_e, nep->fp, nep->U, nep->Et);
+    NEP_LAUNCH_CHECK();
+    return NEP_OK;
+}
+
+int ann_tier(int D)
+{
+    const int tiers[] = {24, 40, 56, 72, 88, 104, 120};
+    for (int t : tiers) if (D <= t) return t;
+    return -1;
+}
+
+int dispatch_ann(nep_t* nep)
+{
+    switch (nep->DP) {
+        case 24: return launch_ann<24>(nep);
+        case 40: return launch_ann<40>(nep);
+        case 56: return launch_ann<56>(nep);
+        case 72: return launch_ann<72>(nep);
+        case 88: return launch_ann<88>(nep);
+        case 104: return launch_ann<104>(nep);
+        case 120: return launch_ann<120>(nep);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "descriptor too long");
+}
+
+int evaluate(nep_t* nep, const double* pos_dev)
+{
+    static const NepCoef C = make_coef();
+    const NepDims& d = nep->d;
+    const int n = d.n;
+    cudaStream_t st = nep->stream;
+    k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, 1.0 / nep->box[0], 1.0 / nep->box[1],
+                                               1.0 / nep->box[2], nep->posq);
+    NEP_LAUNCH_CHECK();
+    NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
+    k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
+                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->disp_max);
+    NEP_LAUNCH_CHECK();
+    NEP_TRY(dispatch_radial(nep));
+    NEP_TRY(dispatch_angular(nep, C, false));
+    NEP_TRY(dispatch_ann(nep));
+    NEP_TRY(dispatch_angular(nep, C, true));
+    k_final<<<div_up(n, 128), 128, 0, st>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->rev, nep->Et,
+                                            nep->pf, nep->U, nep->e_out, nep->f_out, nep->w_out);
+    NEP_LAUNCH_CHECK();
+    nep->have_eval = true;
+    return NEP_OK;
+}
+
+int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
+{
+    if (n <= 0 || n > NEP_MAX_ATOMS || !box || !(skin >= 0.0)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad n, box or skin");
+    for (int a = 0; a < 9; ++a)
+        if (a % 4 != 0 && box[a] != 0.0) return nep_fail(nep, NEP_ERR_UNSUPPORTED_BOX, "only orthorhombic boxes are supported");
+    const double L[3] = {box[0], box[4], box[8]};
+    const double rcut = nep->h.rc_radial + skin;
+    for (int a = 0; a < 3; ++a)
+        if (!(L[a] >= 2.0 * rcut)) return nep_fail(nep, NEP_ERR_BOX_TOO_SMALL, "box edge < 2 (rc_radial + skin)");
+    const bool same_n = (n == nep->n);
+    nep->skin = skin;
+    int64_t nc = 1;
+    const double cell_min = 0.5 * rcut * (1.0 + 1e-6);
+    for (int a = 0; a < 3; ++a) {
+        nep->box[a] = L[a];
+        int c = (int)floor(L[a] / cell_min);
+        if (c < 1) c = 1;
+        if (c > 1024) c = 1024;
+        nep->ncell[a] = c;
+        nc *= c;
+    }
+    nep->n_cells = nc;
+    nep->d.sx = (float)(L[0] / 4294967296.0);
+    nep->d.sy = (float)(L[1] / 4294967296.0);
+    nep->d.sz = (float)(L[2] / 4294967296.0);
+    if (!same_n || n > nep->atom_cap) {
+        nep->n = n;
+        nep->d.n = (int)n;
+        NEP_TRY(alloc_atoms(nep, n));
+    }
+    if (nc + 1 > nep->cell_cap) {
+        NEP_TRY(dev_alloc(nep, &nep->cell_count, (size_t)nc + 1));
+        NEP_TRY(dev_alloc(nep, &nep->cell_start, (size_t)nc + 1));
+        nep->cell_cap = nc + 1;
+    }
+    const int64_t nb = div_up(nc + 1, SCAN_THREADS * SCAN_ITEMS);
+    if (nb > nep->scan_cap) {
+        NEP_TRY(dev_alloc(nep, &nep->scan_tmp, (size_t)nb));
+        nep->scan_cap = nb;
+    }
+    return NEP_OK;
+}
+
+}  // namespace
+
+// =======================================================================================================
+extern "C" {
+
+const char* nep_status_string(int status)
+{
+    switch (status) {
+        case NEP_OK: return "ok";
+        case NEP_ERR_INVALID_ARG: return "invalid argument";
+        case NEP_ERR_BOX_TOO_SMALL: return "box too small for the cutoff (minimum image)";
+        case NEP_ERR_UNSUPPORTED_BOX: return "unsupported (non-orthorhombic) box";
+        case NEP_ERR_NEIGHBOR_OVERFLOW: return "neighbour list overflow";
+        case NEP_ERR_STATE: return "call out of order";
+        case NEP_ERR_CUDA: return "CUDA error";
+        case NEP_ERR_NOMEM: return "out of memory";
+    }
+    return "unknown status";
+}
+
+const char* nep_last_error(const nep_t* nep) { return nep ? nep->err : "null handle"; }
+
+int64_t nep_launch_count(const nep_t* nep) { return nep ? nep->launches : 0; }
+
+int nep_num_descriptors(const nep_hyper_t* h)
+{
+    const int rc = validate_hyper(h);
+    return rc != NEP_OK ? rc : n_des(h);
+}
+
+int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const float* c_angular,
+               const float* w0, const float* b0, const float* w1, const float* b1,
+               const double* mass_amu, int device, void* cuda_stream)
+{
+    if (!out) return NEP_ERR_INVALID_ARG;
+    *out = nullptr;
+    int rc = validate_hyper(h);
+    if (rc != NEP_OK) return rc;
+    if (!c_radial || !c_angular || !w0 || !b0 || !w1 || !b1 || !mass_amu) return NEP_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return NEP_ERR_CUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_CUDA; }
+
+    nep_t* nep = new (std::nothrow) nep_ctx();
+    if (!nep) return NEP_ERR_NOMEM;
+    memset(nep, 0, sizeof(*nep));
+    nep->h = *h;
+    nep->device = device;
+    nep->stream = (cudaStream_t)cuda_stream;
+    NepDims& d = nep->d;
+    d.T = h->n_types; d.NR = h->n_max_radial + 1; d.KR = h->basis_radial + 1;
+    d.NA = h->n_max_angular + 1; d.KA = h->basis_angular + 1;
+    d.D = n_des(h); d.H = h->n_neurons;
+    d.NRP = round_up4(d.NR); d.NAP = round_up4(d.NA); d.KRP = round_up4(d.KR);
+    d.has4 = h->l_max_4b >= 2; d.has5 = h->l_max_5b >= 1; d.nblk = 4 + d.has4 + d.has5;
+    d.rcR = (float)h->rc_radial; d.rcA = (float)h->rc_angular;
+    d.rcR_inv = (float)(1.0 / h->rc_radial); d.rcA_inv = (float)(1.0 / h->rc_angular);
+    d.rcR2 = d.rcR * d.rcR; d.rcA2 = d.rcA * d.rcA;
+    nep->DP = ann_tier(d.D);
+    if (nep->DP < 0) { delete nep; return NEP_ERR_INVALID_ARG; }
+    for (int t = 0; t < d.T; ++t) {
+        if (!(mass_amu[t] > 0.0)) { delete nep; return NEP_ERR_INVALID_ARG; }
+        nep->mass[t] = mass_amu[t];
+    }
+
+    // re-laid-out parameter tables
+    const int T = d.T, TT = T * T;
+    std::vector<float> cRt((size_t)TT * d.KR * d.NRP, 0.0f), cAt((size_t)TT * d.KA * d.NAP, 0.0f);
+    std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
+    for (int tt = 0; tt < TT; ++tt) {
+        for (int nn = 0; nn < d.NR; ++nn)
+            for (int k = 0; k < d.KR; ++k) {
+                const float v = c_radial[((size_t)tt * d.NR + nn) * d.KR + k];
+                cRt[((size_t)tt * d.KR + k) * d.NRP + nn] = v;
+                cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
+            }
+        for (int nn = 0; nn < d.NA; ++nn)
+            for (int k = 0; k < d.KA; ++k)
+                cAt[((size_t)tt * d.KA + k) * d.NAP + nn] = c_angular[((size_t)tt * d.NA + nn) * d.KA + k];
+    }
+    for (int m = 0; m < d.H; ++m)
+        for (int v = 0; v < d.D; ++v) w0p[(size_t)m * nep->DP + v] = w0[(size_t)m * d.D + v];
+    nep->b1 = b1[0];
+
+#define UPLOAD(dst, vec)                                                                          \
+    do {                                                                                          \
+        rc = dev_alloc(nep, &nep->dst, (vec).size());                                             \
+        if (rc == NEP_OK && cudaMemcpy(nep->dst, (vec).data(), (vec).size() * sizeof((vec)[0]),   \
+                                       cudaMemcpyHostToDevice) != cudaSuccess) rc = NEP_ERR_CUDA; \
+        if (rc != NEP_OK) { nep_destroy(nep); return rc; }                                        \
+    } while (0)
+    UPLOAD(cR_t, cRt);
+    UPLOAD(cA_t, cAt);
+    UPLOAD(cR_e, cRe);
+    UPLOAD(w0p, w0p);
+    std::vector<float> vb0(b0, b0 + d.H), vw1(w1, w1 + d.H);
+    UPLOAD(b0, vb0);
+    UPLOAD(w1, vw1);
+    std::vector<double> vm(nep->mass, nep->mass + d.T);
+    UPLOAD(mass_dev, vm);
+#undef UPLOAD
+    rc = dev_alloc(nep, &nep->flags, 8);
+    if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 1);
+    if (rc != NEP_OK) { nep_destroy(nep); return rc; }
+    cudaMemset(nep->disp_max, 0, sizeof(unsigned));
+    if (cudaDeviceSynchronize() != cudaSuccess) { nep_destroy(nep); return NEP_ERR_CUDA; }
+    *out = nep;
+    return NEP_OK;
+}
+
+int nep_destroy(nep_t* nep)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    cudaSetDevice(nep->device);
+    cudaStreamSynchronize(nep->stream);
+    void* ptrs[] = {nep->cR_t, nep->cA_t, nep->cR_e, nep->w0p, nep->b0, nep->w1, nep->mass_dev, nep->type_orig, nep->perm,
+                    nep->posq, nep->posq_build, nep->cell_of, nep->rank_in_cell, nep->order_tmp, nep->cell_count,
+                    nep->cell_start, nep->scan_tmp, nep->listA, nep->cntA, nep->listS, nep->cntS, nep->rev, nep->cA,
+                    nep->ncA, nep->cB, nep->ncB, nep->flags, nep->disp_max, nep->q, nep->fp, nep->S, nep->Et, nep->U,
+                    nep->pf, nep->e_out, nep->f_out, nep->w_out};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    cudaGetLastError();
+    delete nep;
+    return NEP_OK;
+}
+
+int nep_neighbors(nep_t* nep, int64_t n, const double* pos_dev, const int32_t* type_dev, const double box[9], double skin)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_dev || !type_dev) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    nep->have_lists = nep->have_eval = nep->force_current = false;
+    NEP_TRY(setup_system(nep, n, box, skin));
+    NEP_CUDA(cudaMemcpyAsync(nep->type_orig, type_dev, sizeof(int) * (size_t)n, cudaMemcpyDeviceToDevice, nep->stream));
+    return build_lists(nep, pos_dev);
+}
+
+int nep_max_neighbors(nep_t* nep, int which, int32_t* max_count_host)
+{
+    if (!nep || !max_count_host || (which != 0 && which != 1)) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    *max_count_host = which == 0 ? nep->maxR_skin : nep->maxA_skin;
+    return NEP_OK;
+}
+
+int nep_get_neighbors(nep_t* nep, int which, int32_t* count_dev, int32_t* list_dev, int32_t cap)
+{
+    if (!nep || !count_dev || !list_dev || (which != 0 && which != 1)) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    if (cap < (which == 0 ? nep->maxR_skin : nep->maxA_skin)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "cap smaller than the longest list");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    k_export_lists<<<div_up(n, 128), 128, 0, nep->stream>>>(n, which, nep->perm, nep->listA, nep->cntA, nep->listS, nep->cntS,
+                                                          count_dev, list_dev, cap);
+    NEP_LAUNCH_CHECK();
+    return NEP_OK;
+}
+
+int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* virial_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const size_t n = (size_t)nep->n;
+    if (energy_dev) NEP_CUDA(cudaMemcpyAsync(energy_dev, nep->e_out, sizeof(double) * n, cudaMemcpyDeviceToDevice, nep->stream));
+    if (force_dev) NEP_CUDA(cudaMemcpyAsync(force_dev, nep->f_out, sizeof(double) * 3 * n, cudaMemcpyDeviceToDevice, nep->stream));
+    if (virial_dev) NEP_CUDA(cudaMemcpyAsync(virial_dev, nep->w_out, sizeof(double) * 9 * n, cudaMemcpyDeviceToDevice, nep->stream));
+    return NEP_OK;
+}
+
+int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* force_dev, double* virial_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_dev) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    NEP_TRY(evaluate(nep, pos_dev));
+    nep->force_current = true;
+    nep->force_pos_tag = pos_dev;
+    return nep_get_last(nep, energy_dev, force_dev, virial_dev);
+}
+
+int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_dev || !vel_dev || n_steps < 0 || rebuild_every < 1 || !(skin >= 0.0) || !(dt_fs == dt_fs))
+        return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad md_step argument");
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    cudaStream_t st = nep->stream;
+    if (skin != nep->skin) {
+        // a different skin takes effect at once: lists are rebuilt for the current positions
+        const double box9[9] = {nep->box[0], 0, 0, 0, nep->box[1], 0, 0, 0, nep->box[2]};
+        NEP_TRY(setup_system(nep, nep->n, box9, skin));
+        NEP_TRY(build_lists(nep, pos_dev));
+        nep->force_current = false;
+    }
+    if (!nep->force_current || nep->force_pos_tag != pos_dev) NEP_TRY(evaluate(nep, pos_dev));
+    const double hdt = 0.5 * dt_fs * kAccConv;
+    const int TB = 256;
+    for (int s = 0; s < n_steps; ++s) {
+        k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev);
+        NEP_LAUNCH_CHECK();
+        nep->steps_since_build++;
+        if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
+        NEP_TRY(evaluate(nep, pos_dev));
+        k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev);
+        NEP_LAUNCH_CHECK();
+    }
+    nep->force_current = true;
+    nep->force_pos_tag = pos_dev;
+    return NEP_OK;
+}
+
+int nep_max_displacement(nep_t* nep, double* disp_host)
+{
+    if (!nep || !disp_host) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    unsigned bits = 0;
+    NEP_CUDA(cudaMemcpyAsync(&bits, nep->disp_max, sizeof(bits), cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    float r2;
+    memcpy(&r2, &bits, sizeof(r2));
+    *disp_host = sqrt((double)r2);
+    return NEP_OK;
+}
+
+int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    if (q_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->q, q_dev); NEP_LAUNCH_CHECK(); }
+    if (fp_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->fp, fp_dev); NEP_LAUNCH_CHECK(); }
+    return NEP_OK;
+}
+
+int nep_get_angular_sums(nep_t* nep, float* S_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    if (S_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.NA * NEP_NUM_S, nep->perm, nep->S, S_dev); NEP_LAUNCH_CHECK(); }
+    return NEP_OK;
+}
+
+// ---- host-buffer entry points ---------------------------------------------------------------------------
+static int stage_alloc(nep_t* nep, int64_t n, double** pos, double** vel, int** type)
+{
+    // staging buffers live for one call: simple and leak-free; the copies dominate anyway
+    *pos = nullptr; *type = nullptr;
+    if (vel) *vel = nullptr;
+    if (cudaMalloc((void**)pos, sizeof(double) * 3 * (size_t)n) != cudaSuccess ||
+        (vel && cudaMalloc((void**)vel, sizeof(double) * 3 * (size_t)n) != cudaSuccess) ||
+        cudaMalloc((void**)type, sizeof(int) * (size_t)n) != cudaSuccess) {
+        cudaGetLastError();
+        if (*pos) cudaFree(*pos);
+        if (vel && *vel) cudaFree(*vel);
+        if (*type) cudaFree(*type);
+        return nep_fail(nep, NEP_ERR_NOMEM, "staging allocation failed");
+    }
+    return NEP_OK;
+}
+
+static int download_results(nep_t* nep, double* energy_host, double* force_host, double* virial_host)
+{
+    const size_t n = (size_t)nep->n;
+    if (energy_host) NEP_CUDA(cudaMemcpyAsync(energy_host, nep->e_out, sizeof(double) * n, cudaMemcpyDeviceToHost, nep->stream));
+    if (force_host) NEP_CUDA(cudaMemcpyAsync(force_host, nep->f_out, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, nep->stream));
+    if (virial_host) NEP_CUDA(cudaMemcpyAsync(virial_host, nep->w_out, sizeof(double) * 9 * n, cudaMemcpyDeviceToHost, nep->stream));
+    return NEP_OK;
+}
+
+int nep_compute_host(nep_t* nep, int64_t n, const double* pos_host, const int32_t* type_host, const double box[9],
+                     double skin, double* energy_host, double* force_host, double* virial_host)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_host || !type_host || n <= 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n <= 0");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    double* pos; int* type;
+    NEP_TRY(stage_alloc(nep, n, &pos, nullptr, &type));
+    int rc = NEP_OK;
+    if (cudaMemcpyAsync(pos, pos_host, sizeof(double) * 3 * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
+        cudaMemcpyAsync(type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess)
+        rc = nep_fail(nep, NEP_ERR_CUDA, "H2D copy failed");
+    if (rc == NEP_OK) rc = nep_neighbors(nep, n, pos, type, box, skin);
+    if (rc == NEP_OK) rc = evaluate(nep, pos);
+    if (rc == NEP_OK) rc = download_results(nep, energy_host, force_host, virial_host);
+    if (cudaStreamSynchronize(nep->stream) != cudaSuccess && rc == NEP_OK) rc = nep_fail(nep, NEP_ERR_CUDA, "stream sync failed");
+    nep->force_current = false;
+    cudaFree(pos); cudaFree(type);
+    return rc;
+}
+
+int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const int32_t* type_host, const double box[9],
+                double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin,
+                double* energy_host, double* force_host, double* virial_host)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_host || !vel_host || !type_host || n <= 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n <= 0");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    double *pos, *vel; int* type;
+    NEP_TRY(stage_alloc(nep, n, &pos, &vel, &type));
+    int rc = NEP_OK;
+    const size_t b3 = sizeof(double) * 3 * (size_t)n;
+    if (cudaMemcpyAsync(pos, pos_host, b3, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
+        cudaMemcpyAsync(vel, vel_host, b3, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
+        cudaMemcpyAsync(type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess)
+        rc = nep_fail(nep, NEP_ERR_CUDA, "H2D copy failed");
+    if (rc == NEP_OK) rc = nep_neighbors(nep, n, pos, type, box, skin);
+    if (rc == NEP_OK) rc = md_step(nep, pos, vel, dt_fs, n_steps, rebuild_every, skin);
+    if (rc == NEP_OK &&
+        (cudaMemcpyAsync(pos_host, pos, b3, cudaMemcpyDeviceToHost, nep->stream) != cudaSuccess ||
+         cudaMemcpyAsync(vel_host, vel, b3, cudaMemcpyDeviceToHost, nep->stream) != cudaSuccess))
+        rc = nep_fail(nep, NEP_ERR_CUDA, "D2H copy failed");
+    if (rc == NEP_OK) rc = download_results(nep, energy_host, force_host, virial_host);
+    if (cudaStreamSynchronize(nep->stream) != cudaSuccess && rc == NEP_OK) rc = nep_fail(nep, NEP_ERR_CUDA, "stream sync failed");
+    nep->force_current = false;      // the staging buffers die with this call
+    cudaFree(pos); cudaFree(vel); cudaFree(type);
+    return rc;
+}
+
+}  // extern "C"

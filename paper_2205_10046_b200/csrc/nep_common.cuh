@@ -1,0 +1,173 @@
+// nep_common.cuh -- context, device-side constants and small device helpers shared by the kernels
+// of the B200-native NEP3 library.  (Product code: shares nothing with oracle/.)
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/nep.h"
+
+#define NEP_MAX_TYPES 16
+#define NEP_NUM_S 24            // sums S_{n,k}, k = 0..23 (Eq. 12)
+#define NEP_NCH_MAX 5           // angular n-values handled per pass (24*5 accumulators in registers)
+#define NEP_SLOT_BITS 8         // packed angular entry: (j << 8) | skin slot
+#define NEP_MAX_ATOMS (1 << 24)
+
+// ---------------------------------------------------------------------------------------------------
+// Scalars every kernel needs; passed by value as a kernel argument (lives in the constant bank).
+struct NepDims {
+    int n;                       // atoms
+    int T, NR, KR, NA, KA, D, H;
+    int NRP, NAP;                // NR, NA rounded up to a multiple of 4 (row stride of the c tables)
+    int KRP;                     // KR rounded up to 4 (row stride of the per-atom E table)
+    int nblk, has4, has5;        // descriptor blocks after the radial one; 4-/5-body present
+    float rcR, rcA, rcR_inv, rcA_inv, rcR2, rcA2;
+    float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
+    int capA, capS;              // storage rows of the skin lists (angular-range part, outer shell)
+};
+
+struct nep_ctx {
+    nep_hyper_t h;
+    NepDims d;
+    int device;
+    cudaStream_t stream;
+    char err[512];
+    int64_t launches;
+
+    // model (device)
+    float* cR_t;     // [T*T][KR][NRP]   c_radial transposed so that the n-values of one k are contiguous
+    float* cA_t;     // [T*T][KA][NAP]
+    float* cR_e;     // [T(ti)][T(tj)][NR][KRP]  for the per-atom E table
+    float* w0p;      // [H][DP] rows padded with zeros to DP
+    float* b0;       // [H]
+    float* w1;       // [H]
+    float b1;
+    int DP;          // descriptor length padded to the ANN kernel's tier
+    double mass[NEP_MAX_TYPES];
+    double* mass_dev;
+
+    // system
+    int64_t n;
+    double box[3];
+    double skin;
+    int ncell[3];
+    int64_t n_cells;
+    bool have_lists;
+    bool have_eval;          // internal E/F/W hold an evaluation
+    bool force_current;      // ... and it belongs to the positions md_step will continue from
+    const double* force_pos_tag;
+    int steps_since_build;
+    int maxA_skin, maxR_skin;   // list sizes of the last build (angular-range part; radial = A + shell)
+
+    // per-atom (device); "sorted" = internal spatial order, "orig" = caller's order
+    int* type_orig;          // [n]
+    int* perm;               // [n] sorted -> orig
+    int4* posq;              // [n] sorted: quantised x,y,z (units of L/2^32) + type
+    int4* posq_build;        // [n] copy at the last build (displacement check)
+    unsigned* cell_of;       // [n] orig: cell id        (build scratch)
+    unsigned* rank_in_cell;  // [n] orig                 (build scratch)
+    int* order_tmp;          // [n]                      (build scratch)
+    unsigned* cell_count;    // [n_cells + 1]
+    unsigned* cell_start;    // [n_cells + 1]
+    unsigned* scan_tmp;      // block totals
+    int64_t cell_cap, scan_cap;
+
+    int capA, capS;          // allocated rows
+    int* listA;  int* cntA;  // [capA][n] sorted indices with |r| < rcA + skin
+    int* listS;  int* cntS;  // [capS][n] rcA + skin <= |r| < rcR + skin
+    unsigned char* rev;      // [capA][n] slot of i in j's listA
+    int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|slot with |r| < rcA
+    int* cB; int* ncB;       // [capA+capS][n] per step: j with rcA <= |r| < rcR
+    int* flags;              // [4] device: 0 overflow A, 1 overflow S, 2 max cntA, 3 max (cntA+cntS)
+    unsigned* disp_max;      // [1] device: float bits of max displacement^2 since build
+    int64_t atom_cap;        // allocated atoms
+
+    float* q;                // [D][n]
+    float* fp;               // [D][n]
+    float* S;                // [NA*24][n]
+    float* Et;               // [n][T][KRP]  E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
+    float* U;                // [n]
+    float4* pf;              // [capA][n] angular partial forces dU_i/dr_ij at skin slots
+    double* e_out;           // [n]    orig order
+    double* f_out;           // [n][3]
+    double* w_out;           // [n][9]
+};
+
+// ---------------------------------------------------------------------------------------------------
+#define NEP_CUDA(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            snprintf(nep->err, sizeof(nep->err), "%s:%d: %s: %s", __FILE__, __LINE__, #call,        \
+                     cudaGetErrorString(e_));                                                       \
+            return NEP_ERR_CUDA;                                                                    \
+        }                                                                                           \
+    } while (0)
+
+#define NEP_LAUNCH_CHECK()                                                                          \
+    do {                                                                                            \
+        nep->launches++;                                                                            \
+        cudaError_t e_ = cudaGetLastError();                                                        \
+        if (e_ != cudaSuccess) {                                                                    \
+            snprintf(nep->err, sizeof(nep->err), "%s:%d: launch: %s", __FILE__, __LINE__,           \
+                     cudaGetErrorString(e_));                                                       \
+            return NEP_ERR_CUDA;                                                                    \
+        }                                                                                           \
+    } while (0)
+
+static inline int nep_fail(nep_t* nep, int status, const char* msg)
+{
+    if (nep) snprintf(nep->err, sizeof(nep->err), "%s", msg);
+    return status;
+}
+
+static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+static inline int round_up4(int a) { return (a + 3) & ~3; }
+
+// ---------------------------------------------------------------------------------------------------
+// Pair geometry from quantised coordinates.  Positions are stored as 32-bit fractions of the box edge,
+// so the wrapped integer difference IS the minimum image (exact, branch-free); the result is converted
+// to Angstrom in fp32.  d = r_j - r_i.  dx(i,j) = -dx(j,i) bit for bit, so r2 is the same
+// for both orderings of a pair and both atoms take the same in-cutoff decision.
+__device__ __forceinline__ void pair_vec(const int4& pi, const int4& pj, const NepDims& D,
+                                         float& dx, float& dy, float& dz, float& r2)
+{
+    dx = (float)(int)((unsigned)pj.x - (unsigned)pi.x) * D.sx;
+    dy = (float)(int)((unsigned)pj.y - (unsigned)pi.y) * D.sy;
+    dz = (float)(int)((unsigned)pj.z - (unsigned)pi.z) * D.sz;
+    r2 = dx * dx + dy * dy + dz * dz;
+}
+
+// Cutoff function Eq. (5) and the Chebyshev argument of Eq. (4).
+// f_k(r) = 1/2 [T_k(x)+1] f_c(r), x = 2 (r/rc - 1)^2 - 1.  The recurrence state is advanced by the
+// caller: T_{k+1} = 2 x T_k - T_{k-1};  T_k' = k U_{k-1}, U_{k+1} = 2 x U_k - U_{k-1}.
+struct BasisHead {
+    float x, two_x;       // Chebyshev argument
+    float hfc;            // f_c / 2
+    float hdfc;           // f_c' / 2
+    float hfc_dx;         // (f_c / 2) * dx/dr
+};
+
+template <bool WITH_DERIV>
+__device__ __forceinline__ BasisHead basis_head(float r, float rc_inv)
+{
+    BasisHead b;
+    float t = r * rc_inv;
+    float y = t - 1.0f;
+    b.x = 2.0f * y * y - 1.0f;
+    b.two_x = 2.0f * b.x;
+    if (WITH_DERIV) {
+        float s, c;
+        sincospif(t, &s, &c);
+        b.hfc = 0.25f * c + 0.25f;
+        b.hdfc = -0.25f * 3.14159265358979323846f * rc_inv * s;
+        b.hfc_dx = b.hfc * (4.0f * y * rc_inv);
+    } else {
+        b.hfc = 0.25f * cospif(t) + 0.25f;
+        b.hdfc = 0.0f;
+        b.hfc_dx = 0.0f;
+    }
+    return b;
+}

@@ -1,0 +1,272 @@
+// nep_neighbor.cuh -- (a1) cell-binned construction of the radial and angular Verlet lists.
+//
+// The paper takes the lists NN^R/NL^R, NN^A/NL^A as inputs and does not describe
+// their construction; this is the B200 design:
+//   1. positions -> 32-bit box fractions; cell id from the top bits; histogram (atomics)
+//   2. exclusive scan of the histogram (own 3-kernel scan)
+//   3. scatter + per-cell sort by atom index  => deterministic spatial order `perm`
+//   4. one thread per atom walks the 5x5x5 stencil rows (contiguous ranges of sorted atoms),
+//      tests candidates in fp32 and resolves anything inside a guard band around a cutoff with the
+//      exact fp64 predicate of reading A8, so the sets equal an fp64 brute force bit for bit
+//   5. reverse index: slot of i in j's angular list (for the scatter-free gather of Eq. 22-24)
+// The angular-range list (|r| < rcA+skin) and the outer shell (rcA+skin <= |r| < rcR+skin) are stored
+// disjointly; the radial list is their union.
+#pragma once
+#include "nep_common.cuh"
+
+struct BuildParams {
+    int n;
+    int ncx, ncy, ncz;
+    int hx, hy, hz;          // stencil half widths (2) -- or "all cells" when 2h+1 >= nc
+    double Lx, Ly, Lz;
+    double inv_Lx, inv_Ly, inv_Lz;
+    float sx, sy, sz;
+    float cutA2, cutR2;      // (rcA+skin)^2, (rcR+skin)^2 in fp32 (fast test)
+    float guardA, guardR;    // half width of the fp64-resolve band around each
+    double cutA2_d, cutR2_d; // exact fp64 thresholds rc*rc
+    int capA, capS;
+};
+
+__device__ __forceinline__ unsigned quantize_frac(double x, double inv_L)
+{
+    double f = x * inv_L;
+    f -= floor(f);
+    return (unsigned)(unsigned long long)(f * 4294967296.0);
+}
+
+__device__ __forceinline__ int cell_coord(unsigned q, int nc) { return (int)(((unsigned long long)q * (unsigned)nc) >> 32); }
+
+// ---- 1. cell id + histogram ------------------------------------------------------------------------
+__global__ void k_cell_hist(BuildParams P, const double* __restrict__ pos, unsigned* __restrict__ cell_of,
+                            unsigned* __restrict__ rank_in_cell, unsigned* __restrict__ cell_count)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    unsigned qx = quantize_frac(pos[3 * (size_t)i + 0], P.inv_Lx);
+    unsigned qy = quantize_frac(pos[3 * (size_t)i + 1], P.inv_Ly);
+    unsigned qz = quantize_frac(pos[3 * (size_t)i + 2], P.inv_Lz);
+    unsigned c = ((unsigned)cell_coord(qz, P.ncz) * P.ncy + cell_coord(qy, P.ncy)) * P.ncx + cell_coord(qx, P.ncx);
+    cell_of[i] = c;
+    rank_in_cell[i] = atomicAdd(&cell_count[c], 1u);
+}
+
+// ---- 2. exclusive scan (3 kernels, 1024 items per block) -------------------------------------------
+#define SCAN_ITEMS 4
+#define SCAN_THREADS 256
+__global__ void k_scan_blocks(const unsigned* __restrict__ in, unsigned* __restrict__ out,
+                              unsigned* __restrict__ block_tot, int64_t n)
+{
+    __shared__ unsigned warp_tot[SCAN_THREADS / 32];
+    int64_t base = ((int64_t)blockIdx.x * SCAN_THREADS + threadIdx.x) * SCAN_ITEMS;
+    unsigned v[SCAN_ITEMS], sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? in[base + k] : 0u; sum += v[k]; }
+    unsigned incl = sum;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+    if (lane == 31) warp_tot[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+        unsigned t = (lane < SCAN_THREADS / 32) ? warp_tot[lane] : 0u, inc = t;
+#pragma unroll
+        for (int o = 1; o < SCAN_THREADS / 32; o <<= 1) { unsigned u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+        if (lane < SCAN_THREADS / 32) warp_tot[lane] = inc - t;      // exclusive warp offsets
+        if (lane == SCAN_THREADS / 32 - 1) block_tot[blockIdx.x] = inc;
+    }
+    __syncthreads();
+    unsigned run = warp_tot[w] + incl - sum;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { if (base + k < n) out[base + k] = run; run += v[k]; }
+}
+
+__global__ void k_scan_totals(unsigned* __restrict__ block_tot, int nblocks)
+{
+    // one block; serial over chunks of blockDim.x with a running carry
+    __shared__ unsigned sh[1024];
+    __shared__ unsigned carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < nblocks; base += blockDim.x) {
+        int i = base + threadIdx.x;
+        unsigned v = (i < nblocks) ? block_tot[i] : 0u;
+        sh[threadIdx.x] = v;
+        __syncthreads();
+        for (int o = 1; o < (int)blockDim.x; o <<= 1) {
+            unsigned t = (threadIdx.x >= (unsigned)o) ? sh[threadIdx.x - o] : 0u;
+            __syncthreads();
+            sh[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < nblocks) block_tot[i] = carry + sh[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry += sh[threadIdx.x];
+        __syncthreads();
+    }
+}
+
+__global__ void k_scan_add(unsigned* __restrict__ out, const unsigned* __restrict__ block_tot, int64_t n)
+{
+    int64_t base = ((int64_t)blockIdx.x * SCAN_THREADS + threadIdx.x) * SCAN_ITEMS;
+    unsigned add = block_tot[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) out[base + k] += add;
+}
+
+// ---- 3. scatter, per-cell sort by atom index, quantised sorted positions ----------------------------
+__global__ void k_scatter(int n, const unsigned* __restrict__ cell_of, const unsigned* __restrict__ rank_in_cell,
+                          const unsigned* __restrict__ cell_start, int* __restrict__ order_tmp)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    order_tmp[cell_start[cell_of[i]] + rank_in_cell[i]] = i;
+}
+
+__global__ void k_sort_cells(int64_t n_cells, const unsigned* __restrict__ cell_start, int* __restrict__ order_tmp)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cells) return;
+    int lo = (int)cell_start[c], hi = (int)cell_start[c + 1];
+    for (int a = lo + 1; a < hi; ++a) {              // insertion sort: a cell holds a handful of atoms
+        int v = order_tmp[a], b = a - 1;
+        while (b >= lo && order_tmp[b] > v) { order_tmp[b + 1] = order_tmp[b]; --b; }
+        order_tmp[b + 1] = v;
+    }
+}
+
+// sorted quantised positions from the caller's fp64 positions (also used every step)
+__global__ void k_quantize(int n, const double* __restrict__ pos, const int* __restrict__ type_orig,
+                           const int* __restrict__ perm, double inv_Lx, double inv_Ly, double inv_Lz,
+                           int4* __restrict__ posq)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int i = perm[s];
+    int4 q;
+    q.x = (int)quantize_frac(pos[3 * (size_t)i + 0], inv_Lx);
+    q.y = (int)quantize_frac(pos[3 * (size_t)i + 1], inv_Ly);
+    q.z = (int)quantize_frac(pos[3 * (size_t)i + 2], inv_Lz);
+    q.w = type_orig[i];
+    posq[s] = q;
+}
+
+// ---- 4. list build -----------------------------------------------------------------------------------
+// exact predicate of reading A8, literally: d = (rj - ri) - L*rint((rj - ri)/L);
+// d2 = (dx*dx + dy*dy) + dz*dz; all IEEE fp64 round-to-nearest, no FMA contraction.
+__device__ __forceinline__ double exact_d2(const double* __restrict__ pos, int i, int j, const BuildParams& P)
+{
+    double tx = __dsub_rn(pos[3 * (size_t)j + 0], pos[3 * (size_t)i + 0]);
+    double ty = __dsub_rn(pos[3 * (size_t)j + 1], pos[3 * (size_t)i + 1]);
+    double tz = __dsub_rn(pos[3 * (size_t)j + 2], pos[3 * (size_t)i + 2]);
+    tx = __dsub_rn(tx, __dmul_rn(P.Lx, rint(__ddiv_rn(tx, P.Lx))));
+    ty = __dsub_rn(ty, __dmul_rn(P.Ly, rint(__ddiv_rn(ty, P.Ly))));
+    tz = __dsub_rn(tz, __dmul_rn(P.Lz, rint(__ddiv_rn(tz, P.Lz))));
+    return __dadd_rn(__dadd_rn(__dmul_rn(tx, tx), __dmul_rn(ty, ty)), __dmul_rn(tz, tz));
+}
+
+__global__ void __launch_bounds__(128)
+k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restrict__ perm,
+              const int4* __restrict__ posq, const unsigned* __restrict__ cell_start,
+              int* __restrict__ listA, int* __restrict__ cntA, int* __restrict__ listS, int* __restrict__ cntS,
+              int* __restrict__ flags)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n) return;
+    const int4 pi = posq[s];
+    const int cx = cell_coord((unsigned)pi.x, P.ncx);
+    const int cy = cell_coord((unsigned)pi.y, P.ncy);
+    const int cz = cell_coord((unsigned)pi.z, P.ncz);
+    const bool allx = 2 * P.hx + 1 >= P.ncx, ally = 2 * P.hy + 1 >= P.ncy, allz = 2 * P.hz + 1 >= P.ncz;
+    const int nz = allz ? P.ncz : 2 * P.hz + 1, ny = ally ? P.ncy : 2 * P.hy + 1;
+    int na = 0, ns = 0;
+    const size_t n = (size_t)P.n;
+
+    for (int iz = 0; iz < nz; ++iz) {
+        int zc = allz ? iz : cz - P.hz + iz;
+        if (zc < 0) zc += P.ncz; else if (zc >= P.ncz) zc -= P.ncz;
+        for (int iy = 0; iy < ny; ++iy) {
+            int yc = ally ? iy : cy - P.hy + iy;
+            if (yc < 0) yc += P.ncy; else if (yc >= P.ncy) yc -= P.ncy;
+            const unsigned row = ((unsigned)zc * P.ncy + yc) * P.ncx;
+            // x range(s) of this row: contiguous in the sorted order
+            int r0a, r0b, r1a = 0, r1b = -1;
+            if (allx) { r0a = 0; r0b = P.ncx - 1; }
+            else {
+                int lo = cx - P.hx, hi = cx + P.hx;
+                if (lo < 0) { r0a = lo + P.ncx; r0b = P.ncx - 1; r1a = 0; r1b = hi; }
+                else if (hi >= P.ncx) { r0a = lo; r0b = P.ncx - 1; r1a = 0; r1b = hi - P.ncx; }
+                else { r0a = lo; r0b = hi; }
+            }
+            for (int part = 0; part < 2; ++part) {
+                const int ca = part ? r1a : r0a, cb = part ? r1b : r0b;
+                if (cb < ca) continue;
+                const int t0 = (int)cell_start[row + ca], t1 = (int)cell_start[row + cb + 1];
+                for (int t = t0; t < t1; ++t) {
+                    if (t == s) continue;
+                    const int4 pj = posq[t];
+                    float dx = (float)(int)((unsigned)pj.x - (unsigned)pi.x) * P.sx;
+                    float dy = (float)(int)((unsigned)pj.y - (unsigned)pi.y) * P.sy;
+                    float dz = (float)(int)((unsigned)pj.z - (unsigned)pi.z) * P.sz;
+                    float r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 >= P.cutR2 + P.guardR) continue;
+                    bool inR = r2 < P.cutR2 - P.guardR;
+                    bool inA = r2 < P.cutA2 - P.guardA;
+                    const bool nearR = !inR;                                    // within the R guard band
+                    const bool nearA = !inA && r2 < P.cutA2 + P.guardA;
+                    if (nearR || nearA) {
+                        double d2 = exact_d2(pos, perm[s], perm[t], P);
+                        inR = d2 < P.cutR2_d;
+                        inA = d2 < P.cutA2_d;
+                    }
+                    if (inA) {
+                        if (na < P.capA) listA[(size_t)na * n + s] = t;
+                        ++na;
+                    } else if (inR) {
+                        if (ns < P.capS) listS[(size_t)ns * n + s] = t;
+                        ++ns;
+                    }
+                }
+            }
+        }
+    }
+    cntA[s] = min(na, P.capA);
+    cntS[s] = min(ns, P.capS);
+    if (na > P.capA) atomicOr(&flags[0], 1);
+    if (ns > P.capS) atomicOr(&flags[1], 1);
+    atomicMax(&flags[2], na);
+    atomicMax(&flags[3], na + ns);
+    atomicMax(&flags[4], ns);
+}
+
+// ---- 5. reverse index -----------------------------------------------------------------------------------
+__global__ void k_build_rev(int n, int capA, const int* __restrict__ listA, const int* __restrict__ cntA,
+                            unsigned char* __restrict__ rev)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int c = cntA[s];
+    for (int m = 0; m < c; ++m) {
+        const int j = listA[(size_t)m * n + s];
+        const int cj = cntA[j];
+        int found = 0;
+        for (int mm = 0; mm < cj; ++mm)
+            if (listA[(size_t)mm * n + j] == s) { found = mm; break; }
+        rev[(size_t)m * n + s] = (unsigned char)found;
+    }
+}
+
+// ---- export in the caller's order and numbering ------------------------------------------------------------
+__global__ void k_export_lists(int n, int which, const int* __restrict__ perm,
+                               const int* __restrict__ listA, const int* __restrict__ cntA,
+                               const int* __restrict__ listS, const int* __restrict__ cntS,
+                               int* __restrict__ count_out, int* __restrict__ list_out, int cap)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int i = perm[s];
+    const int ca = cntA[s], cs = which == 0 ? cntS[s] : 0;
+    int* row = list_out + (size_t)i * cap;
+    for (int m = 0; m < ca; ++m) row[m] = perm[listA[(size_t)m * n + s]];
+    for (int m = 0; m < cs; ++m) row[ca + m] = perm[listS[(size_t)m * n + s]];
+    count_out[i] = ca + cs;
+}
