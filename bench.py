@@ -1,0 +1,413 @@
+#!/usr/bin/env python
+"""bench.py -- atom-step/s of the NEP3 hot path (BASELINE.json metric) on one B200 per rank.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config IDX] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: one velocity-Verlet NVE
+step = half kick + drift, [neighbour lists rebuilt every `rebuild_every` steps], energy / force /
+virial evaluation, half kick -- everything inside the library's sm_100a kernels, through the C ABI
+(include/nep.h).  The default workload is BASELINE.json configs[3] (1,000,188-atom five-species fcc
+alloy), the configuration north_star's throughput target is quoted on.  Seeded synthetic inputs
+(workloads.py); weights are the seeded random model, not a trained one.
+
+Prints ONE JSON line (rank 0).  Keys beyond the base contract:
+  roofline     the dominant kernel: algorithmic flops (or bytes) per launch / CUDA-event duration
+  kernels      the same for every kernel that ran in the timed region (events recorded by the library
+               on its own stream, nep_profile_*)
+  cpu_baseline the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
+  e2e          the same metric through md_run_host() with pinned HOST buffers: every step uploads
+               positions + velocities and downloads positions, velocities, energies and forces
+
+Multi-GPU: the path has no sharding in north_star ("no multi-GPU sharding or collectives"), so --gpus N
+runs N independent replicas ("replicas only"); torch.distributed is used for the barrier
+and the max-over-ranks time only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import workloads as W
+
+METRIC = "atom-step/s (NEP force+MD step, 1 B200) and % of FP32/HBM roofline"
+UNIT = "atom-step/s"
+SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0     # B200_PROFILING.md "Nominal figures"
+L2_BYTES = 126e6
+
+
+# ---------------------------------------------------------------------------------------------------
+# Algorithmic cost model.  FMA = 2 flops.  Units are the
+# ordered pairs inside the cutoffs at the timed evaluation (nep_pair_counts) and the atoms.
+def kernel_costs(h: W.Hyper, n_atoms: int, pairs_r: int, pairs_a: int, list_r: int, list_a: int):
+    """{kernel: (flops per launch, bytes per launch)} -- what the METHOD must compute / move, not what
+    the kernels happen to execute.  list_r / list_a: entries of the skin lists (radial = all)."""
+    NR, KR, NA, KA, D, H = h.NR, h.KR, h.NA, h.KA, h.n_des, h.n_neurons
+    n = n_atoms
+    out = {}
+    # a2 radial descriptor: per pair r, f_c, x, T_k, f_k and the NR x KR contraction
+    out["radial"] = (pairs_r * (35 + 4 * KR + 2 * NR * KR),
+                     n * (16 + 4 * NR) + 4 * pairs_r)
+    # a3+a4: g_n (NA x KA), 24 b_k, 24 NA accumulations; per atom the components from S
+    out["angular"] = (pairs_a * (90 + 2 * NA * KA + 2 * 24 * NA) + n * 30 * NA,
+                      n * (16 + 4 * 24 * NA + 4 * 6 * NA) + 4 * pairs_a)
+    # a5: forward + backward of the network
+    out["ann"] = (n * (4 * D * H + 10 * H), n * (8 * D + 4))
+    # a7: g, g' (4 NA KA), A_k, B_k (4 x 24 NA), assembly of b_k / grad P_k (~500); per atom G_nk
+    out["force_angular"] = (pairs_a * (4 * NA * KA + 4 * 24 * NA + 500) + n * 3 * 24 * NA,
+                            n * (16 + 4 * 24 * NA + 4 * 6 * NA) + pairs_a * (4 + 12))
+    # a6+a8: radial partial forces both directions, sums; angular gather of own + reverse partial force
+    out["final"] = (pairs_r * (55 + 8 * KR + 4 * NR * KR) + pairs_a * 30,
+                    n * (16 + 4 + 8 * 13) + 4 * pairs_r + pairs_a * (4 + 1 + 2 * 12) + pairs_r * 4 * NR)
+    # per-step filter of the skin lists to the in-cutoff lists (~12 flops per listed pair)
+    out["filter"] = (list_r * 12, n * 32 + 4 * list_r + 4 * pairs_r)
+    out["quantize"] = (n * 9, n * (24 + 4 + 4 + 16))
+    out["kick_drift"] = (n * 3 * 5, n * (3 * 8 * 5 + 4))
+    out["kick"] = (n * 3 * 3, n * (3 * 8 * 3 + 4))
+    return out
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.proc, self.lines = gpu_index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "50", "-i", str(self.idx)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(self.NAMES, f[3:7]):
+                if val == "Active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(pw)}
+
+
+def measured_peaks():
+    """HBM GB/s from MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload: str):
+    """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this workload:
+    profiles/traffic_<workload>.csv with lines `kernel,dram_bytes_per_launch`."""
+    path = os.path.join(ROOT, "profiles", f"traffic_{workload}.csv")
+    out = {}
+    try:
+        with open(path) as f:
+            for line in f:
+                k, _, v = line.strip().partition(",")
+                try:
+                    out[k] = float(v)
+                except ValueError:
+                    pass
+    except OSError:
+        pass
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# The oracle on the host cores: cpu_baseline leg and --impl reference arm.
+def oracle_sample_config(cfg: W.Config, n_target: int) -> W.Config:
+    """A smaller replica of `cfg` (same lattice, species rule, model, sigma, temperature) with about
+    n_target atoms, cubic cell count, box >= 2 (rc + skin)."""
+    per_cell = len(W._BASIS[cfg.lattice])
+    c = max(1, round((n_target / per_cell) ** (1.0 / 3.0)))
+    c_min = int(np.ceil(2.0 * (cfg.hyper.rc_radial + cfg.skin) / cfg.a + 1e-9))
+    return W.get_config(cfg.index, tuple(max(c_min, min(c, full)) for full in cfg.cells))
+
+
+def run_oracle_steps(cfg: W.Config, n_steps: int):
+    """Times oracle.md (initial evaluation + n_steps velocity-Verlet steps, fp64, brute-force
+    neighbours every evaluation).  Returns (seconds, atoms, evaluations)."""
+    import oracle
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    oracle.lib()
+    t0 = time.perf_counter()
+    oracle.md(cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box, cfg.dt_fs, n_steps)
+    return time.perf_counter() - t0, len(s.pos), n_steps + 1
+
+
+def cpu_baseline(cfg: W.Config):
+    import oracle
+    scfg = oracle_sample_config(cfg, 32000)
+    secs, n, evals = run_oracle_steps(scfg, 2)
+    return {"value": n * evals / secs, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n}-atom replica ({'x'.join(map(str, scfg.cells))} cells) of {cfg.name}, "
+                      f"{evals} fp64 force evaluations (oracle.md, 2 NVE steps) in {secs:.1f} s, "
+                      "O(N^2) neighbour search included"}
+
+
+def config_dict(cfg: W.Config, n_atoms: int, extra=None):
+    h = cfg.hyper
+    d = {"workload": cfg.name, "atoms": n_atoms, "species": h.n_types,
+         "rc_radial_angular": [h.rc_radial, h.rc_angular], "n_max": [h.n_max_radial, h.n_max_angular],
+         "basis": [h.basis_radial, h.basis_angular], "l_max": [h.l_max_3b, h.l_max_4b, h.l_max_5b],
+         "neurons": h.n_neurons, "n_descriptors": h.n_des, "dt_fs": cfg.dt_fs, "skin": cfg.skin,
+         "rebuild_every": cfg.rebuild_every, "temperature_K": cfg.temperature}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    cfg = W.get_config(args.config)
+    budget_s = 150.0
+    rate_guess = 600.0 * oracle.num_threads()             # atom-step/s of the oracle, order of magnitude
+    n_target = int(min(32000, max(2000, rate_guess * budget_s / (args.steps + args.warmup + 1))))
+    scfg = oracle_sample_config(cfg, n_target)
+    if args.warmup > 0:
+        run_oracle_steps(scfg, max(0, args.warmup - 1))
+    secs, n, evals = run_oracle_steps(scfg, args.steps)
+    value = n * args.steps / secs
+    sample = (f"{n}-atom replica ({'x'.join(map(str, scfg.cells))} cells) of {cfg.name} per step; "
+              f"{args.steps} NVE steps + initial evaluation timed together")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic (seeded lattice + random weights, workloads.py)",
+            "config": config_dict(cfg, n, {"sample": sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+def max_over_ranks(x: float, world: int, device: str = "cpu") -> float:
+    """MAX all-reduce of one float over the ranks (the job's time is the slowest rank's)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, atoms_per_rank: int, steps: int, ms_max: float) -> float:
+    """Replicas only: every rank advances its own `atoms_per_rank` atoms by `steps` steps."""
+    return world * atoms_per_rank * steps / (ms_max * 1e-3)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2205_10046_b200 import NEP          # raises if libnep_b200.so is missing: no fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the NEP path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = W.get_config(args.config)
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    n = len(s.pos)
+    K, Wm = args.steps, args.warmup
+    nep = NEP(cfg.hyper, p, s.masses, device=local)
+    pos = torch.tensor(s.pos, device=dev)
+    vel = torch.tensor(s.vel, device=dev)
+    types = torch.tensor(s.types, device=dev)
+
+    # ---- device-resident arm: inputs already in HBM when the timed region starts
+    nep.nep_neighbors(pos, types, s.box, cfg.skin)
+    nep.md_step(pos, vel, cfg.dt_fs, Wm, cfg.rebuild_every, cfg.skin)            # warm-up (untimed)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    nep.nep_profile(True)
+    l0 = nep.nep_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    nep.md_step(pos, vel, cfg.dt_fs, K, cfg.rebuild_every, cfg.skin)
+    ev1.record()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
+    clocks = sampler.stop()
+    launches = nep.nep_launch_count() - l0
+    prof = nep.nep_profile_read()
+    nep.nep_profile(False)
+    pairs_r, pairs_a = nep.nep_pair_counts()
+    cnt_r, _ = nep.nep_get_neighbors(0)
+    cnt_a, _ = nep.nep_get_neighbors(1)
+    list_r, list_a = int(cnt_r.sum().item()), int(cnt_a.sum().item())
+    del cnt_r, cnt_a
+    disp = nep.nep_max_displacement()
+    dev_bytes = nep.nep_device_bytes()
+    assert torch.isfinite(pos).all() and torch.isfinite(vel).all(), "non-finite state after the timed region"
+    value = whole_job_value(world, n, K, ms)
+
+    # ---- end-to-end arm: md_run_host with pinned host buffers, one call per step
+    pos_h = torch.tensor(s.pos).pin_memory()
+    vel_h = torch.tensor(s.vel).pin_memory()
+    typ_h = torch.tensor(s.types).pin_memory()
+    e_h = torch.empty(n, dtype=torch.float64).pin_memory()
+    f_h = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+    nep.md_run_host(pos_h, vel_h, typ_h, s.box, cfg.dt_fs, 1, cfg.rebuild_every, cfg.skin, e_h, f_h)   # starts the run
+    for _ in range(max(3, min(Wm, 10))):
+        nep.md_run_host(pos_h, vel_h, None, None, cfg.dt_fs, 1, cfg.rebuild_every, cfg.skin, e_h, f_h)
+    barrier()
+    ev0.record()
+    for _ in range(K):
+        nep.md_run_host(pos_h, vel_h, None, None, cfg.dt_fs, 1, cfg.rebuild_every, cfg.skin, e_h, f_h)
+    ev1.record()
+    barrier()
+    ms_e2e = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
+    h2d = pos_h.numel() * 8 + vel_h.numel() * 8
+    d2h = h2d + e_h.numel() * 8 + f_h.numel() * 8
+    e2e = {"value": whole_job_value(world, n, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / K,
+           "api": "md_run_host(n_steps=1) per step, pinned host pos/vel in, pos/vel/energy/force out"}
+
+    # ---- rooflines
+    fp32_probe = nep.nep_probe_fp32()
+    hbm_peak, hbm_src = measured_peaks()
+    alu_peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12        # TFLOP/s, derived
+    costs = kernel_costs(cfg.hyper, n, pairs_r, pairs_a, list_r, list_a)
+    traffic = ncu_traffic(cfg.name)
+    t_sum = sum(v[0] for v in prof.values())
+    kernels = []
+    for name, (tot_ms, cnt) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
+        avg_s = tot_ms / cnt * 1e-3
+        entry = {"name": name, "launches": cnt, "avg_us": avg_s * 1e6, "share": tot_ms / t_sum}
+        if name in costs and avg_s > 0:
+            fl, by = costs[name]
+            entry.update({"tflops": fl / avg_s / 1e12, "alu_frac": fl / avg_s / 1e12 / alu_peak,
+                          "gbs": by / avg_s / 1e9, "hbm_frac": by / avg_s / 1e9 / hbm_peak,
+                          "flops_per_launch": fl, "bytes_per_launch": by})
+        kernels.append(entry)
+    top = next((k for k in kernels if "tflops" in k), None)
+    roofline = None
+    if top is not None:
+        if top["alu_frac"] >= top["hbm_frac"]:
+            roofline = {"kernel": top["name"], "bound": "alu", "achieved": top["tflops"], "peak": alu_peak,
+                        "unit": "TFLOP/s", "frac": top["alu_frac"],
+                        "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                        "peak_probe_tflops": fp32_probe, "frac_of_probe": top["tflops"] / fp32_probe}
+        else:
+            roofline = {"kernel": top["name"], "bound": "hbm", "achieved": top["gbs"], "peak": hbm_peak,
+                        "unit": "GB/s", "frac": top["hbm_frac"], "peak_source": hbm_src}
+        roofline["traffic"] = traffic.get(top["name"])
+        roofline["avg_us"] = top["avg_us"]
+        roofline["share_of_step"] = top["share"]
+    step_flops = sum(costs[k["name"]][0] * k["launches"] for k in kernels if k["name"] in costs) / K
+    step_bytes = sum(costs[k["name"]][1] * k["launches"] for k in kernels if k["name"] in costs) / K
+    step = {"flops_per_atom": step_flops / n, "bytes_per_atom": step_bytes / n,
+            "tflops": world * step_flops * K / (ms * 1e-3) / 1e12 / world,
+            "alu_frac": step_flops * K / (ms * 1e-3) / 1e12 / alu_peak,
+            "hbm_frac": step_bytes * K / (ms * 1e-3) / 1e9 / hbm_peak,
+            "kernel_time_share_of_wall": t_sum / ms if world == 1 else None}
+
+    cpu = cpu_baseline(cfg) if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic (seeded lattice + random weights, workloads.py)",
+                "config": config_dict(cfg, n, {
+                    "parallelism": "replicas only" if world > 1 else "single GPU",
+                    "l2_policy": f"inputs larger than L2: the handle's per-step working set is "
+                                 f"{dev_bytes / 1e6:.0f} MB of device memory vs 126 MB of L2",
+                    "pairs_in_rc_per_atom": [pairs_r / n, pairs_a / n],
+                    "list_entries_per_atom": [list_r / n, list_a / n],
+                    "max_displacement_since_build": disp}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "kernels": kernels, "step": step, "fp32_probe_tflops": fp32_probe,
+                "cpu_baseline": cpu, "impl": "ours"}
+        print(json.dumps(line), flush=True)
+    nep.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: 1M atoms)")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -129,9 +129,16 @@ int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* viri
 int nep_max_displacement(nep_t* nep, double* disp_host);
 
 /* ---- host-buffer entry points (end-to-end path: H2D copies, kernels, D2H copies) -------------------
- * nep_compute_host: nep_neighbors + nep_compute on HOST arrays (pageable or pinned); synchronises.
- * md_run_host: uploads pos/vel, runs nep_neighbors (first call or when n changed) and md_step, downloads
- *   pos/vel and, if non-NULL, the final energy/force/virial; synchronises.                            */
+ * All *_host arrays are HOST memory (pageable or pinned; pinned makes the copies asynchronous DMA).
+ * The device staging copies are owned by the handle and reused between calls.  Both synchronise.
+ * nep_compute_host: upload pos/type, nep_neighbors + one evaluation, download the non-NULL results.
+ * md_run_host: upload pos/vel, run n_steps of md_step, download pos/vel and the non-NULL results of the
+ *   final evaluation.  type_host != NULL STARTS a run: types are uploaded and the lists built from the
+ *   uploaded positions (box, skin as in nep_neighbors).  type_host == NULL CONTINUES the run the previous
+ *   md_run_host call on this handle left (same n): types, lists, rebuild cadence and the forces of the
+ *   last evaluation carry over, `box` is ignored; the uploaded positions must be the ones that call
+ *   returned (velocities may have been changed, e.g. by a host-side thermostat).  NEP_ERR_STATE if there
+ *   is nothing to continue.                                                                            */
 int nep_compute_host(nep_t* nep, int64_t n, const double* pos_host, const int32_t* type_host,
                      const double box[9], double skin,
                      double* energy_host, double* force_host, double* virial_host);
@@ -145,8 +152,27 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev);
 int nep_get_angular_sums(nep_t* nep, float* S_dev);
 
-/* Number of kernel launches the handle has enqueued so far (for bench.py's gpu_launches).             */
+/* ---- measurement support (bench.py) ---------------------------------------------------------------
+ * nep_launch_count: kernel launches the handle has enqueued so far (bench.py's gpu_launches).
+ * nep_device_bytes: device memory the handle currently owns (model tables, lists, scratch, staging).
+ * nep_profile(enable): switches per-kernel timing on/off and clears the totals.  While on, every kernel
+ *   launch is bracketed by a CUDA event pair on the handle's stream (no synchronisation added, except a
+ *   drain every 32768 launches).  nep_profile_read: synchronises and returns, per kernel id
+ *   k < nep_profile_num_kernels(), the summed device time in ms and the number of launches since the
+ *   last nep_profile() call; nep_profile_kernel_name(k) names the id ("radial", "force_angular", ...).
+ * nep_probe_fp32: runs an FP32 FMA throughput probe (independent 3-register FFMA chains, no memory
+ *   traffic) on `device`/`cuda_stream` and returns the best of 5 timed launches in TFLOP/s: the measured
+ *   denominator of the ALU roofline.  Synchronises.                                                    */
+/* nep_pair_counts: ordered pairs inside r_c^R and inside r_c^A at the last evaluation (the sums of
+ *   NN_i^R and NN_i^A without skin): the units of the per-kernel flop counts.  Synchronises. */
+int nep_pair_counts(nep_t* nep, int64_t* radial_pairs_host, int64_t* angular_pairs_host);
 int64_t nep_launch_count(const nep_t* nep);
+int64_t nep_device_bytes(const nep_t* nep);
+int nep_profile(nep_t* nep, int enable);
+int nep_profile_num_kernels(void);
+const char* nep_profile_kernel_name(int k);
+int nep_profile_read(nep_t* nep, double* ms_total_host, int64_t* launches_host);
+int nep_probe_fp32(int device, void* cuda_stream, double* tflops_host);
 
 const char* nep_last_error(const nep_t* nep);
 const char* nep_status_string(int status);

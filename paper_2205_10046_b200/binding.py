@@ -20,7 +20,8 @@ exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums",
-    "nep_launch_count", "nep_last_error", "nep_status_string",
+    "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
+    "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
 
 
@@ -91,6 +92,20 @@ def load_library():
     L.nep_get_angular_sums.argtypes = [vp, vp]
     L.nep_launch_count.restype = i64
     L.nep_launch_count.argtypes = [vp]
+    L.nep_pair_counts.restype = C.c_int
+    L.nep_pair_counts.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+    L.nep_device_bytes.restype = i64
+    L.nep_device_bytes.argtypes = [vp]
+    L.nep_profile.restype = C.c_int
+    L.nep_profile.argtypes = [vp, C.c_int]
+    L.nep_profile_num_kernels.restype = C.c_int
+    L.nep_profile_num_kernels.argtypes = []
+    L.nep_profile_kernel_name.restype = C.c_char_p
+    L.nep_profile_kernel_name.argtypes = [C.c_int]
+    L.nep_profile_read.restype = C.c_int
+    L.nep_profile_read.argtypes = [vp, dp, C.POINTER(i64)]
+    L.nep_probe_fp32.restype = C.c_int
+    L.nep_probe_fp32.argtypes = [C.c_int, vp, dp]
     L.nep_last_error.restype = C.c_char_p
     L.nep_last_error.argtypes = [vp]
     L.nep_status_string.restype = C.c_char_p
@@ -246,6 +261,33 @@ class NEP:
     def nep_launch_count(self) -> int:
         return int(self._L.nep_launch_count(self._h_ptr))
 
+    def nep_pair_counts(self):
+        """(ordered pairs inside rc_radial, inside rc_angular) at the last evaluation."""
+        r, a = C.c_int64(0), C.c_int64(0)
+        self._check(self._L.nep_pair_counts(self._h_ptr, C.byref(r), C.byref(a)))
+        return r.value, a.value
+
+    def nep_device_bytes(self) -> int:
+        return int(self._L.nep_device_bytes(self._h_ptr))
+
+    def nep_profile(self, enable: bool):
+        self._check(self._L.nep_profile(self._h_ptr, 1 if enable else 0))
+
+    def nep_profile_read(self):
+        """{kernel name: (total ms, launches)} since the last nep_profile() call; synchronises."""
+        k = self._L.nep_profile_num_kernels()
+        ms = (C.c_double * k)()
+        cnt = (C.c_int64 * k)()
+        self._check(self._L.nep_profile_read(self._h_ptr, ms, cnt))
+        return {self._L.nep_profile_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(k) if cnt[i] > 0}
+
+    def nep_probe_fp32(self) -> float:
+        v = C.c_double(0.0)
+        rc = self._L.nep_probe_fp32(self.device, C.c_void_p(self.stream), C.byref(v))
+        if rc != 0:
+            raise NepError(rc, self._L.nep_status_string(rc).decode())
+        return v.value
+
     # host-buffer entry points: numpy arrays or pinned CPU tensors (anything exposing a host pointer)
     @staticmethod
     def _host_ptr(a):
@@ -267,8 +309,9 @@ class NEP:
 
     def md_run_host(self, pos, vel, types, box, dt_fs: float, n_steps: int, rebuild_every: int, skin: float,
                     energy=None, force=None, virial=None):
+        """types=None continues the run of the previous md_run_host call (see include/nep.h)."""
         n = pos.shape[0]
-        b = _box9(box)
+        b = _box9(box if box is not None else np.zeros(3))
         self._check(self._L.md_run_host(self._h_ptr, n, self._host_ptr(pos), self._host_ptr(vel),
                                         self._host_ptr(types), b.ctypes.data_as(C.POINTER(C.c_double)),
                                         float(dt_fs), int(n_steps), int(rebuild_every), float(skin),

@@ -9,6 +9,7 @@
 #include "nep_common.cuh"
 #include "nep_neighbor.cuh"
 #include "nep_kernels.cuh"
+#include "nep_probe.cuh"
 
 namespace {
 
@@ -61,11 +62,18 @@ int n_des(const nep_hyper_t* h)
     return (h->n_max_radial + 1) + (h->n_max_angular + 1) * nblk;     // Eq. (20)
 }
 
+void disown(nep_t* nep, void* p)
+{
+    for (int a = 0; a < nep->n_owned; ++a)
+        if (nep->owned[a].p == p) { nep->owned[a] = nep->owned[--nep->n_owned]; return; }
+}
+
 template <typename T>
 int dev_alloc(nep_t* nep, T** p, size_t count)
 {
-    if (*p) { cudaFree(*p); *p = nullptr; }
+    if (*p) { disown(nep, *p); cudaFree(*p); *p = nullptr; }
     if (count == 0) count = 1;
+    if (nep->n_owned >= (int)(sizeof(nep->owned) / sizeof(nep->owned[0]))) return nep_fail(nep, NEP_ERR_NOMEM, "allocation table full");
     cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
     if (e != cudaSuccess) {
         *p = nullptr;
@@ -73,6 +81,9 @@ int dev_alloc(nep_t* nep, T** p, size_t count)
         cudaGetLastError();
         return NEP_ERR_NOMEM;
     }
+    nep->owned[nep->n_owned].p = *p;
+    nep->owned[nep->n_owned].bytes = count * sizeof(T);
+    nep->n_owned++;
     return NEP_OK;
 }
 #define NEP_TRY(x) do { int rc_ = (x); if (rc_ != NEP_OK) return rc_; } while (0)
@@ -150,24 +161,17 @@ int build_lists(nep_t* nep, const double* pos_dev)
 
     const int TB = 256;
     NEP_CUDA(cudaMemsetAsync(nep->cell_count, 0, sizeof(unsigned) * (size_t)(nep->n_cells + 1), st));
-    k_cell_hist<<<div_up(n, TB), TB, 0, st>>>(P, pos_dev, nep->cell_of, nep->rank_in_cell, nep->cell_count);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_CELL_HIST, k_cell_hist<<<div_up(n, TB), TB, 0, st>>>(P, pos_dev, nep->cell_of, nep->rank_in_cell, nep->cell_count));
     {
         const int64_t m = nep->n_cells + 1;
         const int nb = div_up(m, SCAN_THREADS * SCAN_ITEMS);
-        k_scan_blocks<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_count, nep->cell_start, nep->scan_tmp, m);
-        NEP_LAUNCH_CHECK();
-        k_scan_totals<<<1, 1024, 0, st>>>(nep->scan_tmp, nb);
-        NEP_LAUNCH_CHECK();
-        k_scan_add<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_start, nep->scan_tmp, m);
-        NEP_LAUNCH_CHECK();
+        NEP_LAUNCH(NEP_K_SCAN, k_scan_blocks<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_count, nep->cell_start, nep->scan_tmp, m));
+        NEP_LAUNCH(NEP_K_SCAN, k_scan_totals<<<1, 1024, 0, st>>>(nep->scan_tmp, nb));
+        NEP_LAUNCH(NEP_K_SCAN, k_scan_add<<<nb, SCAN_THREADS, 0, st>>>(nep->cell_start, nep->scan_tmp, m));
     }
-    k_scatter<<<div_up(n, TB), TB, 0, st>>>(n, nep->cell_of, nep->rank_in_cell, nep->cell_start, nep->perm);
-    NEP_LAUNCH_CHECK();
-    k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm);
-    NEP_LAUNCH_CHECK();
-    k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, P.inv_Lx, P.inv_Ly, P.inv_Lz, nep->posq);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_SCATTER, k_scatter<<<div_up(n, TB), TB, 0, st>>>(n, nep->cell_of, nep->rank_in_cell, nep->cell_start, nep->perm));
+    NEP_LAUNCH(NEP_K_SORT_CELLS, k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm));
+    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, P.inv_Lx, P.inv_Ly, P.inv_Lz, nep->posq));
     NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
 
     if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
@@ -180,9 +184,8 @@ int build_lists(nep_t* nep, const double* pos_dev)
     for (int attempt = 0; attempt < 4; ++attempt) {
         P.capA = nep->capA; P.capS = nep->capS;
         NEP_CUDA(cudaMemsetAsync(nep->flags, 0, sizeof(int) * 8, st));
-        k_build_lists<<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
-                                                    nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags);
-        NEP_LAUNCH_CHECK();
+        NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
+                                                    nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
         int fl[8];
         NEP_CUDA(cudaMemcpyAsync(fl, nep->flags, sizeof(fl), cudaMemcpyDeviceToHost, st));
         NEP_CUDA(cudaStreamSynchronize(st));
@@ -196,8 +199,7 @@ int build_lists(nep_t* nep, const double* pos_dev)
         if (fl[1]) capS = fl[4] + 8;
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
-    k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA, nep->listA, nep->cntA, nep->rev);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA, nep->listA, nep->cntA, nep->rev));
     nep->steps_since_build = 0;
     nep->have_lists = true;
     return NEP_OK;
@@ -210,8 +212,7 @@ int launch_radial(nep_t* nep)
     const NepDims& d = nep->d;
     const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KR * d.NRP;
     NEP_TRY(allow_smem(nep, k_radial<NR>, sm));
-    k_radial<NR><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_t, nep->q);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_RADIAL, k_radial<NR><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_t, nep->q));
     return NEP_OK;
 }
 
@@ -233,13 +234,12 @@ int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int ac
     const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KA * d.NAP;
     if (!force_pass) {
         NEP_TRY(allow_smem(nep, k_angular<NCH>, sm));
-        k_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q);
+        NEP_LAUNCH(NEP_K_ANGULAR, k_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q));
     } else {
         NEP_TRY(allow_smem(nep, k_force_angular<NCH>, sm));
-        k_force_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->posq, nep->cA, nep->ncA,
-                                                                        nep->cA_t, nep->S, nep->fp, nep->pf);
+        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, k_force_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->posq, nep->cA, nep->ncA,
+                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf));
     }
-    NEP_LAUNCH_CHECK();
     return NEP_OK;
 }
 
@@ -271,9 +271,8 @@ int launch_ann(nep_t* nep)
     const NepDims& d = nep->d;
     const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H);
     NEP_TRY(allow_smem(nep, k_ann<DP>, sm));
-    k_ann<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
-                                                        nep->cR_e, nep->fp, nep->U, nep->Et);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
+                                                        nep->cR_e, nep->fp, nep->U, nep->Et));
     return NEP_OK;
 }
 
@@ -304,20 +303,17 @@ int evaluate(nep_t* nep, const double* pos_dev)
     const NepDims& d = nep->d;
     const int n = d.n;
     cudaStream_t st = nep->stream;
-    k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, 1.0 / nep->box[0], 1.0 / nep->box[1],
-                                               1.0 / nep->box[2], nep->posq);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, 1.0 / nep->box[0], 1.0 / nep->box[1],
+                                               1.0 / nep->box[2], nep->posq));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
-    k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
-                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->disp_max);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
+                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->disp_max));
     NEP_TRY(dispatch_radial(nep));
     NEP_TRY(dispatch_angular(nep, C, false));
     NEP_TRY(dispatch_ann(nep));
     NEP_TRY(dispatch_angular(nep, C, true));
-    k_final<<<div_up(n, 128), 128, 0, st>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->rev, nep->Et,
-                                            nep->pf, nep->U, nep->e_out, nep->f_out, nep->w_out);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_FINAL, k_final<<<div_up(n, 128), 128, 0, st>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->rev, nep->Et,
+                                            nep->pf, nep->U, nep->e_out, nep->f_out, nep->w_out));
     nep->have_eval = true;
     return NEP_OK;
 }
@@ -480,12 +476,12 @@ int nep_destroy(nep_t* nep)
     if (!nep) return NEP_ERR_INVALID_ARG;
     cudaSetDevice(nep->device);
     cudaStreamSynchronize(nep->stream);
-    void* ptrs[] = {nep->cR_t, nep->cA_t, nep->cR_e, nep->w0p, nep->b0, nep->w1, nep->mass_dev, nep->type_orig, nep->perm,
-                    nep->posq, nep->posq_build, nep->cell_of, nep->rank_in_cell, nep->order_tmp, nep->cell_count,
-                    nep->cell_start, nep->scan_tmp, nep->listA, nep->cntA, nep->listS, nep->cntS, nep->rev, nep->cA,
-                    nep->ncA, nep->cB, nep->ncB, nep->flags, nep->disp_max, nep->q, nep->fp, nep->S, nep->Et, nep->U,
-                    nep->pf, nep->e_out, nep->f_out, nep->w_out};
-    for (void* p : ptrs) if (p) cudaFree(p);
+    for (int a = 0; a < nep->n_owned; ++a) cudaFree(nep->owned[a].p);
+    if (nep->prof_ev) {
+        for (int a = 0; a < 2 * NEP_PROF_PAIRS; ++a) cudaEventDestroy(nep->prof_ev[a]);
+        free(nep->prof_ev);
+        free(nep->prof_kid);
+    }
     cudaGetLastError();
     delete nep;
     return NEP_OK;
@@ -517,9 +513,8 @@ int nep_get_neighbors(nep_t* nep, int which, int32_t* count_dev, int32_t* list_d
     if (cap < (which == 0 ? nep->maxR_skin : nep->maxA_skin)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "cap smaller than the longest list");
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
-    k_export_lists<<<div_up(n, 128), 128, 0, nep->stream>>>(n, which, nep->perm, nep->listA, nep->cntA, nep->listS, nep->cntS,
-                                                          count_dev, list_dev, cap);
-    NEP_LAUNCH_CHECK();
+    NEP_LAUNCH(NEP_K_EXPORT, k_export_lists<<<div_up(n, 128), 128, 0, nep->stream>>>(n, which, nep->perm, nep->listA, nep->cntA, nep->listS, nep->cntS,
+                                                          count_dev, list_dev, cap));
     return NEP_OK;
 }
 
@@ -567,13 +562,11 @@ int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t 
     const double hdt = 0.5 * dt_fs * kAccConv;
     const int TB = 256;
     for (int s = 0; s < n_steps; ++s) {
-        k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev);
-        NEP_LAUNCH_CHECK();
+        NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
         NEP_TRY(evaluate(nep, pos_dev));
-        k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev);
-        NEP_LAUNCH_CHECK();
+        NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
     }
     nep->force_current = true;
     nep->force_pos_tag = pos_dev;
@@ -600,8 +593,8 @@ int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev)
     if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
-    if (q_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->q, q_dev); NEP_LAUNCH_CHECK(); }
-    if (fp_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->fp, fp_dev); NEP_LAUNCH_CHECK(); }
+    if (q_dev) { NEP_LAUNCH(NEP_K_EXPORT, k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->q, q_dev)); }
+    if (fp_dev) { NEP_LAUNCH(NEP_K_EXPORT, k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.D, nep->perm, nep->fp, fp_dev)); }
     return NEP_OK;
 }
 
@@ -611,25 +604,19 @@ int nep_get_angular_sums(nep_t* nep, float* S_dev)
     if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
-    if (S_dev) { k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.NA * NEP_NUM_S, nep->perm, nep->S, S_dev); NEP_LAUNCH_CHECK(); }
+    if (S_dev) { NEP_LAUNCH(NEP_K_EXPORT, k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.NA * NEP_NUM_S, nep->perm, nep->S, S_dev)); }
     return NEP_OK;
 }
 
 // ---- host-buffer entry points ---------------------------------------------------------------------------
-static int stage_alloc(nep_t* nep, int64_t n, double** pos, double** vel, int** type)
+static int stage_alloc(nep_t* nep, int64_t n)
 {
-    // staging buffers live for one call: simple and leak-free; the copies dominate anyway
-    *pos = nullptr; *type = nullptr;
-    if (vel) *vel = nullptr;
-    if (cudaMalloc((void**)pos, sizeof(double) * 3 * (size_t)n) != cudaSuccess ||
-        (vel && cudaMalloc((void**)vel, sizeof(double) * 3 * (size_t)n) != cudaSuccess) ||
-        cudaMalloc((void**)type, sizeof(int) * (size_t)n) != cudaSuccess) {
-        cudaGetLastError();
-        if (*pos) cudaFree(*pos);
-        if (vel && *vel) cudaFree(*vel);
-        if (*type) cudaFree(*type);
-        return nep_fail(nep, NEP_ERR_NOMEM, "staging allocation failed");
-    }
+    if (n <= nep->h_cap && nep->h_pos) return NEP_OK;
+    nep->h_cap = 0;
+    NEP_TRY(dev_alloc(nep, &nep->h_pos, 3 * (size_t)n));
+    NEP_TRY(dev_alloc(nep, &nep->h_vel, 3 * (size_t)n));
+    NEP_TRY(dev_alloc(nep, &nep->h_type, (size_t)n));
+    nep->h_cap = n;
     return NEP_OK;
 }
 
@@ -646,21 +633,17 @@ int nep_compute_host(nep_t* nep, int64_t n, const double* pos_host, const int32_
                      double skin, double* energy_host, double* force_host, double* virial_host)
 {
     if (!nep) return NEP_ERR_INVALID_ARG;
-    if (!pos_host || !type_host || n <= 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n <= 0");
+    if (!pos_host || !type_host || n <= 0 || n > NEP_MAX_ATOMS) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or bad n");
     NEP_CUDA(cudaSetDevice(nep->device));
-    double* pos; int* type;
-    NEP_TRY(stage_alloc(nep, n, &pos, nullptr, &type));
-    int rc = NEP_OK;
-    if (cudaMemcpyAsync(pos, pos_host, sizeof(double) * 3 * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
-        cudaMemcpyAsync(type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess)
-        rc = nep_fail(nep, NEP_ERR_CUDA, "H2D copy failed");
-    if (rc == NEP_OK) rc = nep_neighbors(nep, n, pos, type, box, skin);
-    if (rc == NEP_OK) rc = evaluate(nep, pos);
-    if (rc == NEP_OK) rc = download_results(nep, energy_host, force_host, virial_host);
-    if (cudaStreamSynchronize(nep->stream) != cudaSuccess && rc == NEP_OK) rc = nep_fail(nep, NEP_ERR_CUDA, "stream sync failed");
-    nep->force_current = false;
-    cudaFree(pos); cudaFree(type);
-    return rc;
+    nep->h_run = false;
+    NEP_TRY(stage_alloc(nep, n));
+    NEP_CUDA(cudaMemcpyAsync(nep->h_pos, pos_host, sizeof(double) * 3 * (size_t)n, cudaMemcpyHostToDevice, nep->stream));
+    NEP_CUDA(cudaMemcpyAsync(nep->h_type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream));
+    NEP_TRY(nep_neighbors(nep, n, nep->h_pos, nep->h_type, box, skin));
+    NEP_TRY(evaluate(nep, nep->h_pos));
+    NEP_TRY(download_results(nep, energy_host, force_host, virial_host));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    return NEP_OK;
 }
 
 int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const int32_t* type_host, const double box[9],
@@ -668,27 +651,117 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
                 double* energy_host, double* force_host, double* virial_host)
 {
     if (!nep) return NEP_ERR_INVALID_ARG;
-    if (!pos_host || !vel_host || !type_host || n <= 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n <= 0");
+    if (!pos_host || !vel_host || n <= 0 || n > NEP_MAX_ATOMS) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or bad n");
     NEP_CUDA(cudaSetDevice(nep->device));
-    double *pos, *vel; int* type;
-    NEP_TRY(stage_alloc(nep, n, &pos, &vel, &type));
-    int rc = NEP_OK;
+    const bool cont = (type_host == nullptr);
+    if (cont && !(nep->h_run && n == nep->n && nep->have_lists))
+        return nep_fail(nep, NEP_ERR_STATE, "md_run_host: type_host == NULL continues a run, but none is in progress for this n");
+    if (!cont && !box) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null box");
+    nep->h_run = false;
+    NEP_TRY(stage_alloc(nep, n));
     const size_t b3 = sizeof(double) * 3 * (size_t)n;
-    if (cudaMemcpyAsync(pos, pos_host, b3, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
-        cudaMemcpyAsync(vel, vel_host, b3, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess ||
-        cudaMemcpyAsync(type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream) != cudaSuccess)
-        rc = nep_fail(nep, NEP_ERR_CUDA, "H2D copy failed");
-    if (rc == NEP_OK) rc = nep_neighbors(nep, n, pos, type, box, skin);
-    if (rc == NEP_OK) rc = md_step(nep, pos, vel, dt_fs, n_steps, rebuild_every, skin);
-    if (rc == NEP_OK &&
-        (cudaMemcpyAsync(pos_host, pos, b3, cudaMemcpyDeviceToHost, nep->stream) != cudaSuccess ||
-         cudaMemcpyAsync(vel_host, vel, b3, cudaMemcpyDeviceToHost, nep->stream) != cudaSuccess))
-        rc = nep_fail(nep, NEP_ERR_CUDA, "D2H copy failed");
-    if (rc == NEP_OK) rc = download_results(nep, energy_host, force_host, virial_host);
-    if (cudaStreamSynchronize(nep->stream) != cudaSuccess && rc == NEP_OK) rc = nep_fail(nep, NEP_ERR_CUDA, "stream sync failed");
-    nep->force_current = false;      // the staging buffers die with this call
-    cudaFree(pos); cudaFree(vel); cudaFree(type);
-    return rc;
+    NEP_CUDA(cudaMemcpyAsync(nep->h_pos, pos_host, b3, cudaMemcpyHostToDevice, nep->stream));
+    NEP_CUDA(cudaMemcpyAsync(nep->h_vel, vel_host, b3, cudaMemcpyHostToDevice, nep->stream));
+    if (!cont) {
+        NEP_CUDA(cudaMemcpyAsync(nep->h_type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream));
+        NEP_TRY(nep_neighbors(nep, n, nep->h_pos, nep->h_type, box, skin));
+    }
+    NEP_TRY(md_step(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin));
+    NEP_CUDA(cudaMemcpyAsync(pos_host, nep->h_pos, b3, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaMemcpyAsync(vel_host, nep->h_vel, b3, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_TRY(download_results(nep, energy_host, force_host, virial_host));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    nep->h_run = true;
+    return NEP_OK;
+}
+
+// ---- measurement support ----------------------------------------------------------------------------------
+static const char* const kKernelNames[NEP_K_COUNT] = {
+    "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
+    "angular", "ann", "force_angular", "final", "kick_drift", "kick", "export"};
+
+int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
+
+const char* nep_profile_kernel_name(int k) { return (k >= 0 && k < NEP_K_COUNT) ? kKernelNames[k] : ""; }
+
+int nep_profile(nep_t* nep, int enable)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    NEP_CUDA(cudaSetDevice(nep->device));
+    if (enable && !nep->prof_ev) {
+        nep->prof_ev = (cudaEvent_t*)calloc(2 * NEP_PROF_PAIRS, sizeof(cudaEvent_t));
+        nep->prof_kid = (int*)calloc(NEP_PROF_PAIRS, sizeof(int));
+        if (!nep->prof_ev || !nep->prof_kid) return nep_fail(nep, NEP_ERR_NOMEM, "profile buffers");
+        for (int a = 0; a < 2 * NEP_PROF_PAIRS; ++a) NEP_CUDA(cudaEventCreate(&nep->prof_ev[a]));
+    }
+    nep_prof_drain(nep);
+    for (int k = 0; k < NEP_K_COUNT; ++k) { nep->prof_ms[k] = 0.0; nep->prof_n[k] = 0; }
+    nep->prof_on = enable != 0;
+    return NEP_OK;
+}
+
+int nep_profile_read(nep_t* nep, double* ms_total_host, int64_t* launches_host)
+{
+    if (!nep || !ms_total_host || !launches_host) return NEP_ERR_INVALID_ARG;
+    NEP_CUDA(cudaSetDevice(nep->device));
+    nep_prof_drain(nep);
+    for (int k = 0; k < NEP_K_COUNT; ++k) { ms_total_host[k] = nep->prof_ms[k]; launches_host[k] = nep->prof_n[k]; }
+    return NEP_OK;
+}
+
+int nep_pair_counts(nep_t* nep, int64_t* radial_pairs_host, int64_t* angular_pairs_host)
+{
+    if (!nep || !radial_pairs_host || !angular_pairs_host) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const size_t n = (size_t)nep->n;
+    std::vector<int> a(n), b(n);
+    NEP_CUDA(cudaMemcpyAsync(a.data(), nep->ncA, sizeof(int) * n, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaMemcpyAsync(b.data(), nep->ncB, sizeof(int) * n, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    int64_t sa = 0, sb = 0;
+    for (size_t i = 0; i < n; ++i) { sa += a[i]; sb += b[i]; }
+    *angular_pairs_host = sa;
+    *radial_pairs_host = sa + sb;
+    return NEP_OK;
+}
+
+int64_t nep_device_bytes(const nep_t* nep)
+{
+    if (!nep) return 0;
+    size_t tot = 0;
+    for (int a = 0; a < nep->n_owned; ++a) tot += nep->owned[a].bytes;
+    return (int64_t)tot;
+}
+
+int nep_probe_fp32(int device, void* cuda_stream, double* tflops_host)
+{
+    if (!tflops_host) return NEP_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_CUDA; }
+    float* sink = nullptr;
+    if (cudaMalloc((void**)&sink, sizeof(float) * 1024) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_NOMEM; }
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(a, st);
+        k_probe_ffma<<<blocks, threads, 0, st>>>(iters, 1.0f + 1e-7f * rep, sink);
+        cudaEventRecord(b, st);
+        cudaEventSynchronize(b);
+        float ms = 0.0f;
+        cudaEventElapsedTime(&ms, a, b);
+        const double tf = 2.0 * NEP_PROBE_CHAINS * (double)iters * blocks * threads / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(sink);
+    if (cudaGetLastError() != cudaSuccess) return NEP_ERR_CUDA;
+    *tflops_host = best;
+    return NEP_OK;
 }
 
 }  // extern "C"

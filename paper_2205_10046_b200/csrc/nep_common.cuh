@@ -15,6 +15,14 @@
 #define NEP_SLOT_BITS 8         // packed angular entry: (j << 8) | skin slot
 #define NEP_MAX_ATOMS (1 << 24)
 
+// Kernel ids for the optional per-kernel CUDA-event timing (nep_profile_*; bench.py's roofline leg).
+enum NepKernelId {
+    NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
+    NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FINAL,
+    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_EXPORT, NEP_K_COUNT
+};
+#define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
+
 // ---------------------------------------------------------------------------------------------------
 // Scalars every kernel needs; passed by value as a kernel argument (lives in the constant bank).
 struct NepDims {
@@ -35,6 +43,14 @@ struct nep_ctx {
     cudaStream_t stream;
     char err[512];
     int64_t launches;
+
+    // per-kernel timing (off by default): one event pair per launch on `stream`, drained on read
+    bool prof_on;
+    cudaEvent_t* prof_ev;    // [2 * NEP_PROF_PAIRS], created on first enable
+    int* prof_kid;           // [NEP_PROF_PAIRS] kernel id of each pair
+    int prof_used;
+    double prof_ms[NEP_K_COUNT];
+    int64_t prof_n[NEP_K_COUNT];
 
     // model (device)
     float* cR_t;     // [T*T][KR][NRP]   c_radial transposed so that the n-values of one k are contiguous
@@ -93,6 +109,15 @@ struct nep_ctx {
     double* e_out;           // [n]    orig order
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]
+
+    // staging of the host-buffer entry points (device copies of the caller's host arrays)
+    double* h_pos; double* h_vel; int* h_type;
+    int64_t h_cap;
+    bool h_run;              // an md_run_host trajectory is in progress (continuation allowed)
+
+    // bookkeeping of owned device memory (nep_device_bytes)
+    struct { void* p; size_t bytes; } owned[96];
+    int n_owned;
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -115,6 +140,46 @@ struct nep_ctx {
                      cudaGetErrorString(e_));                                                       \
             return NEP_ERR_CUDA;                                                                    \
         }                                                                                           \
+    } while (0)
+
+// Drains the recorded event pairs into prof_ms / prof_n (synchronises the stream).
+static inline void nep_prof_drain(nep_t* nep)
+{
+    if (!nep->prof_ev || nep->prof_used == 0) return;
+    cudaEventSynchronize(nep->prof_ev[2 * (nep->prof_used - 1) + 1]);
+    for (int p = 0; p < nep->prof_used; ++p) {
+        float ms = 0.0f;
+        if (cudaEventElapsedTime(&ms, nep->prof_ev[2 * p], nep->prof_ev[2 * p + 1]) == cudaSuccess) {
+            nep->prof_ms[nep->prof_kid[p]] += (double)ms;
+            nep->prof_n[nep->prof_kid[p]] += 1;
+        }
+    }
+    cudaGetLastError();
+    nep->prof_used = 0;
+}
+
+static inline void nep_prof_begin(nep_t* nep, int kid)
+{
+    if (!nep->prof_on) return;
+    if (nep->prof_used == NEP_PROF_PAIRS) nep_prof_drain(nep);
+    nep->prof_kid[nep->prof_used] = kid;
+    cudaEventRecord(nep->prof_ev[2 * nep->prof_used], nep->stream);
+}
+
+static inline void nep_prof_end(nep_t* nep)
+{
+    if (!nep->prof_on) return;
+    cudaEventRecord(nep->prof_ev[2 * nep->prof_used + 1], nep->stream);
+    nep->prof_used++;
+}
+
+// NEP_LAUNCH(kernel id, kernel<<<...>>>(...)): launch + error check (+ event pair when profiling)
+#define NEP_LAUNCH(kid, ...)                                                                        \
+    do {                                                                                            \
+        nep_prof_begin(nep, (kid));                                                                 \
+        __VA_ARGS__;                                                                                \
+        nep_prof_end(nep);                                                                          \
+        NEP_LAUNCH_CHECK();                                                                         \
     } while (0)
 
 static inline int nep_fail(nep_t* nep, int status, const char* msg)
