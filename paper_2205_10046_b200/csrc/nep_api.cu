@@ -148,6 +148,7 @@ int build_lists(nep_t* nep, const double* pos_dev)
     BuildParams P;
     P.n = n;
     P.ncx = nep->ncell[0]; P.ncy = nep->ncell[1]; P.ncz = nep->ncell[2];
+    P.ntx = nep->ntile[0]; P.nty = nep->ntile[1];
     P.hx = P.hy = P.hz = 2;
     P.Lx = nep->box[0]; P.Ly = nep->box[1]; P.Lz = nep->box[2];
     P.inv_Lx = 1.0 / P.Lx; P.inv_Ly = 1.0 / P.Ly; P.inv_Lz = 1.0 / P.Lz;
@@ -206,39 +207,55 @@ int build_lists(nep_t* nep, const double* pos_dev)
 }
 
 // ---- one evaluation of (a2)-(a8) into the internal output buffers ---------------------------------------
-template <int NR>
-int launch_radial(nep_t* nep)
+const size_t kSmemTableMax = 96 * 1024;     // larger coefficient tables are read from global memory (L1)
+
+template <int KP>
+int launch_radial1(nep_t* nep)
 {
     const NepDims& d = nep->d;
-    const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KR * d.NRP;
-    NEP_TRY(allow_smem(nep, k_radial<NR>, sm));
-    NEP_LAUNCH(NEP_K_RADIAL, k_radial<NR><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_t, nep->q));
+    NEP_LAUNCH(NEP_K_RADIAL, k_radial1<KP><<<div_up(d.n, 128), 128, 0, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_q, nep->q));
     return NEP_OK;
 }
 
 int dispatch_radial(nep_t* nep)
 {
-    switch (nep->d.NR) {
-#define CASE(N) case N: return launch_radial<N>(nep);
-        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
-        CASE(9) CASE(10) CASE(11) CASE(12) CASE(13) CASE(14) CASE(15) CASE(16)
-#undef CASE
+    const NepDims& d = nep->d;
+    if (d.T == 1) {
+        switch (nep->KP) {
+            case 4: return launch_radial1<4>(nep);
+            case 8: return launch_radial1<8>(nep);
+            case 12: return launch_radial1<12>(nep);
+            case 16: return launch_radial1<16>(nep);
+            case 20: return launch_radial1<20>(nep);
+            case 24: return launch_radial1<24>(nep);
+            case 28: return launch_radial1<28>(nep);
+            case 32: return launch_radial1<32>(nep);
+        }
+        return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
     }
-    return nep_fail(nep, NEP_ERR_INVALID_ARG, "n_max_radial out of range");
+    const size_t tab_bytes = sizeof(float) * (size_t)d.T * d.T * nep->strideR;
+    const int tab_in_smem = tab_bytes <= kSmemTableMax;
+    int bs = 128;
+    while (bs > 32 && sizeof(float) * (size_t)d.T * d.KR * bs + (tab_in_smem ? tab_bytes : 0) > 160 * 1024) bs >>= 1;
+    const size_t sm = sizeof(float) * (size_t)d.T * d.KR * bs + (tab_in_smem ? tab_bytes : 0);
+    NEP_TRY(allow_smem(nep, k_radial_multi, sm));
+    NEP_LAUNCH(NEP_K_RADIAL, k_radial_multi<<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, tab_in_smem, nep->posq, nep->cA, nep->ncA,
+                                                                          nep->cB, nep->ncB, nep->cR_t, nep->q));
+    return NEP_OK;
 }
 
-template <int NCH>
+template <int NCH, bool SM>
 int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int accumulate)
 {
     const NepDims& d = nep->d;
-    const size_t sm = sizeof(float) * (size_t)d.T * d.T * d.KA * d.NAP;
+    const size_t sm = SM ? sizeof(float) * (size_t)d.T * d.T * nep->strideA : 0;
     if (!force_pass) {
-        NEP_TRY(allow_smem(nep, k_angular<NCH>, sm));
-        NEP_LAUNCH(NEP_K_ANGULAR, k_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q));
+        NEP_TRY(allow_smem(nep, k_angular<NCH, SM>, sm));
+        NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->strideA, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q)));
     } else {
-        NEP_TRY(allow_smem(nep, k_force_angular<NCH>, sm));
-        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, k_force_angular<NCH><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->posq, nep->cA, nep->ncA,
-                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf));
+        NEP_TRY(allow_smem(nep, k_force_angular<NCH, SM>, sm));
+        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->strideA, nep->posq, nep->cA, nep->ncA,
+                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf)));
     }
     return NEP_OK;
 }
@@ -246,18 +263,25 @@ int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int ac
 int dispatch_angular(nep_t* nep, const NepCoef& C, bool force_pass)
 {
     const int NA = nep->d.NA;
-    const int npass = (NA + NEP_NCH_MAX - 1) / NEP_NCH_MAX;
+    if (sizeof(float) * (size_t)nep->d.T * nep->d.T * nep->strideA > kSmemTableMax) {
+        // huge coefficient table: passes of 4 channels reading the table from global memory; the table
+        // is zero-padded to NAP = round_up4(NA) columns and surplus channels are not stored
+        for (int n0 = 0; n0 < NA; n0 += 4) NEP_TRY((launch_angular<4, false>(nep, C, n0, force_pass, n0 > 0)));
+        return NEP_OK;
+    }
+    const int npass = (NA + nep->nch_max - 1) / nep->nch_max;
     const int base = NA / npass, rem = NA % npass;
     int n0 = 0;
     for (int p = 0; p < npass; ++p) {
         const int nch = base + (p < rem ? 1 : 0);
         int rc;
         switch (nch) {
-            case 1: rc = launch_angular<1>(nep, C, n0, force_pass, p > 0); break;
-            case 2: rc = launch_angular<2>(nep, C, n0, force_pass, p > 0); break;
-            case 3: rc = launch_angular<3>(nep, C, n0, force_pass, p > 0); break;
-            case 4: rc = launch_angular<4>(nep, C, n0, force_pass, p > 0); break;
-            default: rc = launch_angular<5>(nep, C, n0, force_pass, p > 0); break;
+            case 1: rc = launch_angular<1, true>(nep, C, n0, force_pass, p > 0); break;
+            case 2: rc = launch_angular<2, true>(nep, C, n0, force_pass, p > 0); break;
+            case 3: rc = launch_angular<3, true>(nep, C, n0, force_pass, p > 0); break;
+            case 4: rc = launch_angular<4, true>(nep, C, n0, force_pass, p > 0); break;
+            case 5: rc = launch_angular<5, true>(nep, C, n0, force_pass, p > 0); break;
+            default: rc = launch_angular<6, true>(nep, C, n0, force_pass, p > 0); break;
         }
         if (rc != NEP_OK) return rc;
         n0 += nch;
@@ -269,7 +293,7 @@ template <int DP>
 int launch_ann(nep_t* nep)
 {
     const NepDims& d = nep->d;
-    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H);
+    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H + 16 * 128);
     NEP_TRY(allow_smem(nep, k_ann<DP>, sm));
     NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
                                                         nep->cR_e, nep->fp, nep->U, nep->Et));
@@ -337,7 +361,8 @@ int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
         if (c < 1) c = 1;
         if (c > 1024) c = 1024;
         nep->ncell[a] = c;
-        nc *= c;
+        nep->ntile[a] = (c + 3) / 4;
+        nc *= 4 * (int64_t)nep->ntile[a];
     }
     nep->n_cells = nc;
     nep->d.sx = (float)(L[0] / 4294967296.0);
@@ -426,20 +451,33 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
         nep->mass[t] = mass_amu[t];
     }
 
-    // re-laid-out parameter tables
+    // re-laid-out parameter tables (layouts documented at the kernels that read them)
     const int T = d.T, TT = T * T;
-    std::vector<float> cRt((size_t)TT * d.KR * d.NRP, 0.0f), cAt((size_t)TT * d.KA * d.NAP, 0.0f);
+    nep->KP = round_up4(d.KR);
+    nep->strideR = (d.KR * d.NRP) | 1;
+    nep->strideA = (d.KA * d.NAP) | 1;
+    nep->nch_max = 5;
+    if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) nep->nch_max = v; }
+    std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f), cAt((size_t)TT * nep->strideA, 0.0f);
+    std::vector<float> cRq((size_t)d.NR * nep->KP, 0.0f);
     std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
     for (int tt = 0; tt < TT; ++tt) {
         for (int nn = 0; nn < d.NR; ++nn)
             for (int k = 0; k < d.KR; ++k) {
                 const float v = c_radial[((size_t)tt * d.NR + nn) * d.KR + k];
-                cRt[((size_t)tt * d.KR + k) * d.NRP + nn] = v;
+                cRt[(size_t)tt * nep->strideR + (size_t)k * d.NRP + nn] = v;
                 cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
+                if (TT == 1) cRq[(size_t)nn * nep->KP + k] = v;
             }
-        for (int nn = 0; nn < d.NA; ++nn)
-            for (int k = 0; k < d.KA; ++k)
-                cAt[((size_t)tt * d.KA + k) * d.NAP + nn] = c_angular[((size_t)tt * d.NA + nn) * d.KA + k];
+        for (int nn = 0; nn < d.NA; ++nn) {
+            const float* c = c_angular + ((size_t)tt * d.NA + nn) * d.KA;
+            double csum = 2.0 * (double)c[0];                      // csum'_n = 2 c_n0 + sum_{k>=1} c_nk
+            for (int k = 1; k < d.KA; ++k) {
+                cAt[(size_t)tt * nep->strideA + (size_t)(k - 1) * d.NAP + nn] = c[k];
+                csum += (double)c[k];
+            }
+            cAt[(size_t)tt * nep->strideA + (size_t)(d.KA - 1) * d.NAP + nn] = (float)csum;
+        }
     }
     for (int m = 0; m < d.H; ++m)
         for (int v = 0; v < d.D; ++v) w0p[(size_t)m * nep->DP + v] = w0[(size_t)m * d.D + v];
@@ -453,6 +491,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
         if (rc != NEP_OK) { nep_destroy(nep); return rc; }                                        \
     } while (0)
     UPLOAD(cR_t, cRt);
+    UPLOAD(cR_q, cRq);
     UPLOAD(cA_t, cAt);
     UPLOAD(cR_e, cRe);
     UPLOAD(w0p, w0p);

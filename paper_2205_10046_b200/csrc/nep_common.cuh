@@ -11,7 +11,7 @@
 
 #define NEP_MAX_TYPES 16
 #define NEP_NUM_S 24            // sums S_{n,k}, k = 0..23 (Eq. 12)
-#define NEP_NCH_MAX 5           // angular n-values handled per pass (24*5 accumulators in registers)
+#define NEP_NCH_MAX 6           // most angular n-values handled per pass (24*NCH accumulators in registers)
 #define NEP_SLOT_BITS 8         // packed angular entry: (j << 8) | skin slot
 #define NEP_MAX_ATOMS (1 << 24)
 
@@ -53,9 +53,13 @@ struct nep_ctx {
     int64_t prof_n[NEP_K_COUNT];
 
     // model (device)
-    float* cR_t;     // [T*T][KR][NRP]   c_radial transposed so that the n-values of one k are contiguous
-    float* cA_t;     // [T*T][KA][NAP]
+    float* cR_t;     // [T*T] x strideR: rows [k][NRP]   c_radial with the n-values of one k contiguous
+    float* cR_q;     // [NR][KP]  (T == 1 only) zero-padded rows for k_radial1
+    float* cA_t;     // [T*T] x strideA: rows k = 1..KA-1 then csum' (see k_angular), NAP floats each
     float* cR_e;     // [T(ti)][T(tj)][NR][KRP]  for the per-atom E table
+    int strideR, strideA;   // odd type-pair strides (floats) of cR_t / cA_t: bank-conflict-free lookups
+    int KP;                 // KR rounded up to a multiple of 4
+    int nch_max;            // angular n-values per pass (<= NEP_NCH_MAX)
     float* w0p;      // [H][DP] rows padded with zeros to DP
     float* b0;       // [H]
     float* w1;       // [H]
@@ -69,7 +73,8 @@ struct nep_ctx {
     double box[3];
     double skin;
     int ncell[3];
-    int64_t n_cells;
+    int ntile[3];            // 4-cell tiles per axis
+    int64_t n_cells;         // padded: ntile[0]*ntile[1]*ntile[2]*64
     bool have_lists;
     bool have_eval;          // internal E/F/W hold an evaluation
     bool force_current;      // ... and it belongs to the positions md_step will continue from

@@ -1,15 +1,17 @@
 // nep_kernels.cuh -- (a2)-(a8): descriptors, network, partial forces, force/virial accumulation.
 //
-// One thread per atom in the internal spatial order (adjacent threads = adjacent atoms, so neighbour
-// gathers of the 16-byte quantised positions hit L1/L2).  Per-atom arrays are stored [component][atom]
-// so that a warp reads/writes 128 contiguous bytes per component.  Kernels per evaluation:
-//   k_filter         skin lists -> this step's in-cutoff lists (removes the in-cutoff divergence)
-//   k_radial<NR>     Eqs. (2)-(5)      radial descriptor
-//   k_angular<NCH>   Eq. (12), (13)-(19) angular sums (24*NCH accumulators in registers) and components
-//   k_ann<DP>        Eq. (1) / Listing 1; also E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
-//   k_force_angular<NCH>  last three terms of Eq. (21): dU_i/dr_ij for every angular pair
-//   k_final          first term of Eq. (21) for both directions via the E tables; Eqs. (22)-(24):
-//                    scatter-free gather of dU_j/dr_ji through the reverse index
+// One thread per atom in the internal spatial order (tile-major Morton order of the cells, so that a
+// warp's 32 atoms and their neighbours are a compact blob and the neighbour gathers hit L1).  Per-atom
+// arrays are stored [component][atom] so that a warp reads/writes 128 contiguous bytes per component.
+// Every pair loop is software-pipelined: the index two pairs ahead and the position one pair ahead
+// are in flight while the current pair is computed.  Kernels per evaluation:
+//   k_filter              skin lists -> this step's in-cutoff lists (removes the in-cutoff divergence)
+//   k_radial1<KP> / k_radial_multi   Eqs. (2)-(5) radial descriptor via per-type basis sums
+//   k_angular<NCH,SM>     Eq. (12), (13)-(19) angular sums (24*NCH accumulators in registers) + components
+//   k_ann<DP>             Eq. (1) / Listing 1; also E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
+//   k_force_angular<NCH,SM>  last three terms of Eq. (21): dU_i/dr_ij for every angular pair
+//   k_final               first term of Eq. (21) for both directions via the E tables; Eqs. (22)-(24):
+//                         scatter-free gather of dU_j/dr_ji through the reverse index
 #pragma once
 #include "nep_common.cuh"
 
@@ -18,6 +20,37 @@ struct NepCoef {
     float c3[NEP_NUM_S];
     float c4[5];
     float c5[3];
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Software-pipelined walk over one atom's neighbour entries  e_m = list[m*n + s], m = 0..cnt-1.
+// DECODE(e) gives the neighbour's sorted index.  Usage:
+//   PairWalk w(list, n, s, cnt, posq);  while (w.next()) { use w.e (entry), w.pj (neighbour posq) }
+template <int SHIFT>
+struct PairWalk {
+    const int* __restrict__ list;
+    const int4* __restrict__ posq;
+    size_t n;
+    int s, cnt, m;
+    int e, e1, e2;       // current entry, next, next-next
+    int4 pj, p1;         // current / next neighbour position
+    __device__ __forceinline__ PairWalk(const int* __restrict__ list_, size_t n_, int s_, int cnt_,
+                                        const int4* __restrict__ posq_)
+        : list(list_), posq(posq_), n(n_), s(s_), cnt(cnt_), m(-1)
+    {
+        e1 = (cnt > 0) ? list[s] : 0;
+        e2 = (cnt > 1) ? list[n + s] : 0;
+        p1 = (cnt > 0) ? posq[e1 >> SHIFT] : make_int4(0, 0, 0, 0);
+    }
+    __device__ __forceinline__ bool next()
+    {
+        if (++m >= cnt) return false;
+        e = e1; pj = p1;
+        e1 = e2;
+        if (m + 1 < cnt) p1 = posq[e1 >> SHIFT];
+        if (m + 2 < cnt) e2 = list[(size_t)(m + 2) * n + s];
+        return true;
+    }
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -39,19 +72,37 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
     }
     int na = 0, nb = 0;
     const int ca = cntA[s];
-    for (int m = 0; m < ca; ++m) {
-        const int j = listA[(size_t)m * n + s];
-        float dx, dy, dz, r2;
-        pair_vec(pi, posq[j], D, dx, dy, dz, r2);
-        if (r2 < D.rcA2) { cA[(size_t)na * n + s] = (j << NEP_SLOT_BITS) | m; ++na; }
-        else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j; ++nb; }
+    for (int m0 = 0; m0 < ca; m0 += 4) {                 // 4 independent gathers in flight
+        int j[4]; int4 pj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) j[u] = (m0 + u < ca) ? listA[(size_t)(m0 + u) * n + s] : s;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (m0 + u < ca) {
+                float dx, dy, dz, r2;
+                pair_vec(pi, pj[u], D, dx, dy, dz, r2);
+                if (r2 < D.rcA2) { cA[(size_t)na * n + s] = (j[u] << NEP_SLOT_BITS) | (m0 + u); ++na; }
+                else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j[u]; ++nb; }
+            }
+        }
     }
     const int cs = cntS[s];
-    for (int m = 0; m < cs; ++m) {
-        const int j = listS[(size_t)m * n + s];
-        float dx, dy, dz, r2;
-        pair_vec(pi, posq[j], D, dx, dy, dz, r2);
-        if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j; ++nb; }
+    for (int m0 = 0; m0 < cs; m0 += 4) {
+        int j[4]; int4 pj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) j[u] = (m0 + u < cs) ? listS[(size_t)(m0 + u) * n + s] : s;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (m0 + u < cs) {
+                float dx, dy, dz, r2;
+                pair_vec(pi, pj[u], D, dx, dy, dz, r2);
+                if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j[u]; ++nb; }
+            }
+        }
     }
     ncA[s] = na;
     ncB[s] = nb;
@@ -59,53 +110,143 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
 
 // ---------------------------------------------------------------------------------------------------
 // (a2) q_n = sum_j sum_k c^{ij}_{nk} f_k(r_ij)      Eqs. (2)-(4)
-template <int NR>
-__global__ void __launch_bounds__(128)
-k_radial(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, const int* __restrict__ ncA,
-         const int* __restrict__ cB, const int* __restrict__ ncB, const float* __restrict__ cR_t,
-         float* __restrict__ q)
+// Re-association (exact in real arithmetic): q_n = sum_t sum_k c[ti][t][n][k] F_t,k with the per-type
+// basis sums F_t,k = sum_{j of type t} f_k(r_ij), so that a pair costs the Chebyshev recurrence and one
+// FMA per k, and the coefficient contraction is done once per atom.  With f_k = (T_k + 1) f_c / 2:
+// F_k = A_k + A_0 (k >= 1), F_0 = 2 A_0, where A_k = sum_j T_k(x_ij) f_c(r_ij)/2.
+
+// one pair's contribution to A_0..A_{K-1} held in registers (K compile-time)
+template <int KP>
+__device__ __forceinline__ void radial_accumulate(float r2, float rc_inv, float* A)
 {
-    extern __shared__ float sc[];                       // [T*T][KR][NRP]
-    const int tab = D.T * D.T * D.KR * D.NRP;
-    for (int t = threadIdx.x; t < tab; t += blockDim.x) sc[t] = cR_t[t];
-    __syncthreads();
+    const float r = r2 * rsqrtf(r2);
+    const BasisHead h = basis_head<false>(r, rc_inv);
+    A[0] += h.hfc;
+    float Tkm1 = 1.0f, Tk = h.x;
+    if (KP > 1) A[1] = fmaf(Tk, h.hfc, A[1]);
+#pragma unroll
+    for (int k = 2; k < KP; ++k) {
+        const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+        Tkm1 = Tk; Tk = Tn;
+        A[k] = fmaf(Tk, h.hfc, A[k]);
+    }
+}
+
+// single-species systems: accumulators in registers.  KP = KR rounded up to a multiple of 4 (the
+// surplus accumulators are finite and multiply zero-padded coefficients).
+template <int KP>
+__global__ void __launch_bounds__(128)
+k_radial1(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, const int* __restrict__ ncA,
+          const int* __restrict__ cB, const int* __restrict__ ncB, const float* __restrict__ cR_q,
+          float* __restrict__ q)
+{
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    float qn[NR];
+    float A[KP];
 #pragma unroll
-    for (int a = 0; a < NR; ++a) qn[a] = 0.0f;
-    const int na = ncA[s], tot = na + ncB[s];
-    for (int m = 0; m < tot; ++m) {
-        const int j = (m < na) ? (cA[(size_t)m * n + s] >> NEP_SLOT_BITS) : cB[(size_t)(m - na) * n + s];
-        const int4 pj = posq[j];
-        float dx, dy, dz, r2;
-        pair_vec(pi, pj, D, dx, dy, dz, r2);
-        const float r = r2 * rsqrtf(r2);
-        const BasisHead h = basis_head<false>(r, D.rcR_inv);
-        const float* c = sc + (size_t)((pi.w * D.T + pj.w) * D.KR) * D.NRP;
-        float Tkm1 = 1.0f, Tk = h.x;
-        float f = 2.0f * h.hfc;                          // k = 0: (T_0 + 1) f_c / 2
-#pragma unroll
-        for (int a = 0; a < NR; ++a) qn[a] = fmaf(c[a], f, qn[a]);
-        if (D.KR > 1) {
-            c += D.NRP;
-            f = (Tk + 1.0f) * h.hfc;                     // k = 1
-#pragma unroll
-            for (int a = 0; a < NR; ++a) qn[a] = fmaf(c[a], f, qn[a]);
-        }
-        for (int k = 2; k < D.KR; ++k) {
-            const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-            Tkm1 = Tk; Tk = Tn;
-            c += D.NRP;
-            f = (Tk + 1.0f) * h.hfc;
-#pragma unroll
-            for (int a = 0; a < NR; ++a) qn[a] = fmaf(c[a], f, qn[a]);
+    for (int k = 0; k < KP; ++k) A[k] = 0.0f;
+    {
+        PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
+        while (w.next()) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            radial_accumulate<KP>(r2, D.rcR_inv, A);
         }
     }
+    {
+        PairWalk<0> w(cB, n, s, ncB[s], posq);
+        while (w.next()) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            radial_accumulate<KP>(r2, D.rcR_inv, A);
+        }
+    }
+    const float H = A[0];
+    A[0] = 2.0f * H;
 #pragma unroll
-    for (int a = 0; a < NR; ++a) q[(size_t)a * n + s] = qn[a];
+    for (int k = 1; k < KP; ++k) A[k] += H;
+    for (int a = 0; a < D.NR; ++a) {                     // cR_q: [NR][KP] zero-padded (T == 1)
+        const float* c = cR_q + a * KP;
+        float acc = 0.0f;
+#pragma unroll
+        for (int k = 0; k < KP; ++k) acc = fmaf(__ldg(c + k), A[k], acc);
+        q[(size_t)a * n + s] = acc;
+    }
+}
+
+// any number of species: accumulators A[t][k] in shared memory, [t][k][thread] (conflict-free).
+__device__ __forceinline__ void radial_accumulate_smem(float r2, float rc_inv, int KR, int BS, float* acc)
+{
+    const float r = r2 * rsqrtf(r2);
+    const BasisHead h = basis_head<false>(r, rc_inv);
+    acc[0] += h.hfc;
+    float Tkm1 = 1.0f, Tk = h.x;
+    if (KR > 1) acc[BS] = fmaf(Tk, h.hfc, acc[BS]);
+    for (int k = 2; k < KR; ++k) {
+        const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+        Tkm1 = Tk; Tk = Tn;
+        acc[k * BS] = fmaf(Tk, h.hfc, acc[k * BS]);
+    }
+}
+
+__global__ void
+k_radial_multi(NepDims D, int tab_stride, int tab_in_smem, const int4* __restrict__ posq, const int* __restrict__ cA,
+               const int* __restrict__ ncA, const int* __restrict__ cB, const int* __restrict__ ncB,
+               const float* __restrict__ cR_t, float* __restrict__ q)
+{
+    extern __shared__ float sm[];                        // A[T][KR][BS], then table [T*T] x tab_stride
+    const int BS = blockDim.x;
+    float* sacc = sm;
+    float* sc = sm + (size_t)D.T * D.KR * BS;
+    const int tab = tab_in_smem ? D.T * D.T * tab_stride : 0;
+    for (int t = threadIdx.x; t < tab; t += BS) sc[t] = cR_t[t];
+    for (int t = threadIdx.x; t < D.T * D.KR * BS; t += BS) sacc[t] = 0.0f;   // own column only
+    const float* ctab = tab_in_smem ? sc : cR_t;         // huge tables stay in global memory (L1)
+    __syncthreads();
+    const int s = blockIdx.x * BS + threadIdx.x;
+    if (s >= D.n) return;
+    const size_t n = (size_t)D.n;
+    const int4 pi = posq[s];
+    float* my = sacc + threadIdx.x;
+    const int tstride = D.KR * BS;
+    {
+        PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
+        while (w.next()) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            radial_accumulate_smem(r2, D.rcR_inv, D.KR, BS, my + w.pj.w * tstride);
+        }
+    }
+    {
+        PairWalk<0> w(cB, n, s, ncB[s], posq);
+        while (w.next()) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            radial_accumulate_smem(r2, D.rcR_inv, D.KR, BS, my + w.pj.w * tstride);
+        }
+    }
+    // q_n = sum_t sum_k c[ti][t][n][k] F_t,k ; table rows [tp][k][NRP], tp stride odd (conflict-free)
+    for (int a0 = 0; a0 < D.NR; a0 += 4) {
+        float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+        for (int t = 0; t < D.T; ++t) {
+            const float* A = my + t * tstride;
+            const float* c = ctab + (size_t)(pi.w * D.T + t) * tab_stride + a0;
+            const float H = A[0];
+            float F = 2.0f * H;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) acc[u] = fmaf(c[u], F, acc[u]);
+            for (int k = 1; k < D.KR; ++k) {
+                c += D.NRP;
+                F = A[k * BS] + H;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) acc[u] = fmaf(c[u], F, acc[u]);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) if (a0 + u < D.NR) q[(size_t)(a0 + u) * n + s] = acc[u];
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -150,17 +291,31 @@ __device__ __forceinline__ void q_from_S(const float* S, const NepCoef& C, float
     out[5] = C.c5[0] * s0 * s0 * s0 * s0 + C.c5[1] * s0 * s0 * p + C.c5[2] * p * p;
 }
 
+// The angular coefficient table, per type pair tp = ti*T + tj (stride `tab_stride`, odd, so that the
+// lanes of a warp -- which differ in tp -- hit different banks): rows r = 0..KA-2 hold c_{n,k=r+1},
+// row KA-1 holds csum'_n = 2 c_{n0} + sum_{k>=1} c_{nk}; NAP floats per row.  Then
+//   g_n(r) = (f_c/2) [ sum_{k>=1} c_nk T_k(x) + csum'_n ]                       (Eqs. 3-4)
+// SM = true: the table is staged in shared memory; false: read from global memory (huge tables).
+template <bool SM>
+__device__ __forceinline__ const float* stage_table(const float* __restrict__ tab_g, int count, float* sc)
+{
+    if (SM) {
+        for (int t = threadIdx.x; t < count; t += blockDim.x) sc[t] = tab_g[t];
+        __syncthreads();
+        return sc;
+    }
+    return tab_g;
+}
+
 // (a3)+(a4) S_nk = sum_j g_n(r_ij) b_k(r_hat_ij) for n = n0..n0+NCH-1, then the components.
-template <int NCH>
+template <int NCH, bool SM>
 __global__ void __launch_bounds__(128)
-k_angular(NepDims D, NepCoef C, int n0, const int4* __restrict__ posq, const int* __restrict__ cA,
+k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
           const int* __restrict__ ncA, const float* __restrict__ cA_t, float* __restrict__ S_out,
           float* __restrict__ q)
 {
-    extern __shared__ float sc[];                       // [T*T][KA][NAP]
-    const int tab = D.T * D.T * D.KA * D.NAP;
-    for (int t = threadIdx.x; t < tab; t += blockDim.x) sc[t] = cA_t[t];
-    __syncthreads();
+    extern __shared__ float sc[];
+    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
@@ -170,34 +325,27 @@ k_angular(NepDims D, NepCoef C, int n0, const int4* __restrict__ posq, const int
     for (int a = 0; a < NCH; ++a)
 #pragma unroll
         for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = 0.0f;
-    const int na = ncA[s];
-    for (int m = 0; m < na; ++m) {
-        const int j = cA[(size_t)m * n + s] >> NEP_SLOT_BITS;
-        const int4 pj = posq[j];
+    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride + n0;
+    PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
+    while (w.next()) {
         float dx, dy, dz, r2;
-        pair_vec(pi, pj, D, dx, dy, dz, r2);
+        pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<false>(r, D.rcA_inv);
-        const float* c = sc + (size_t)((pi.w * D.T + pj.w) * D.KA) * D.NAP + n0;
+        const float* c = tab_i + (size_t)w.pj.w * tab_stride;
         float g[NCH];
+#pragma unroll
+        for (int a = 0; a < NCH; ++a) g[a] = 0.0f;
         float Tkm1 = 1.0f, Tk = h.x;
-        float f = 2.0f * h.hfc;
+        for (int k = 1; k < D.KA; ++k) {
 #pragma unroll
-        for (int a = 0; a < NCH; ++a) g[a] = c[a] * f;
-        if (D.KA > 1) {
-            c += D.NAP;
-            f = (Tk + 1.0f) * h.hfc;
-#pragma unroll
-            for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], f, g[a]);
-        }
-        for (int k = 2; k < D.KA; ++k) {
+            for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], Tk, g[a]);
             const float Tn = fmaf(h.two_x, Tk, -Tkm1);
             Tkm1 = Tk; Tk = Tn;
             c += D.NAP;
-            f = (Tk + 1.0f) * h.hfc;
-#pragma unroll
-            for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], f, g[a]);
         }
+#pragma unroll
+        for (int a = 0; a < NCH; ++a) g[a] = (g[a] + c[a]) * h.hfc;
         float b[NEP_NUM_S];
         angular_b(dx * rinv, dy * rinv, dz * rinv, b);
 #pragma unroll
@@ -207,15 +355,17 @@ k_angular(NepDims D, NepCoef C, int n0, const int4* __restrict__ posq, const int
     }
 #pragma unroll
     for (int a = 0; a < NCH; ++a) {
-        float out[6];
-        q_from_S(S[a], C, out);
         const int nn = n0 + a;
+        if (nn < D.NA) {
+            float out[6];
+            q_from_S(S[a], C, out);
 #pragma unroll
-        for (int l = 0; l < 4; ++l) q[(size_t)(D.NR + l * D.NA + nn) * n + s] = out[l];
-        if (D.has4) q[(size_t)(D.NR + 4 * D.NA + nn) * n + s] = out[4];
-        if (D.has5) q[(size_t)(D.NR + (4 + D.has4) * D.NA + nn) * n + s] = out[5];
+            for (int l = 0; l < 4; ++l) q[(size_t)(D.NR + l * D.NA + nn) * n + s] = out[l];
+            if (D.has4) q[(size_t)(D.NR + 4 * D.NA + nn) * n + s] = out[4];
+            if (D.has5) q[(size_t)(D.NR + (4 + D.has4) * D.NA + nn) * n + s] = out[5];
 #pragma unroll
-        for (int k = 0; k < NEP_NUM_S; ++k) S_out[(size_t)(nn * NEP_NUM_S + k) * n + s] = S[a][k];
+            for (int k = 0; k < NEP_NUM_S; ++k) S_out[(size_t)(nn * NEP_NUM_S + k) * n + s] = S[a][k];
+        }
     }
 }
 
@@ -229,10 +379,11 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
       const float* __restrict__ b0, const float* __restrict__ w1, float b1, const float* __restrict__ cR_e,
       float* __restrict__ fp, float* __restrict__ U, float* __restrict__ Et)
 {
-    extern __shared__ float sw[];                       // w0p [H][DP], then b0 [H], w1 [H]
+    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H], then Fp_R [16][BS]
     for (int t = threadIdx.x; t < D.H * DP; t += blockDim.x) sw[t] = w0p[t];
     float* sb0 = sw + D.H * DP;
     float* sw1 = sb0 + D.H;
+    float* sfp = sw1 + D.H;
     for (int t = threadIdx.x; t < D.H; t += blockDim.x) { sb0[t] = b0[t]; sw1[t] = w1[t]; }
     __syncthreads();
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -265,16 +416,24 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
     U[s] = e - b1;
 #pragma unroll
     for (int d = 0; d < DP; ++d) if (d < D.D) fp[(size_t)d * n + s] = fv[d];
-    // E table (atom-major so that neighbours can gather a row with 128-bit loads)
+    // E table (atom-major so that neighbours can gather a row with 128-bit loads).  The radial Fp_n go
+    // through shared memory so that the n loop can be a run-time loop (NR <= 16 <= DP).
+    float* myfp = sfp + threadIdx.x;
+#pragma unroll
+    for (int d = 0; d < 16; ++d) if (d < D.NR) myfp[d * blockDim.x] = fv[d];
     const int ti = posq[s].w;
     for (int t = 0; t < D.T; ++t) {
-        const float* c = cR_e + (size_t)((ti * D.T + t) * D.NR) * D.KRP;
-        float* out = Et + ((size_t)s * D.T + t) * D.KRP;
-        for (int k = 0; k < D.KRP; ++k) {
-            float acc = 0.0f;
-#pragma unroll
-            for (int a = 0; a < 16; ++a) if (a < D.NR && a < DP) acc = fmaf(fv[a < DP ? a : 0], __ldg(c + a * D.KRP + k), acc);
-            out[k] = acc;
+        const float4* c = reinterpret_cast<const float4*>(cR_e + (size_t)((ti * D.T + t) * D.NR) * D.KRP);
+        float4* out = reinterpret_cast<float4*>(Et + ((size_t)s * D.T + t) * D.KRP);
+        for (int k4 = 0; k4 < D.KRP / 4; ++k4) {
+            float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            for (int a = 0; a < D.NR; ++a) {
+                const float f = myfp[a * blockDim.x];
+                const float4 cc = __ldg(c + a * (D.KRP / 4) + k4);
+                acc.x = fmaf(f, cc.x, acc.x); acc.y = fmaf(f, cc.y, acc.y);
+                acc.z = fmaf(f, cc.z, acc.z); acc.w = fmaf(f, cc.w, acc.w);
+            }
+            out[k4] = acc;
         }
     }
 }
@@ -307,16 +466,17 @@ __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float 
 //   grad[g b_k] = (g' - l_k g / r) b_k(u) u + (g / r) gradP_k(u),  P_k the degree-l_k polynomial of b_k.
 // With A_k = sum_n G_nk g_n, B_k = sum_n G_nk g_n':
 //   pf = [sum_k (B_k - l_k A_k / r) b_k] u + (1/r) sum_k A_k gradP_k(u).
-template <int NCH>
+// g_n and g_n' from the table of k_angular:  with G0_n = sum_{k>=1} c_nk T_k + csum'_n and
+// G1_n = sum_{k>=1} c_nk T_k'(x):  g_n = (f_c/2) G0_n,  g_n' = (f_c'/2) G0_n + (f_c/2) x'(r) G1_n;
+// T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}'.
+template <int NCH, bool SM>
 __global__ void __launch_bounds__(128)
-k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, const int4* __restrict__ posq,
+k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
                 const int* __restrict__ cA, const int* __restrict__ ncA, const float* __restrict__ cA_t,
                 const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf)
 {
-    extern __shared__ float sc[];                       // [T*T][KA][NAP]
-    const int tab = D.T * D.T * D.KA * D.NAP;
-    for (int t = threadIdx.x; t < tab; t += blockDim.x) sc[t] = cA_t[t];
-    __syncthreads();
+    extern __shared__ float sc[];
+    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
@@ -324,7 +484,7 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, const int4* __rest
     float G[NCH][NEP_NUM_S];
 #pragma unroll
     for (int a = 0; a < NCH; ++a) {
-        const int nn = n0 + a;
+        const int nn = min(n0 + a, D.NA - 1);
         float Sv[NEP_NUM_S], f3[4];
 #pragma unroll
         for (int k = 0; k < NEP_NUM_S; ++k) Sv[k] = S_in[(size_t)(nn * NEP_NUM_S + k) * n + s];
@@ -333,40 +493,38 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, const int4* __rest
         const float f4 = D.has4 ? fp[(size_t)(D.NR + 4 * D.NA + nn) * n + s] : 0.0f;
         const float f5 = D.has5 ? fp[(size_t)(D.NR + (4 + D.has4) * D.NA + nn) * n + s] : 0.0f;
         G_from_S(Sv, f3, f4, f5, C, G[a]);
+        if (n0 + a >= D.NA) {                              // padded channel of the global-table fallback
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S; ++k) G[a][k] = 0.0f;
+        }
     }
-    const int na = ncA[s];
-    for (int m = 0; m < na; ++m) {
-        const int e = cA[(size_t)m * n + s];
-        const int j = e >> NEP_SLOT_BITS, slot = e & ((1 << NEP_SLOT_BITS) - 1);
-        const int4 pj = posq[j];
+    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride + n0;
+    PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
+    while (w.next()) {
+        const int slot = w.e & ((1 << NEP_SLOT_BITS) - 1);
         float dx, dy, dz, r2;
-        pair_vec(pi, pj, D, dx, dy, dz, r2);
+        pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<true>(r, D.rcA_inv);
-        const float* c = sc + (size_t)((pi.w * D.T + pj.w) * D.KA) * D.NAP + n0;
+        const float* c = tab_i + (size_t)w.pj.w * tab_stride;
         float g[NCH], dg[NCH];
-        {   // g_n = sum_k c_nk f_k,  g_n' = sum_k c_nk f_k';  f_k' = T_k' (f_c/2) x' + (T_k + 1) f_c'/2
-            float Tkm1 = 1.0f, Tk = h.x, Ukm1 = 1.0f, Uk = h.two_x;   // T_0,T_1 ; U_0,U_1
-            float f = 2.0f * h.hfc, df = 2.0f * h.hdfc;               // k = 0
 #pragma unroll
-            for (int a = 0; a < NCH; ++a) { g[a] = c[a] * f; dg[a] = c[a] * df; }
-            if (D.KA > 1) {                                          // k = 1: T_1' = U_0 = 1
-                c += D.NAP;
-                f = (Tk + 1.0f) * h.hfc;
-                df = fmaf(Tk + 1.0f, h.hdfc, h.hfc_dx);
+        for (int a = 0; a < NCH; ++a) { g[a] = 0.0f; dg[a] = 0.0f; }
+        {
+            float Tkm1 = 1.0f, Tk = h.x, Dkm1 = 0.0f, Dk = 1.0f;      // T_0,T_1 ; T_0',T_1'
+            for (int k = 1; k < D.KA; ++k) {
 #pragma unroll
-                for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], f, g[a]); dg[a] = fmaf(c[a], df, dg[a]); }
-            }
-            for (int k = 2; k < D.KA; ++k) {                         // T_k' = k U_{k-1}
+                for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
+                const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
                 const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-                Tkm1 = Tk; Tk = Tn;
+                Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
                 c += D.NAP;
-                f = (Tk + 1.0f) * h.hfc;
-                df = fmaf(Tk + 1.0f, h.hdfc, (float)k * Uk * h.hfc_dx);
-                const float Un = fmaf(h.two_x, Uk, -Ukm1);
-                Ukm1 = Uk; Uk = Un;
+            }
 #pragma unroll
-                for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], f, g[a]); dg[a] = fmaf(c[a], df, dg[a]); }
+            for (int a = 0; a < NCH; ++a) {
+                const float G0 = g[a] + c[a];
+                g[a] = G0 * h.hfc;
+                dg[a] = fmaf(G0, h.hdfc, dg[a] * h.hfc_dx);
             }
         }
         const float x = dx * rinv, y = dy * rinv, z = dz * rinv;
@@ -417,8 +575,46 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, const int4* __rest
 // ---------------------------------------------------------------------------------------------------
 // (a6)+(a8) forces and virials.
 //  radial: dU_i/dr_ij = [sum_k E^i[tj][k] f_k'(r)] u,  dU_j/dr_ji = -[sum_k E^j[ti][k] f_k'(r)] u
+//    f_k' = P_k + f_c'/2 with P_k = T_k f_c'/2 + T_k' (f_c/2) x':  P_0 = f_c'/2, P_1 = x f_c'/2 + (f_c/2) x',
+//    P_{k+1} = 2 x P_k - P_{k-1} + 2 (f_c/2) x' T_k   (from T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}')
 //  angular: dU_i/dr_ij read at own slot, dU_j/dr_ji gathered from j's row at the reverse slot
 //  F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji)  (Eqs. 22-23);  W_i = sum_j r_ij (x) dU_j/dr_ji  (Eq. 24)
+struct FinalAcc {
+    float fx, fy, fz, w[9];
+};
+
+__device__ __forceinline__ void final_radial_pair(const NepDims& D, const int4& pi, const int4& pj, const float4* __restrict__ ei4,
+                                                  const float4* __restrict__ ej4, FinalAcc& acc)
+{
+    float dx, dy, dz, r2;
+    pair_vec(pi, pj, D, dx, dy, dz, r2);
+    const float rinv = rsqrtf(r2), r = r2 * rinv;
+    const BasisHead h = basis_head<true>(r, D.rcR_inv);
+    const float c2 = 2.0f * h.hfc_dx;
+    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
+    float mi = 0.0f, mj = 0.0f;
+    const int nk4 = D.KRP >> 2;
+    for (int k4 = 0; k4 < nk4; ++k4) {
+        const float4 a = __ldg(ei4 + k4), bq = __ldg(ej4 + k4);
+        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {bq.x, bq.y, bq.z, bq.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float df = Pa + h.hdfc;                 // f_k'; rows are zero-padded beyond KR
+            mi = fmaf(av[u], df, mi); mj = fmaf(bv[u], df, mj);
+            const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
+            const float Tn = fmaf(h.two_x, Tb, -Ta);
+            Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
+        }
+    }
+    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+    const float ft = mi + mj;                        // (dU_i/dr_ij - dU_j/dr_ji) = (mi + mj) u
+    acc.fx = fmaf(ft, ux, acc.fx); acc.fy = fmaf(ft, uy, acc.fy); acc.fz = fmaf(ft, uz, acc.fz);
+    const float px = -mj * ux, py = -mj * uy, pz = -mj * uz;   // dU_j/dr_ji
+    acc.w[0] = fmaf(dx, px, acc.w[0]); acc.w[1] = fmaf(dx, py, acc.w[1]); acc.w[2] = fmaf(dx, pz, acc.w[2]);
+    acc.w[3] = fmaf(dy, px, acc.w[3]); acc.w[4] = fmaf(dy, py, acc.w[4]); acc.w[5] = fmaf(dy, pz, acc.w[5]);
+    acc.w[6] = fmaf(dz, px, acc.w[6]); acc.w[7] = fmaf(dz, py, acc.w[7]); acc.w[8] = fmaf(dz, pz, acc.w[8]);
+}
+
 __global__ void __launch_bounds__(128)
 k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
         const int* __restrict__ cA, const int* __restrict__ ncA, const int* __restrict__ cB,
@@ -431,64 +627,42 @@ k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
     const int ti = pi.w;
-    float fx = 0.0f, fy = 0.0f, fz = 0.0f;
-    float w[9];
+    FinalAcc acc;
+    acc.fx = acc.fy = acc.fz = 0.0f;
 #pragma unroll
-    for (int a = 0; a < 9; ++a) w[a] = 0.0f;
-    const int na = ncA[s], tot = na + ncB[s];
-    const float* Ei = Et + (size_t)s * D.T * D.KRP;
-    for (int m = 0; m < tot; ++m) {
-        const int j = (m < na) ? (cA[(size_t)m * n + s] >> NEP_SLOT_BITS) : cB[(size_t)(m - na) * n + s];
-        const int4 pj = posq[j];
-        float dx, dy, dz, r2;
-        pair_vec(pi, pj, D, dx, dy, dz, r2);
-        const float rinv = rsqrtf(r2), r = r2 * rinv;
-        const BasisHead h = basis_head<true>(r, D.rcR_inv);
-        const float* ei = Ei + pj.w * D.KRP;
-        const float* ej = Et + ((size_t)j * D.T + ti) * D.KRP;
-        float Tkm1 = 1.0f, Tk = h.x, Ukm1 = 1.0f, Uk = h.two_x;
-        float df = 2.0f * h.hdfc;
-        float mi = ei[0] * df, mj = __ldg(ej) * df;
-        if (D.KR > 1) {
-            df = fmaf(Tk + 1.0f, h.hdfc, h.hfc_dx);
-            mi = fmaf(ei[1], df, mi); mj = fmaf(__ldg(ej + 1), df, mj);
+    for (int a = 0; a < 9; ++a) acc.w[a] = 0.0f;
+    const int na = ncA[s];
+    const int rowf4 = D.KRP >> 2, atomf4 = D.T * rowf4;
+    const float4* Et4 = reinterpret_cast<const float4*>(Et);
+    const float4* Ei4 = Et4 + (size_t)s * atomf4;
+    {   // angular-range pairs: radial part, then the gather of the angular partial forces
+        PairWalk<NEP_SLOT_BITS> w(cA, n, s, na, posq);
+        while (w.next()) {
+            const int j = w.e >> NEP_SLOT_BITS, slot = w.e & ((1 << NEP_SLOT_BITS) - 1);
+            // issue the dependent gathers first
+            const int rs = rev[(size_t)slot * n + s];
+            const float4 own = pf[(size_t)slot * n + s];
+            const float4 oth = __ldg(pf + (size_t)rs * n + j);
+            final_radial_pair(D, pi, w.pj, Ei4 + w.pj.w * rowf4, Et4 + (size_t)j * atomf4 + ti * rowf4, acc);
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            acc.fx += own.x - oth.x; acc.fy += own.y - oth.y; acc.fz += own.z - oth.z;
+            acc.w[0] = fmaf(dx, oth.x, acc.w[0]); acc.w[1] = fmaf(dx, oth.y, acc.w[1]); acc.w[2] = fmaf(dx, oth.z, acc.w[2]);
+            acc.w[3] = fmaf(dy, oth.x, acc.w[3]); acc.w[4] = fmaf(dy, oth.y, acc.w[4]); acc.w[5] = fmaf(dy, oth.z, acc.w[5]);
+            acc.w[6] = fmaf(dz, oth.x, acc.w[6]); acc.w[7] = fmaf(dz, oth.y, acc.w[7]); acc.w[8] = fmaf(dz, oth.z, acc.w[8]);
         }
-        for (int k = 2; k < D.KR; ++k) {
-            const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-            Tkm1 = Tk; Tk = Tn;
-            df = fmaf(Tk + 1.0f, h.hdfc, (float)k * Uk * h.hfc_dx);
-            const float Un = fmaf(h.two_x, Uk, -Ukm1);
-            Ukm1 = Uk; Uk = Un;
-            mi = fmaf(ei[k], df, mi); mj = fmaf(__ldg(ej + k), df, mj);
-        }
-        const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-        const float ft = mi + mj;                        // (dU_i/dr_ij - dU_j/dr_ji) = (mi + mj) u
-        fx = fmaf(ft, ux, fx); fy = fmaf(ft, uy, fy); fz = fmaf(ft, uz, fz);
-        const float px = -mj * ux, py = -mj * uy, pz = -mj * uz;   // dU_j/dr_ji
-        w[0] = fmaf(dx, px, w[0]); w[1] = fmaf(dx, py, w[1]); w[2] = fmaf(dx, pz, w[2]);
-        w[3] = fmaf(dy, px, w[3]); w[4] = fmaf(dy, py, w[4]); w[5] = fmaf(dy, pz, w[5]);
-        w[6] = fmaf(dz, px, w[6]); w[7] = fmaf(dz, py, w[7]); w[8] = fmaf(dz, pz, w[8]);
     }
-    for (int m = 0; m < na; ++m) {
-        const int e = cA[(size_t)m * n + s];
-        const int j = e >> NEP_SLOT_BITS, slot = e & ((1 << NEP_SLOT_BITS) - 1);
-        const int4 pj = posq[j];
-        float dx, dy, dz, r2;
-        pair_vec(pi, pj, D, dx, dy, dz, r2);
-        const float4 own = pf[(size_t)slot * n + s];
-        const int rs = rev[(size_t)slot * n + s];
-        const float4 oth = __ldg(pf + (size_t)rs * n + j);
-        fx += own.x - oth.x; fy += own.y - oth.y; fz += own.z - oth.z;
-        w[0] = fmaf(dx, oth.x, w[0]); w[1] = fmaf(dx, oth.y, w[1]); w[2] = fmaf(dx, oth.z, w[2]);
-        w[3] = fmaf(dy, oth.x, w[3]); w[4] = fmaf(dy, oth.y, w[4]); w[5] = fmaf(dy, oth.z, w[5]);
-        w[6] = fmaf(dz, oth.x, w[6]); w[7] = fmaf(dz, oth.y, w[7]); w[8] = fmaf(dz, oth.z, w[8]);
+    {   // outer shell: radial part only
+        PairWalk<0> w(cB, n, s, ncB[s], posq);
+        while (w.next())
+            final_radial_pair(D, pi, w.pj, Ei4 + w.pj.w * rowf4, Et4 + (size_t)w.e * atomf4 + ti * rowf4, acc);
     }
     const size_t i = (size_t)perm[s];
     if (e_out) e_out[i] = (double)U[s];
-    if (f_out) { f_out[3 * i + 0] = (double)fx; f_out[3 * i + 1] = (double)fy; f_out[3 * i + 2] = (double)fz; }
+    if (f_out) { f_out[3 * i + 0] = (double)acc.fx; f_out[3 * i + 1] = (double)acc.fy; f_out[3 * i + 2] = (double)acc.fz; }
     if (w_out) {
 #pragma unroll
-        for (int a = 0; a < 9; ++a) w_out[9 * i + a] = (double)w[a];
+        for (int a = 0; a < 9; ++a) w_out[9 * i + a] = (double)acc.w[a];
     }
 }
 

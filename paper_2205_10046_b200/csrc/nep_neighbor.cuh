@@ -2,12 +2,14 @@
 //
 // The paper takes the lists NN^R/NL^R, NN^A/NL^A as inputs and does not describe
 // their construction; this is the B200 design:
-//   1. positions -> 32-bit box fractions; cell id from the top bits; histogram (atomics)
+//   1. positions -> 32-bit box fractions; cell coordinates from the top bits; cells are ranked
+//      tile-major (4x4x4-cell tiles, Morton order inside a tile) so that consecutive atoms -- a warp,
+//      a thread block -- form a compact blob whose neighbourhood fits L1; histogram (atomics)
 //   2. exclusive scan of the histogram (own 3-kernel scan)
 //   3. scatter + per-cell sort by atom index  => deterministic spatial order `perm`
-//   4. one thread per atom walks the 5x5x5 stencil rows (contiguous ranges of sorted atoms),
-//      tests candidates in fp32 and resolves anything inside a guard band around a cutoff with the
-//      exact fp64 predicate of reading A8, so the sets equal an fp64 brute force bit for bit
+//   4. one thread per atom walks the 5x5x5 stencil cells, tests candidates in fp32 and resolves
+//      anything inside a guard band around a cutoff with the exact fp64 predicate of reading A8, so
+//      the sets equal an fp64 brute force bit for bit
 //   5. reverse index: slot of i in j's angular list (for the scatter-free gather of Eq. 22-24)
 // The angular-range list (|r| < rcA+skin) and the outer shell (rcA+skin <= |r| < rcR+skin) are stored
 // disjointly; the radial list is their union.
@@ -17,6 +19,7 @@
 struct BuildParams {
     int n;
     int ncx, ncy, ncz;
+    int ntx, nty;            // tiles (4 cells) per axis x, y: cell rank = tile * 64 + Morton(cell & 3)
     int hx, hy, hz;          // stencil half widths (2) -- or "all cells" when 2h+1 >= nc
     double Lx, Ly, Lz;
     double inv_Lx, inv_Ly, inv_Lz;
@@ -36,6 +39,14 @@ __device__ __forceinline__ unsigned quantize_frac(double x, double inv_L)
 
 __device__ __forceinline__ int cell_coord(unsigned q, int nc) { return (int)(((unsigned long long)q * (unsigned)nc) >> 32); }
 
+// rank of cell (cx,cy,cz) in the sorted order: 4x4x4 tiles row-major, Morton order inside a tile
+__device__ __forceinline__ unsigned cell_rank(int cx, int cy, int cz, int ntx, int nty)
+{
+    const unsigned tile = ((unsigned)(cz >> 2) * nty + (cy >> 2)) * ntx + (cx >> 2);
+    const unsigned m = (cx & 1) | ((cy & 1) << 1) | ((cz & 1) << 2) | ((cx & 2) << 2) | ((cy & 2) << 3) | ((cz & 2) << 4);
+    return tile * 64u + m;
+}
+
 // ---- 1. cell id + histogram ------------------------------------------------------------------------
 __global__ void k_cell_hist(BuildParams P, const double* __restrict__ pos, unsigned* __restrict__ cell_of,
                             unsigned* __restrict__ rank_in_cell, unsigned* __restrict__ cell_count)
@@ -45,7 +56,7 @@ __global__ void k_cell_hist(BuildParams P, const double* __restrict__ pos, unsig
     unsigned qx = quantize_frac(pos[3 * (size_t)i + 0], P.inv_Lx);
     unsigned qy = quantize_frac(pos[3 * (size_t)i + 1], P.inv_Ly);
     unsigned qz = quantize_frac(pos[3 * (size_t)i + 2], P.inv_Lz);
-    unsigned c = ((unsigned)cell_coord(qz, P.ncz) * P.ncy + cell_coord(qy, P.ncy)) * P.ncx + cell_coord(qx, P.ncx);
+    unsigned c = cell_rank(cell_coord(qx, P.ncx), cell_coord(qy, P.ncy), cell_coord(qz, P.ncz), P.ntx, P.nty);
     cell_of[i] = c;
     rank_in_cell[i] = atomicAdd(&cell_count[c], 1u);
 }
@@ -177,7 +188,7 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
     const int cy = cell_coord((unsigned)pi.y, P.ncy);
     const int cz = cell_coord((unsigned)pi.z, P.ncz);
     const bool allx = 2 * P.hx + 1 >= P.ncx, ally = 2 * P.hy + 1 >= P.ncy, allz = 2 * P.hz + 1 >= P.ncz;
-    const int nz = allz ? P.ncz : 2 * P.hz + 1, ny = ally ? P.ncy : 2 * P.hy + 1;
+    const int nz = allz ? P.ncz : 2 * P.hz + 1, ny = ally ? P.ncy : 2 * P.hy + 1, nx = allx ? P.ncx : 2 * P.hx + 1;
     int na = 0, ns = 0;
     const size_t n = (size_t)P.n;
 
@@ -187,20 +198,11 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
         for (int iy = 0; iy < ny; ++iy) {
             int yc = ally ? iy : cy - P.hy + iy;
             if (yc < 0) yc += P.ncy; else if (yc >= P.ncy) yc -= P.ncy;
-            const unsigned row = ((unsigned)zc * P.ncy + yc) * P.ncx;
-            // x range(s) of this row: contiguous in the sorted order
-            int r0a, r0b, r1a = 0, r1b = -1;
-            if (allx) { r0a = 0; r0b = P.ncx - 1; }
-            else {
-                int lo = cx - P.hx, hi = cx + P.hx;
-                if (lo < 0) { r0a = lo + P.ncx; r0b = P.ncx - 1; r1a = 0; r1b = hi; }
-                else if (hi >= P.ncx) { r0a = lo; r0b = P.ncx - 1; r1a = 0; r1b = hi - P.ncx; }
-                else { r0a = lo; r0b = hi; }
-            }
-            for (int part = 0; part < 2; ++part) {
-                const int ca = part ? r1a : r0a, cb = part ? r1b : r0b;
-                if (cb < ca) continue;
-                const int t0 = (int)cell_start[row + ca], t1 = (int)cell_start[row + cb + 1];
+            for (int ix = 0; ix < nx; ++ix) {
+                int xc = allx ? ix : cx - P.hx + ix;
+                if (xc < 0) xc += P.ncx; else if (xc >= P.ncx) xc -= P.ncx;
+                const unsigned rk = cell_rank(xc, yc, zc, P.ntx, P.nty);
+                const int t0 = (int)cell_start[rk], t1 = (int)cell_start[rk + 1];
                 for (int t = t0; t < t1; ++t) {
                     if (t == s) continue;
                     const int4 pj = posq[t];
