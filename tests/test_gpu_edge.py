@@ -1,0 +1,204 @@
+"""Edge and degenerate cases of the CUDA path against the oracle, through the C ABI (-m gpu).
+
+Empty neighbourhoods (one atom; a dilute gas where most atoms see nobody), a dimer, ragged sizes that do
+not fill a warp or a block, atoms exactly on the box faces and outside [0, L), a box of exactly the
+minimum legal size, list overflow beyond the 256-slot limit, zero-step md_step, the host-buffer entry
+points (nep_compute_host / md_run_host) against the device ones, model variants without the 4-/5-body
+blocks and with the largest supported basis sizes.
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2205_10046_b200 as p
+    p.load_library()
+    return p
+
+
+def run_both(pkg, oracle_mod, hyper, params, masses, pos, types, box, skin=0.0):
+    nep = pkg.NEP(hyper, params, masses, device=0)
+    dpos = torch.tensor(pos, device="cuda:0")
+    dtyp = torch.tensor(types, device="cuda:0")
+    nep.nep_neighbors(dpos, dtyp, box, skin)
+    for which, rc in ((0, hyper.rc_radial), (1, hyper.rc_angular)):
+        cnt, lst = nep.nep_get_neighbors(which)
+        ocnt, olst = oracle_mod.neighbors(pos, box, rc + skin)
+        cnt, lst = cnt.cpu().numpy(), lst.cpu().numpy()
+        assert np.array_equal(cnt, ocnt)
+        for i in range(len(pos)):
+            assert set(lst[i, :cnt[i]].tolist()) == set(olst[i, :ocnt[i]].tolist())
+    e, f, w = nep.nep_compute(dpos)
+    eo, fo, wo = oracle_mod.compute(hyper, params, pos, types, box)
+    e, f, w = e.cpu().numpy(), f.cpu().numpy(), w.cpu().numpy()
+    assert np.abs(e - eo).max() <= 1e-5
+    fn = np.linalg.norm(fo, axis=1, keepdims=True)
+    assert (np.abs(f - fo) <= np.maximum(1e-4, 1e-4 * fn)).all()
+    assert np.abs(f - fo).max() <= 1e-4 * max(np.abs(fo).max(), 1e-6)
+    wn = np.linalg.norm(wo, axis=1)
+    # reading A14's floor is the median |W_i|; in a dilute gas the median is 0, so the mean stands in
+    assert (np.linalg.norm(w - wo, axis=1) <= 1e-4 * np.maximum(wn, max(np.median(wn), wn.mean(), 1e-6))).all()
+    nep.close()
+    return e, f, w
+
+
+def test_single_atom_has_no_neighbours(pkg, oracle_mod):
+    """q = 0: U = sum_m w1_m tanh(-b0_m) - b1 (Eq. 1), F = 0, W = 0."""
+    cfg = W.get_config(0)
+    p = W.make_params(cfg, "stress")
+    e, f, w = run_both(pkg, oracle_mod, cfg.hyper, p, [28.0], np.array([[3.0, 4.0, 5.0]]), np.zeros(1, np.int32),
+                       np.array([30.0, 31.0, 32.0]))
+    want = float((p.w1.astype(np.float64) * np.tanh(-p.b0.astype(np.float64))).sum() - p.b1[0])
+    assert abs(e[0] - want) <= 1e-6
+    assert np.all(f == 0.0) and np.all(w == 0.0)
+
+
+@pytest.mark.parametrize("kind", ["baseline", "stress"])
+def test_dimer_and_trimer(pkg, oracle_mod, kind):
+    cfg = W.get_config(2)                                      # 2 species, rc 6/4
+    p = W.make_params(cfg, kind)
+    box = np.array([40.0, 41.0, 42.0])
+    pos = np.array([[1.0, 1.0, 1.0], [3.1, 1.7, 0.2]])
+    run_both(pkg, oracle_mod, cfg.hyper, p, cfg.masses, pos, np.array([0, 1], np.int32), box)
+    pos = np.array([[39.5, 1.0, 1.0], [1.6, 1.7, 41.2], [0.3, 3.9, 0.7]])      # across the faces
+    run_both(pkg, oracle_mod, cfg.hyper, p, cfg.masses, pos, np.array([1, 0, 1], np.int32), box)
+
+
+@pytest.mark.parametrize("n", [31, 33, 129, 257])
+def test_dilute_gas_ragged_sizes(pkg, oracle_mod, n):
+    """Most atoms have empty angular lists, many have empty radial lists; n straddles warp/block sizes."""
+    cfg = W.get_config(3)
+    p = W.make_params(cfg, "stress")
+    pos, types = W.random_cluster(n, n, cfg.hyper.n_types, 38.0, min_dist=1.6)
+    run_both(pkg, oracle_mod, cfg.hyper, p, cfg.masses, pos, types, np.array([40.0, 40.0, 40.0]), skin=0.5)
+
+
+def test_positions_on_faces_and_outside_the_box(pkg, oracle_mod):
+    """Coordinates exactly 0, exactly L, negative and beyond L: the library never requires wrapped input."""
+    cfg = W.get_config(1, (3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    pos = s.pos.copy()
+    pos[0] = [0.0, 0.0, 0.0]
+    pos[1] = [s.box[0], 2.0, 2.5]                                  # x == L
+    pos[5] += s.box * np.array([1.0, -1.0, 2.0])                   # other periodic images
+    pos[9] -= 3.0 * s.box
+    run_both(pkg, oracle_mod, cfg.hyper, p, s.masses, pos, s.types, s.box, skin=0.0)
+
+
+def test_minimum_legal_box(pkg, oracle_mod):
+    """Box edge exactly 2 (rc_radial + skin) is accepted (minimum image still unique); below is refused."""
+    cfg = W.get_config(0)
+    p = W.make_params(cfg)
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 901]))
+    box = np.array([10.0, 10.0, 10.0])
+    g = np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing="ij"), -1).reshape(-1, 3) * 2.5
+    pos = g + rng.normal(0.0, 0.1, g.shape)
+    types = np.zeros(len(pos), np.int32)
+    run_both(pkg, oracle_mod, cfg.hyper, p, [28.0], pos, types, box, skin=0.0)
+    nep = pkg.NEP(cfg.hyper, p, [28.0], device=0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_neighbors(torch.tensor(pos, device="cuda:0"), torch.tensor(types, device="cuda:0"), box * (1 - 1e-9), 0.0)
+    assert ei.value.status == -2
+    nep.close()
+
+
+def test_overflow_beyond_256_angular_neighbours_is_an_error(pkg):
+    cfg = W.get_config(0)
+    p = W.make_params(cfg)
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 902]))
+    pos = rng.uniform(0.0, 12.0, size=(3000, 3))                   # 1.7 atoms / A^3: ~470 inside 4 A
+    nep = pkg.NEP(cfg.hyper, p, [28.0], device=0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_neighbors(torch.tensor(pos, device="cuda:0"), torch.zeros(3000, dtype=torch.int32, device="cuda:0"),
+                          np.array([12.0, 12.0, 12.0]), 0.0)
+    assert ei.value.status == -4
+    nep.close()
+
+
+def test_dense_lists_regrow(pkg, oracle_mod):
+    """Three times the density the first capacity guess is sized for in one corner: lists are regrown,
+    never truncated."""
+    cfg = W.get_config(0)
+    p = W.make_params(cfg)
+    pos, types = W.random_cluster(7, 150, 1, 9.0, min_dist=1.25)
+    pos2, _ = W.random_cluster(8, 40, 1, 30.0, min_dist=2.0)
+    pos = np.concatenate([pos, pos2 + 10.0])
+    run_both(pkg, oracle_mod, cfg.hyper, p, [28.0], pos, np.zeros(len(pos), np.int32), np.array([42.0, 42.0, 42.0]), skin=1.0)
+
+
+@pytest.mark.parametrize("l4,l5", [(0, 0), (2, 0), (0, 1)])
+def test_models_without_many_body_blocks(pkg, oracle_mod, l4, l5):
+    cfg = W.get_config(3, (4, 4, 3))
+    cfg = replace(cfg, hyper=replace(cfg.hyper, l_max_4b=l4, l_max_5b=l5))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    run_both(pkg, oracle_mod, cfg.hyper, p, s.masses, s.pos, s.types, s.box, skin=0.3)
+
+
+@pytest.mark.parametrize("nr,na,kr,ka,H,T", [(0, 0, 0, 0, 1, 1), (1, 7, 3, 15, 7, 3), (15, 15, 31, 31, 120, 2), (12, 8, 12, 8, 50, 3)])
+def test_hyperparameter_extremes(pkg, oracle_mod, nr, na, kr, ka, H, T):
+    """Smallest and largest supported basis / channel / neuron counts; (12,8,12,8,50,3) is the shape of
+    the paper's MgAlCu model (nep.in)."""
+    base = W.get_config(2, (3, 3, 3))
+    hy = W.Hyper(n_types=T, rc_radial=6.0 if T != 3 else 6.0, rc_angular=3.5, n_max_radial=nr, n_max_angular=na,
+                 basis_radial=kr, basis_angular=ka, n_neurons=H)
+    cfg = replace(base, hyper=hy, masses=tuple([24.0, 27.0, 64.0][:T]), species_rule="random" if T > 1 else "single")
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    run_both(pkg, oracle_mod, hy, p, s.masses, s.pos, s.types, s.box, skin=0.0)
+
+
+def test_md_step_zero_steps_and_state_errors(pkg):
+    cfg = W.get_config(0)
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel, types = (torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0"),
+                       torch.tensor(s.types, device="cuda:0"))
+    with pytest.raises(pkg.NepError) as ei:
+        nep.n = len(s.pos)
+        nep.md_step(pos, vel, 1.0, 1, 1, 0.0)
+    assert ei.value.status == -5
+    nep.nep_neighbors(pos, types, s.box, 0.0)
+    p0, v0 = pos.clone(), vel.clone()
+    nep.md_step(pos, vel, 1.0, 0, 1, 0.0)                         # evaluates, moves nothing
+    assert torch.equal(pos, p0) and torch.equal(vel, v0)
+    e, f, w = nep.nep_get_last()
+    e2, f2, w2 = nep.nep_compute(pos)
+    assert torch.equal(e, e2) and torch.equal(f, f2) and torch.equal(w, w2)     # deterministic, bit for bit
+    with pytest.raises(pkg.NepError):
+        nep.md_step(pos, vel, 1.0, 1, 0, 0.0)                     # rebuild_every < 1
+    nep.close()
+
+
+def test_host_buffer_entry_points_match_device_ones(pkg):
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    n = len(s.pos)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel, types = (torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0"),
+                       torch.tensor(s.types, device="cuda:0"))
+    nep.nep_neighbors(pos, types, s.box, 1.0)
+    e, f, w = nep.nep_compute(pos)
+    eh, fh, wh = np.zeros(n), np.zeros((n, 3)), np.zeros((n, 9))
+    nep.nep_compute_host(s.pos, s.types, s.box, 1.0, eh, fh, wh)
+    assert np.array_equal(eh, e.cpu().numpy()) and np.array_equal(fh, f.cpu().numpy()) and np.array_equal(wh, w.cpu().numpy())
+    # 12 steps in one device call == 12 host calls of one step (same rebuild cadence), bit for bit
+    nep.nep_neighbors(pos, types, s.box, 1.0)
+    nep.md_step(pos, vel, 1.0, 12, 5, 1.0)
+    ph, vh = s.pos.copy(), s.vel.copy()
+    nep.md_run_host(ph, vh, s.types, s.box, 1.0, 1, 5, 1.0, eh, fh, wh)
+    for _ in range(11):
+        nep.md_run_host(ph, vh, None, None, 1.0, 1, 5, 1.0, eh, fh, wh)
+    assert np.array_equal(ph, pos.cpu().numpy()) and np.array_equal(vh, vel.cpu().numpy())
+    e, f, w = nep.nep_get_last()
+    assert np.array_equal(fh, f.cpu().numpy())
+    nep.close()
