@@ -102,6 +102,7 @@ int alloc_lists(nep_t* nep, int capA, int capS)
     NEP_TRY(dev_alloc(nep, &nep->listA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->rev, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->cA, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->cAr, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->pf, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->listS, (size_t)capS * n));
     NEP_TRY(dev_alloc(nep, &nep->cB, (size_t)(capA + capS) * n));
@@ -126,6 +127,8 @@ int alloc_atoms(nep_t* nep, int64_t n)
     NEP_TRY(dev_alloc(nep, &nep->cntS, N));
     NEP_TRY(dev_alloc(nep, &nep->ncA, N));
     NEP_TRY(dev_alloc(nep, &nep->ncB, N));
+    NEP_TRY(dev_alloc(nep, &nep->maskA, N * ((1 << NEP_SLOT_BITS) / 64)));
+    NEP_TRY(dev_alloc(nep, &nep->fa, N));
     NEP_TRY(dev_alloc(nep, &nep->q, N * d.D));
     NEP_TRY(dev_alloc(nep, &nep->fp, N * d.D));
     NEP_TRY(dev_alloc(nep, &nep->S, N * d.NA * NEP_NUM_S));
@@ -201,6 +204,7 @@ int build_lists(nep_t* nep, const double* pos_dev)
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
     NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA, nep->listA, nep->cntA, nep->rev));
+    nep->d.maskW = nep->maxA_skin > 0 ? (nep->maxA_skin + 63) / 64 : 1;
     nep->steps_since_build = 0;
     nep->have_lists = true;
     return NEP_OK;
@@ -254,8 +258,8 @@ int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int ac
         NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->strideA, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q)));
     } else {
         NEP_TRY(allow_smem(nep, k_force_angular<NCH, SM>, sm));
-        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->strideA, nep->posq, nep->cA, nep->ncA,
-                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf)));
+        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->strideA, nep->posq, nep->cAr, nep->ncA,
+                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf, nep->fa)));
     }
     return NEP_OK;
 }
@@ -321,6 +325,30 @@ int dispatch_ann(nep_t* nep)
     return nep_fail(nep, NEP_ERR_INVALID_ARG, "descriptor too long");
 }
 
+template <int NK4>
+int launch_final(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    NEP_LAUNCH(NEP_K_FINAL, k_final<NK4><<<div_up(d.n, 128), 128, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->Et,
+                                                            nep->pf, nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out));
+    return NEP_OK;
+}
+
+int dispatch_final(nep_t* nep)
+{
+    switch (nep->d.KRP >> 2) {
+        case 1: return launch_final<1>(nep);
+        case 2: return launch_final<2>(nep);
+        case 3: return launch_final<3>(nep);
+        case 4: return launch_final<4>(nep);
+        case 5: return launch_final<5>(nep);
+        case 6: return launch_final<6>(nep);
+        case 7: return launch_final<7>(nep);
+        case 8: return launch_final<8>(nep);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
+}
+
 int evaluate(nep_t* nep, const double* pos_dev)
 {
     static const NepCoef C = make_coef();
@@ -331,13 +359,13 @@ int evaluate(nep_t* nep, const double* pos_dev)
                                                1.0 / nep->box[2], nep->posq));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
     NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
-                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->disp_max));
+                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->maskA, nep->disp_max));
+    NEP_LAUNCH(NEP_K_CREV, k_crev<<<div_up(n, 256), 256, 0, st>>>(d, nep->cA, nep->ncA, nep->rev, nep->maskA, nep->cAr));
     NEP_TRY(dispatch_radial(nep));
     NEP_TRY(dispatch_angular(nep, C, false));
     NEP_TRY(dispatch_ann(nep));
     NEP_TRY(dispatch_angular(nep, C, true));
-    NEP_LAUNCH(NEP_K_FINAL, k_final<<<div_up(n, 128), 128, 0, st>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->rev, nep->Et,
-                                            nep->pf, nep->U, nep->e_out, nep->f_out, nep->w_out));
+    NEP_TRY(dispatch_final(nep));
     nep->have_eval = true;
     return NEP_OK;
 }
@@ -716,7 +744,7 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 
 // ---- measurement support ----------------------------------------------------------------------------------
 static const char* const kKernelNames[NEP_K_COUNT] = {
-    "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
+    "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "crev", "radial",
     "angular", "ann", "force_angular", "final", "kick_drift", "kick", "export"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }

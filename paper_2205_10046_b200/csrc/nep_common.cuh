@@ -18,7 +18,7 @@
 // Kernel ids for the optional per-kernel CUDA-event timing (nep_profile_*; bench.py's roofline leg).
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
-    NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FINAL,
+    NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_CREV, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FINAL,
     NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_EXPORT, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
@@ -34,6 +34,7 @@ struct NepDims {
     float rcR, rcA, rcR_inv, rcA_inv, rcR2, rcA2;
     float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
     int capA, capS;              // storage rows of the skin lists (angular-range part, outer shell)
+    int maskW;                   // 64-bit words per atom of the in-cutoff mask over the angular skin slots
 };
 
 struct nep_ctx {
@@ -99,7 +100,9 @@ struct nep_ctx {
     int* listA;  int* cntA;  // [capA][n] sorted indices with |r| < rcA + skin
     int* listS;  int* cntS;  // [capS][n] rcA + skin <= |r| < rcR + skin
     unsigned char* rev;      // [capA][n] slot of i in j's listA
-    int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|slot with |r| < rcA
+    int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|skin slot with |r| < rcA
+    int* cAr;                // [capA][n] per step: packed (j<<8)|slot of i in j's cA column (k_angular)
+    unsigned long long* maskA;  // [n][maskW] per step: bit m set <=> skin slot m of listA is inside rcA
     int* cB; int* ncB;       // [capA+capS][n] per step: j with rcA <= |r| < rcR
     int* flags;              // [4] device: 0 overflow A, 1 overflow S, 2 max cntA, 3 max (cntA+cntS)
     unsigned* disp_max;      // [1] device: float bits of max displacement^2 since build
@@ -110,7 +113,8 @@ struct nep_ctx {
     float* S;                // [NA*24][n]
     float* Et;               // [n][T][KRP]  E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
     float* U;                // [n]
-    float4* pf;              // [capA][n] angular partial forces dU_i/dr_ij at skin slots
+    float4* pf;              // [capA][n] received angular partial forces: pf[m][i] = dU_j/dr_ji, j = cA[m][i]
+    float4* fa;              // [n] sum_j dU_i/dr_ij over the angular pairs of i
     double* e_out;           // [n]    orig order
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]

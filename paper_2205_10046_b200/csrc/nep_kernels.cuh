@@ -59,7 +59,7 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
          const int* __restrict__ listA, const int* __restrict__ cntA,
          const int* __restrict__ listS, const int* __restrict__ cntS,
          int* __restrict__ cA, int* __restrict__ ncA, int* __restrict__ cB, int* __restrict__ ncB,
-         unsigned* __restrict__ disp_max)
+         unsigned long long* __restrict__ maskA, unsigned* __restrict__ disp_max)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
@@ -72,6 +72,10 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
     }
     int na = 0, nb = 0;
     const int ca = cntA[s];
+    // maskA[s]: bit m <=> skin slot m is inside rcA this step.  The compact slot of skin slot m is the
+    // number of set bits below m, which is how a neighbour finds the slot of i in i's cA column.
+    unsigned long long mword = 0ull;
+    unsigned long long* mrow = maskA + (size_t)s * D.maskW;
     for (int m0 = 0; m0 < ca; m0 += 4) {                 // 4 independent gathers in flight
         int j[4]; int4 pj[4];
 #pragma unroll
@@ -83,11 +87,16 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
             if (m0 + u < ca) {
                 float dx, dy, dz, r2;
                 pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                if (r2 < D.rcA2) { cA[(size_t)na * n + s] = (j[u] << NEP_SLOT_BITS) | (m0 + u); ++na; }
+                if (r2 < D.rcA2) {
+                    cA[(size_t)na * n + s] = (j[u] << NEP_SLOT_BITS) | (m0 + u); ++na;
+                    mword |= 1ull << ((m0 + u) & 63);
+                }
                 else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j[u]; ++nb; }
             }
         }
+        if (((m0 + 4) & 63) == 0) { mrow[m0 >> 6] = mword; mword = 0ull; }     // word complete
     }
+    if (((ca + 3) & ~3) & 63) mrow[ca >> 6] = mword;     // last word not completed inside the loop
     const int cs = cntS[s];
     for (int m0 = 0; m0 < cs; m0 += 4) {
         int j[4]; int4 pj[4];
@@ -106,6 +115,39 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
     }
     ncA[s] = na;
     ncB[s] = nb;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// cAr[m][i] = (j << 8) | (slot of i in j's cA column), j = cA[m][i]: the address at which atom i
+// delivers dU_i/dr_ij to atom j (k_force_angular).  That slot is the number of in-cutoff skin slots of j
+// below the skin slot of i in j's listA (rev, built with the lists): a popcount of j's mask.
+__global__ void __launch_bounds__(256)
+k_crev(NepDims D, const int* __restrict__ cA, const int* __restrict__ ncA, const unsigned char* __restrict__ rev,
+       const unsigned long long* __restrict__ maskA, int* __restrict__ cAr)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= D.n) return;
+    const size_t n = (size_t)D.n;
+    const int na = ncA[s];
+    for (int m0 = 0; m0 < na; m0 += 4) {                 // 4 independent dependent-load chains in flight
+        int e[4], rs[4];
+        unsigned long long mw[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) e[u] = (m0 + u < na) ? cA[(size_t)(m0 + u) * n + s] : 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) rs[u] = (m0 + u < na) ? rev[(size_t)(e[u] & ((1 << NEP_SLOT_BITS) - 1)) * n + s] : 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) mw[u] = (m0 + u < na) ? maskA[(size_t)(e[u] >> NEP_SLOT_BITS) * D.maskW + (rs[u] >> 6)] : 0ull;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (m0 + u < na) {
+                const int j = e[u] >> NEP_SLOT_BITS;
+                int cs = __popcll(mw[u] & ((1ull << (rs[u] & 63)) - 1ull));
+                for (int ww = 0; ww < (rs[u] >> 6); ++ww) cs += __popcll(maskA[(size_t)j * D.maskW + ww]);
+                cAr[(size_t)(m0 + u) * n + s] = (j << NEP_SLOT_BITS) | cs;
+            }
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -472,8 +514,9 @@ __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float 
 template <int NCH, bool SM>
 __global__ void __launch_bounds__(128)
 k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
-                const int* __restrict__ cA, const int* __restrict__ ncA, const float* __restrict__ cA_t,
-                const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf)
+                const int* __restrict__ cAr, const int* __restrict__ ncA, const float* __restrict__ cA_t,
+                const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf,
+                float4* __restrict__ fa)
 {
     extern __shared__ float sc[];
     const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
@@ -499,9 +542,9 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, co
         }
     }
     const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride + n0;
-    PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
+    float sx = 0.0f, sy = 0.0f, sz = 0.0f;                 // sum_j dU_i/dr_ij
+    PairWalk<NEP_SLOT_BITS> w(cAr, n, s, ncA[s], posq);
     while (w.next()) {
-        const int slot = w.e & ((1 << NEP_SLOT_BITS) - 1);
         float dx, dy, dz, r2;
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -566,10 +609,15 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, co
         NEP_ACC(23, 4, 4.0f * y * (3.0f * x2 - y2), 4.0f * x * (x2 - 3.0f * y2), 0.0f)
 #undef NEP_ACC
         float4 out = make_float4(fmaf(cu, x, rinv * vx), fmaf(cu, y, rinv * vy), fmaf(cu, z, rinv * vz), 0.0f);
-        float4* dst = pf + (size_t)slot * n + s;
+        sx += out.x; sy += out.y; sz += out.z;
+        // delivered to the receiver: row (slot of i in j's column) of atom j -- a fire-and-forget store
+        // here instead of a dependent gather in k_final; only this thread ever touches that element
+        float4* dst = pf + (size_t)(w.e & ((1 << NEP_SLOT_BITS) - 1)) * n + (w.e >> NEP_SLOT_BITS);
         if (accumulate) { const float4 o = *dst; out.x += o.x; out.y += o.y; out.z += o.z; }
         *dst = out;
     }
+    if (accumulate) { const float4 o = fa[s]; sx += o.x; sy += o.y; sz += o.z; }
+    fa[s] = make_float4(sx, sy, sz, 0.0f);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -577,49 +625,66 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, co
 //  radial: dU_i/dr_ij = [sum_k E^i[tj][k] f_k'(r)] u,  dU_j/dr_ji = -[sum_k E^j[ti][k] f_k'(r)] u
 //    f_k' = P_k + f_c'/2 with P_k = T_k f_c'/2 + T_k' (f_c/2) x':  P_0 = f_c'/2, P_1 = x f_c'/2 + (f_c/2) x',
 //    P_{k+1} = 2 x P_k - P_{k-1} + 2 (f_c/2) x' T_k   (from T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}')
-//  angular: dU_i/dr_ij read at own slot, dU_j/dr_ji gathered from j's row at the reverse slot
+//  angular: sum_j dU_i/dr_ij was reduced by k_force_angular (fa); dU_j/dr_ji was delivered by atom j to
+//    row m of this atom's column (pf[m][i], j = cA[m][i]) -- coalesced reads, no gather, no atomics
 //  F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji)  (Eqs. 22-23);  W_i = sum_j r_ij (x) dU_j/dr_ji  (Eq. 24)
+// The row E^j[ti] of the next neighbour is fetched while the current pair is computed (NK4 = KRP/4
+// float4 registers), because that gather is the long-latency operation of this kernel.
 struct FinalAcc {
     float fx, fy, fz, w[9];
 };
 
-__device__ __forceinline__ void final_radial_pair(const NepDims& D, const int4& pi, const int4& pj, const float4* __restrict__ ei4,
-                                                  const float4* __restrict__ ej4, FinalAcc& acc)
+__device__ __forceinline__ void virial_add(FinalAcc& acc, float dx, float dy, float dz, float px, float py, float pz)
 {
-    float dx, dy, dz, r2;
-    pair_vec(pi, pj, D, dx, dy, dz, r2);
-    const float rinv = rsqrtf(r2), r = r2 * rinv;
-    const BasisHead h = basis_head<true>(r, D.rcR_inv);
-    const float c2 = 2.0f * h.hfc_dx;
-    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
-    float mi = 0.0f, mj = 0.0f;
-    const int nk4 = D.KRP >> 2;
-    for (int k4 = 0; k4 < nk4; ++k4) {
-        const float4 a = __ldg(ei4 + k4), bq = __ldg(ej4 + k4);
-        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {bq.x, bq.y, bq.z, bq.w};
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const float df = Pa + h.hdfc;                 // f_k'; rows are zero-padded beyond KR
-            mi = fmaf(av[u], df, mi); mj = fmaf(bv[u], df, mj);
-            const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
-            const float Tn = fmaf(h.two_x, Tb, -Ta);
-            Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
-        }
-    }
-    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-    const float ft = mi + mj;                        // (dU_i/dr_ij - dU_j/dr_ji) = (mi + mj) u
-    acc.fx = fmaf(ft, ux, acc.fx); acc.fy = fmaf(ft, uy, acc.fy); acc.fz = fmaf(ft, uz, acc.fz);
-    const float px = -mj * ux, py = -mj * uy, pz = -mj * uz;   // dU_j/dr_ji
     acc.w[0] = fmaf(dx, px, acc.w[0]); acc.w[1] = fmaf(dx, py, acc.w[1]); acc.w[2] = fmaf(dx, pz, acc.w[2]);
     acc.w[3] = fmaf(dy, px, acc.w[3]); acc.w[4] = fmaf(dy, py, acc.w[4]); acc.w[5] = fmaf(dy, pz, acc.w[5]);
     acc.w[6] = fmaf(dz, px, acc.w[6]); acc.w[7] = fmaf(dz, py, acc.w[7]); acc.w[8] = fmaf(dz, pz, acc.w[8]);
 }
 
+// radial part of one pair; ei4 = row E^i[tj] (own atom, L1), ej = row E^j[ti] (prefetched registers)
+template <int NK4>
+__device__ __forceinline__ void final_radial_pair(const NepDims& D, float dx, float dy, float dz, float r2,
+                                                  const float4* __restrict__ ei4, const float4 (&ej)[NK4], FinalAcc& acc)
+{
+    const float rinv = rsqrtf(r2), r = r2 * rinv;
+    const BasisHead h = basis_head<true>(r, D.rcR_inv);
+    const float c2 = 2.0f * h.hfc_dx;
+    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
+    float mi = 0.0f, mj = 0.0f;
+#pragma unroll
+    for (int k4 = 0; k4 < NK4; ++k4) {
+        const float4 a = __ldg(ei4 + k4), bq = ej[k4];
+        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {bq.x, bq.y, bq.z, bq.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (4 * k4 + u < D.KR) {                      // uniform: skips the padding of the last group
+                const float df = Pa + h.hdfc;             // f_k'
+                mi = fmaf(av[u], df, mi); mj = fmaf(bv[u], df, mj);
+                const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
+                const float Tn = fmaf(h.two_x, Tb, -Ta);
+                Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
+            }
+        }
+    }
+    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+    const float ft = mi + mj;                        // (dU_i/dr_ij - dU_j/dr_ji) = (mi + mj) u
+    acc.fx = fmaf(ft, ux, acc.fx); acc.fy = fmaf(ft, uy, acc.fy); acc.fz = fmaf(ft, uz, acc.fz);
+    virial_add(acc, dx, dy, dz, -mj * ux, -mj * uy, -mj * uz);   // dU_j/dr_ji
+}
+
+template <int NK4>
+__device__ __forceinline__ void load_erow(float4 (&e)[NK4], const float4* __restrict__ row)
+{
+#pragma unroll
+    for (int k4 = 0; k4 < NK4; ++k4) e[k4] = __ldg(row + k4);
+}
+
+template <int NK4>
 __global__ void __launch_bounds__(128)
 k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
         const int* __restrict__ cA, const int* __restrict__ ncA, const int* __restrict__ cB,
-        const int* __restrict__ ncB, const unsigned char* __restrict__ rev, const float* __restrict__ Et,
-        const float4* __restrict__ pf, const float* __restrict__ U,
+        const int* __restrict__ ncB, const float* __restrict__ Et,
+        const float4* __restrict__ pf, const float4* __restrict__ fa, const float* __restrict__ U,
         double* __restrict__ e_out, double* __restrict__ f_out, double* __restrict__ w_out)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -628,34 +693,45 @@ k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
     const int4 pi = posq[s];
     const int ti = pi.w;
     FinalAcc acc;
-    acc.fx = acc.fy = acc.fz = 0.0f;
+    {
+        const float4 own = fa[s];
+        acc.fx = own.x; acc.fy = own.y; acc.fz = own.z;
+    }
 #pragma unroll
     for (int a = 0; a < 9; ++a) acc.w[a] = 0.0f;
     const int na = ncA[s];
-    const int rowf4 = D.KRP >> 2, atomf4 = D.T * rowf4;
+    const int atomf4 = D.T * NK4;
     const float4* Et4 = reinterpret_cast<const float4*>(Et);
     const float4* Ei4 = Et4 + (size_t)s * atomf4;
-    {   // angular-range pairs: radial part, then the gather of the angular partial forces
+    const float4* Ej4 = Et4 + ti * NK4;                  // + j * atomf4: row E^j[ti]
+    float4 ecur[NK4], enext[NK4];
+    {   // angular-range pairs: radial part + the angular partial forces received from the neighbours
         PairWalk<NEP_SLOT_BITS> w(cA, n, s, na, posq);
+        if (na > 0) load_erow<NK4>(enext, Ej4 + (size_t)(w.e1 >> NEP_SLOT_BITS) * atomf4);
         while (w.next()) {
-            const int j = w.e >> NEP_SLOT_BITS, slot = w.e & ((1 << NEP_SLOT_BITS) - 1);
-            // issue the dependent gathers first
-            const int rs = rev[(size_t)slot * n + s];
-            const float4 own = pf[(size_t)slot * n + s];
-            const float4 oth = __ldg(pf + (size_t)rs * n + j);
-            final_radial_pair(D, pi, w.pj, Ei4 + w.pj.w * rowf4, Et4 + (size_t)j * atomf4 + ti * rowf4, acc);
+            const float4 oth = pf[(size_t)w.m * n + s];
+#pragma unroll
+            for (int k4 = 0; k4 < NK4; ++k4) ecur[k4] = enext[k4];
+            if (w.m + 1 < na) load_erow<NK4>(enext, Ej4 + (size_t)(w.e1 >> NEP_SLOT_BITS) * atomf4);
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            acc.fx += own.x - oth.x; acc.fy += own.y - oth.y; acc.fz += own.z - oth.z;
-            acc.w[0] = fmaf(dx, oth.x, acc.w[0]); acc.w[1] = fmaf(dx, oth.y, acc.w[1]); acc.w[2] = fmaf(dx, oth.z, acc.w[2]);
-            acc.w[3] = fmaf(dy, oth.x, acc.w[3]); acc.w[4] = fmaf(dy, oth.y, acc.w[4]); acc.w[5] = fmaf(dy, oth.z, acc.w[5]);
-            acc.w[6] = fmaf(dz, oth.x, acc.w[6]); acc.w[7] = fmaf(dz, oth.y, acc.w[7]); acc.w[8] = fmaf(dz, oth.z, acc.w[8]);
+            final_radial_pair<NK4>(D, dx, dy, dz, r2, Ei4 + w.pj.w * NK4, ecur, acc);
+            acc.fx -= oth.x; acc.fy -= oth.y; acc.fz -= oth.z;
+            virial_add(acc, dx, dy, dz, oth.x, oth.y, oth.z);
         }
     }
     {   // outer shell: radial part only
-        PairWalk<0> w(cB, n, s, ncB[s], posq);
-        while (w.next())
-            final_radial_pair(D, pi, w.pj, Ei4 + w.pj.w * rowf4, Et4 + (size_t)w.e * atomf4 + ti * rowf4, acc);
+        const int nb = ncB[s];
+        PairWalk<0> w(cB, n, s, nb, posq);
+        if (nb > 0) load_erow<NK4>(enext, Ej4 + (size_t)w.e1 * atomf4);
+        while (w.next()) {
+#pragma unroll
+            for (int k4 = 0; k4 < NK4; ++k4) ecur[k4] = enext[k4];
+            if (w.m + 1 < nb) load_erow<NK4>(enext, Ej4 + (size_t)w.e1 * atomf4);
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            final_radial_pair<NK4>(D, dx, dy, dz, r2, Ei4 + w.pj.w * NK4, ecur, acc);
+        }
     }
     const size_t i = (size_t)perm[s];
     if (e_out) e_out[i] = (double)U[s];
