@@ -221,6 +221,28 @@ int launch_radial1(nep_t* nep)
     return NEP_OK;
 }
 
+template <int KP>
+int launch_radial_multi(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    const size_t tab_bytes = sizeof(float) * (size_t)d.T * d.T * nep->strideR;
+    const bool tab_in_smem = tab_bytes <= kSmemTableMax;
+    int bs = 128;
+    auto smem = [&](int b) { return sizeof(float) * (size_t)d.T * KP * b + (tab_in_smem ? tab_bytes : 0); };
+    while (bs > 32 && smem(bs) > 160 * 1024) bs >>= 1;
+    const size_t sm = smem(bs);
+    if (tab_in_smem) {
+        NEP_TRY(allow_smem(nep, k_radial_multi<KP, true>, sm));
+        NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, true><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
+                                                                                        nep->cB, nep->ncB, nep->cR_t, nep->q)));
+    } else {
+        NEP_TRY(allow_smem(nep, k_radial_multi<KP, false>, sm));
+        NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, false><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
+                                                                                         nep->cB, nep->ncB, nep->cR_t, nep->q)));
+    }
+    return NEP_OK;
+}
+
 int dispatch_radial(nep_t* nep)
 {
     const NepDims& d = nep->d;
@@ -237,15 +259,17 @@ int dispatch_radial(nep_t* nep)
         }
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
     }
-    const size_t tab_bytes = sizeof(float) * (size_t)d.T * d.T * nep->strideR;
-    const int tab_in_smem = tab_bytes <= kSmemTableMax;
-    int bs = 128;
-    while (bs > 32 && sizeof(float) * (size_t)d.T * d.KR * bs + (tab_in_smem ? tab_bytes : 0) > 160 * 1024) bs >>= 1;
-    const size_t sm = sizeof(float) * (size_t)d.T * d.KR * bs + (tab_in_smem ? tab_bytes : 0);
-    NEP_TRY(allow_smem(nep, k_radial_multi, sm));
-    NEP_LAUNCH(NEP_K_RADIAL, k_radial_multi<<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, tab_in_smem, nep->posq, nep->cA, nep->ncA,
-                                                                          nep->cB, nep->ncB, nep->cR_t, nep->q));
-    return NEP_OK;
+    switch (nep->KP) {
+        case 4: return launch_radial_multi<4>(nep);
+        case 8: return launch_radial_multi<8>(nep);
+        case 12: return launch_radial_multi<12>(nep);
+        case 16: return launch_radial_multi<16>(nep);
+        case 20: return launch_radial_multi<20>(nep);
+        case 24: return launch_radial_multi<24>(nep);
+        case 28: return launch_radial_multi<28>(nep);
+        case 32: return launch_radial_multi<32>(nep);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
 }
 
 template <int NCH, bool SM>
@@ -297,9 +321,12 @@ template <int DP>
 int launch_ann(nep_t* nep)
 {
     const NepDims& d = nep->d;
-    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H + 16 * 128);
+    int bs = 128;                                        // smaller blocks for networks whose weights fill shared memory
+    auto smem = [&](int b) { return sizeof(float) * ((size_t)d.H * DP + 2 * d.H + (size_t)(16 + d.H) * b); };
+    while (bs > 32 && smem(bs) > 110 * 1024) bs >>= 1;
+    const size_t sm = smem(bs);
     NEP_TRY(allow_smem(nep, k_ann<DP>, sm));
-    NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
+    NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
                                                         nep->cR_e, nep->fp, nep->U, nep->Et));
     return NEP_OK;
 }

@@ -218,47 +218,45 @@ k_radial1(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, 
     }
 }
 
-// any number of species: accumulators A[t][k] in shared memory, [t][k][thread] (conflict-free).
-__device__ __forceinline__ void radial_accumulate_smem(float r2, float rc_inv, int KR, int BS, float* acc)
+// any number of species: accumulators A[t][k] in shared memory, [t][k][thread] (conflict-free).  KP = KR
+// rounded up to a multiple of 4 is a compile-time constant so that the read-modify-write of one pair is
+// KP independent LDS, then the recurrence and FMAs, then KP STS (surplus terms are finite and meet
+// zero-padded coefficients).
+template <int KP>
+__device__ __forceinline__ void radial_accumulate_smem(float r2, float rc_inv, int BS, float* acc)
 {
-    const float r = r2 * rsqrtf(r2);
-    const BasisHead h = basis_head<false>(r, rc_inv);
-    acc[0] += h.hfc;
-    float Tkm1 = 1.0f, Tk = h.x;
-    if (KR > 1) acc[BS] = fmaf(Tk, h.hfc, acc[BS]);
-    for (int k = 2; k < KR; ++k) {
-        const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-        Tkm1 = Tk; Tk = Tn;
-        acc[k * BS] = fmaf(Tk, h.hfc, acc[k * BS]);
-    }
+    float A[KP];
+#pragma unroll
+    for (int k = 0; k < KP; ++k) A[k] = acc[k * BS];
+    radial_accumulate<KP>(r2, rc_inv, A);
+#pragma unroll
+    for (int k = 0; k < KP; ++k) acc[k * BS] = A[k];
 }
 
-__global__ void
-k_radial_multi(NepDims D, int tab_stride, int tab_in_smem, const int4* __restrict__ posq, const int* __restrict__ cA,
+template <int KP, bool TAB_SM>
+__global__ void __launch_bounds__(128)
+k_radial_multi(NepDims D, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
                const int* __restrict__ ncA, const int* __restrict__ cB, const int* __restrict__ ncB,
                const float* __restrict__ cR_t, float* __restrict__ q)
 {
-    extern __shared__ float sm[];                        // A[T][KR][BS], then table [T*T] x tab_stride
+    extern __shared__ float sm[];                        // A[T][KP][BS], then table [T*T] x tab_stride
     const int BS = blockDim.x;
-    float* sacc = sm;
-    float* sc = sm + (size_t)D.T * D.KR * BS;
-    const int tab = tab_in_smem ? D.T * D.T * tab_stride : 0;
-    for (int t = threadIdx.x; t < tab; t += BS) sc[t] = cR_t[t];
-    for (int t = threadIdx.x; t < D.T * D.KR * BS; t += BS) sacc[t] = 0.0f;   // own column only
-    const float* ctab = tab_in_smem ? sc : cR_t;         // huge tables stay in global memory (L1)
+    float* sc = sm + (size_t)D.T * KP * BS;
+    if (TAB_SM) for (int t = threadIdx.x; t < D.T * D.T * tab_stride; t += BS) sc[t] = cR_t[t];
+    float* my = sm + threadIdx.x;
+    for (int t = 0; t < D.T * KP; ++t) my[t * BS] = 0.0f;
     __syncthreads();
     const int s = blockIdx.x * BS + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    float* my = sacc + threadIdx.x;
-    const int tstride = D.KR * BS;
+    const int tstride = KP * BS;
     {
         PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
         while (w.next()) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate_smem(r2, D.rcR_inv, D.KR, BS, my + w.pj.w * tstride);
+            radial_accumulate_smem<KP>(r2, D.rcR_inv, BS, my + w.pj.w * tstride);
         }
     }
     {
@@ -266,7 +264,7 @@ k_radial_multi(NepDims D, int tab_stride, int tab_in_smem, const int4* __restric
         while (w.next()) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate_smem(r2, D.rcR_inv, D.KR, BS, my + w.pj.w * tstride);
+            radial_accumulate_smem<KP>(r2, D.rcR_inv, BS, my + w.pj.w * tstride);
         }
     }
     // q_n = sum_t sum_k c[ti][t][n][k] F_t,k ; table rows [tp][k][NRP], tp stride odd (conflict-free)
@@ -274,14 +272,14 @@ k_radial_multi(NepDims D, int tab_stride, int tab_in_smem, const int4* __restric
         float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
         for (int t = 0; t < D.T; ++t) {
             const float* A = my + t * tstride;
-            const float* c = ctab + (size_t)(pi.w * D.T + t) * tab_stride + a0;
+            const size_t off = (size_t)(pi.w * D.T + t) * tab_stride + a0;
             const float H = A[0];
             float F = 2.0f * H;
+            for (int k = 0; k < D.KR; ++k) {
+                if (k > 0) F = A[k * BS] + H;
+                float c[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) acc[u] = fmaf(c[u], F, acc[u]);
-            for (int k = 1; k < D.KR; ++k) {
-                c += D.NRP;
-                F = A[k * BS] + H;
+                for (int u = 0; u < 4; ++u) c[u] = TAB_SM ? sc[off + k * D.NRP + u] : __ldg(cR_t + off + k * D.NRP + u);
 #pragma unroll
                 for (int u = 0; u < 4; ++u) acc[u] = fmaf(c[u], F, acc[u]);
             }
@@ -421,48 +419,67 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
       const float* __restrict__ b0, const float* __restrict__ w1, float b1, const float* __restrict__ cR_e,
       float* __restrict__ fp, float* __restrict__ U, float* __restrict__ Et)
 {
-    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H], then Fp_R [16][BS]
-    for (int t = threadIdx.x; t < D.H * DP; t += blockDim.x) sw[t] = w0p[t];
+    // Two phases so that neither holds q and Fp in registers at once (occupancy): forward with q in
+    // registers, leaving cf_m = w1_m (1 - tanh^2) in shared memory ([m][thread], conflict-free); backward
+    // Fp_v = sum_m cf_m w0_mv eight components at a time.  Weight reads are warp-uniform (broadcast).
+    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H], Fp_R [16][BS], cf [H][BS]
+    const int BS = blockDim.x;
+    for (int t = threadIdx.x; t < D.H * DP; t += BS) sw[t] = w0p[t];
     float* sb0 = sw + D.H * DP;
     float* sw1 = sb0 + D.H;
     float* sfp = sw1 + D.H;
-    for (int t = threadIdx.x; t < D.H; t += blockDim.x) { sb0[t] = b0[t]; sw1[t] = w1[t]; }
+    float* scf = sfp + 16 * BS;
+    for (int t = threadIdx.x; t < D.H; t += BS) { sb0[t] = b0[t]; sw1[t] = w1[t]; }
     __syncthreads();
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = blockIdx.x * BS + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
-    float qv[DP], fv[DP];
-#pragma unroll
-    for (int d = 0; d < DP; ++d) { qv[d] = (d < D.D) ? q[(size_t)d * n + s] : 0.0f; fv[d] = 0.0f; }
+    float* mycf = scf + threadIdx.x;
     float e = 0.0f;
-    for (int m = 0; m < D.H; ++m) {
-        const float4* w = reinterpret_cast<const float4*>(sw + m * DP);
-        float a0 = -sb0[m], a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+    {
+        float qv[DP];
 #pragma unroll
-        for (int d4 = 0; d4 < DP / 4; ++d4) {
-            const float4 ww = w[d4];
-            a0 = fmaf(ww.x, qv[4 * d4 + 0], a0); a1 = fmaf(ww.y, qv[4 * d4 + 1], a1);
-            a2 = fmaf(ww.z, qv[4 * d4 + 2], a2); a3 = fmaf(ww.w, qv[4 * d4 + 3], a3);
+        for (int d = 0; d < DP; ++d) qv[d] = (d < D.D) ? q[(size_t)d * n + s] : 0.0f;
+        for (int m = 0; m < D.H; ++m) {
+            const float4* w = reinterpret_cast<const float4*>(sw + m * DP);
+            float a0 = -sb0[m], a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+#pragma unroll
+            for (int d4 = 0; d4 < DP / 4; ++d4) {
+                const float4 ww = w[d4];
+                a0 = fmaf(ww.x, qv[4 * d4 + 0], a0); a1 = fmaf(ww.y, qv[4 * d4 + 1], a1);
+                a2 = fmaf(ww.z, qv[4 * d4 + 2], a2); a3 = fmaf(ww.w, qv[4 * d4 + 3], a3);
+            }
+            const float x1 = tanhf((a0 + a1) + (a2 + a3));
+            const float w1m = sw1[m];
+            e = fmaf(w1m, x1, e);
+            mycf[m * BS] = w1m * (1.0f - x1 * x1);
         }
-        const float x1 = tanhf((a0 + a1) + (a2 + a3));
-        const float w1m = sw1[m];
-        e = fmaf(w1m, x1, e);
-        const float cf = w1m * (1.0f - x1 * x1);
+    }
+    float* myfp = sfp + threadIdx.x;
 #pragma unroll
-        for (int d4 = 0; d4 < DP / 4; ++d4) {
-            const float4 ww = w[d4];
-            fv[4 * d4 + 0] = fmaf(cf, ww.x, fv[4 * d4 + 0]); fv[4 * d4 + 1] = fmaf(cf, ww.y, fv[4 * d4 + 1]);
-            fv[4 * d4 + 2] = fmaf(cf, ww.z, fv[4 * d4 + 2]); fv[4 * d4 + 3] = fmaf(cf, ww.w, fv[4 * d4 + 3]);
+    for (int d0 = 0; d0 < DP; d0 += 8) {
+        float acc[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc[u] = 0.0f;
+        const float4* w = reinterpret_cast<const float4*>(sw + d0);
+        for (int m = 0; m < D.H; ++m) {
+            const float cf = mycf[m * BS];
+            const float4 wa = w[m * (DP / 4)], wb = w[m * (DP / 4) + 1];
+            acc[0] = fmaf(cf, wa.x, acc[0]); acc[1] = fmaf(cf, wa.y, acc[1]);
+            acc[2] = fmaf(cf, wa.z, acc[2]); acc[3] = fmaf(cf, wa.w, acc[3]);
+            acc[4] = fmaf(cf, wb.x, acc[4]); acc[5] = fmaf(cf, wb.y, acc[5]);
+            acc[6] = fmaf(cf, wb.z, acc[6]); acc[7] = fmaf(cf, wb.w, acc[7]);
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (d0 + u < D.D) fp[(size_t)(d0 + u) * n + s] = acc[u];
+            // the radial Fp_n go through shared memory so that the E-table loop below can be a run-time
+            // loop over n (NR <= 16 <= DP)
+            if (d0 + u < 16 && d0 + u < D.NR) myfp[(d0 + u) * BS] = acc[u];
         }
     }
     U[s] = e - b1;
-#pragma unroll
-    for (int d = 0; d < DP; ++d) if (d < D.D) fp[(size_t)d * n + s] = fv[d];
-    // E table (atom-major so that neighbours can gather a row with 128-bit loads).  The radial Fp_n go
-    // through shared memory so that the n loop can be a run-time loop (NR <= 16 <= DP).
-    float* myfp = sfp + threadIdx.x;
-#pragma unroll
-    for (int d = 0; d < 16; ++d) if (d < D.NR) myfp[d * blockDim.x] = fv[d];
+    // E table (atom-major so that neighbours can gather a row with 128-bit loads)
     const int ti = posq[s].w;
     for (int t = 0; t < D.T; ++t) {
         const float4* c = reinterpret_cast<const float4*>(cR_e + (size_t)((ti * D.T + t) * D.NR) * D.KRP);
@@ -470,7 +487,7 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
         for (int k4 = 0; k4 < D.KRP / 4; ++k4) {
             float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
             for (int a = 0; a < D.NR; ++a) {
-                const float f = myfp[a * blockDim.x];
+                const float f = myfp[a * BS];
                 const float4 cc = __ldg(c + a * (D.KRP / 4) + k4);
                 acc.x = fmaf(f, cc.x, acc.x); acc.y = fmaf(f, cc.y, acc.y);
                 acc.z = fmaf(f, cc.z, acc.z); acc.w = fmaf(f, cc.w, acc.w);

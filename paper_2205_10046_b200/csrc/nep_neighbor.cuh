@@ -246,13 +246,24 @@ __global__ void k_build_rev(int n, int capA, const int* __restrict__ listA, cons
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
+    // Both atoms walk the same stencil in the same order, and j sees i in the mirrored stencil cell, so i
+    // sits near slot cnt_j - 1 - m * cnt_j / cnt_i of j's list: search outwards from there (two probes in
+    // flight per round).  The entry exists because the predicate is symmetric bit for bit.
     const int c = cntA[s];
     for (int m = 0; m < c; ++m) {
         const int j = listA[(size_t)m * n + s];
         const int cj = cntA[j];
-        int found = 0;
-        for (int mm = 0; mm < cj; ++mm)
-            if (listA[(size_t)mm * n + j] == s) { found = mm; break; }
+        const int* col = listA + j;
+        int hi = cj - 1 - (m * cj) / c;
+        hi = max(0, min(hi, cj - 1));
+        int lo = hi - 1, found = 0;
+        while (lo >= 0 || hi < cj) {
+            const int vlo = (lo >= 0) ? col[(size_t)lo * n] : -1;
+            const int vhi = (hi < cj) ? col[(size_t)hi * n] : -1;
+            if (vhi == s) { found = hi; break; }
+            if (vlo == s) { found = lo; break; }
+            --lo; ++hi;
+        }
         rev[(size_t)m * n + s] = (unsigned char)found;
     }
 }
