@@ -272,47 +272,53 @@ int dispatch_radial(nep_t* nep)
     return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
 }
 
+// resident blocks of a persistent (dynamic-tile) kernel: SMs x occupancy, at most one block per 128 atoms
+template <typename K>
+int persistent_grid(nep_t* nep, K kernel, size_t smem, int* grid)
+{
+    int per_sm = 0;
+    NEP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 128, smem));
+    if (per_sm < 1) per_sm = 1;
+    *grid = (int)fmin((double)div_up(nep->d.n, 128), (double)per_sm * nep->num_sms);
+    return NEP_OK;
+}
+
 template <int NCH, bool SM>
-int launch_angular(nep_t* nep, const NepCoef& C, int n0, bool force_pass, int accumulate)
+int launch_angular(nep_t* nep, const NepCoef& C, int p, bool force_pass)
 {
     const NepDims& d = nep->d;
-    const size_t sm = SM ? sizeof(float) * (size_t)d.T * d.T * nep->strideA : 0;
+    const int stride = nep->pass_stride[p], n0 = nep->pass_n0[p];
+    const float* tab = nep->cA_t + nep->pass_off[p];
+    const size_t sm = SM ? sizeof(float) * (size_t)d.T * d.T * stride : 0;
+    int grid = 0;
     if (!force_pass) {
         NEP_TRY(allow_smem(nep, k_angular<NCH, SM>, sm));
-        NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, nep->strideA, nep->posq, nep->cA, nep->ncA, nep->cA_t, nep->S, nep->q)));
+        NEP_TRY(persistent_grid(nep, k_angular<NCH, SM>, sm, &grid));
+        NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, stride, nep->posq, nep->cA, nep->ncA, tab, nep->S, nep->q,
+                                                                                     nep->tile_ctr + p)));
     } else {
         NEP_TRY(allow_smem(nep, k_force_angular<NCH, SM>, sm));
-        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, C, n0, accumulate, nep->strideA, nep->posq, nep->cAr, nep->ncA,
-                                                                                                 nep->cA_t, nep->S, nep->fp, nep->pf, nep->fa)));
+        NEP_TRY(persistent_grid(nep, k_force_angular<NCH, SM>, sm, &grid));
+        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, p > 0, stride, nep->posq, nep->cAr, nep->ncA, tab,
+                                                                                                 nep->S, nep->fp, nep->pf, nep->fa, nep->tile_ctr + 16 + p)));
     }
     return NEP_OK;
 }
 
 int dispatch_angular(nep_t* nep, const NepCoef& C, bool force_pass)
 {
-    const int NA = nep->d.NA;
-    if (sizeof(float) * (size_t)nep->d.T * nep->d.T * nep->strideA > kSmemTableMax) {
-        // huge coefficient table: passes of 4 channels reading the table from global memory; the table
-        // is zero-padded to NAP = round_up4(NA) columns and surplus channels are not stored
-        for (int n0 = 0; n0 < NA; n0 += 4) NEP_TRY((launch_angular<4, false>(nep, C, n0, force_pass, n0 > 0)));
-        return NEP_OK;
-    }
-    const int npass = (NA + nep->nch_max - 1) / nep->nch_max;
-    const int base = NA / npass, rem = NA % npass;
-    int n0 = 0;
-    for (int p = 0; p < npass; ++p) {
-        const int nch = base + (p < rem ? 1 : 0);
+    for (int p = 0; p < nep->n_pass; ++p) {
         int rc;
-        switch (nch) {
-            case 1: rc = launch_angular<1, true>(nep, C, n0, force_pass, p > 0); break;
-            case 2: rc = launch_angular<2, true>(nep, C, n0, force_pass, p > 0); break;
-            case 3: rc = launch_angular<3, true>(nep, C, n0, force_pass, p > 0); break;
-            case 4: rc = launch_angular<4, true>(nep, C, n0, force_pass, p > 0); break;
-            case 5: rc = launch_angular<5, true>(nep, C, n0, force_pass, p > 0); break;
-            default: rc = launch_angular<6, true>(nep, C, n0, force_pass, p > 0); break;
+        if (!nep->angular_tab_smem) { rc = launch_angular<4, false>(nep, C, p, force_pass); }
+        else switch (nep->pass_nch[p]) {
+            case 1: rc = launch_angular<1, true>(nep, C, p, force_pass); break;
+            case 2: rc = launch_angular<2, true>(nep, C, p, force_pass); break;
+            case 3: rc = launch_angular<3, true>(nep, C, p, force_pass); break;
+            case 4: rc = launch_angular<4, true>(nep, C, p, force_pass); break;
+            case 5: rc = launch_angular<5, true>(nep, C, p, force_pass); break;
+            default: rc = launch_angular<6, true>(nep, C, p, force_pass); break;
         }
         if (rc != NEP_OK) return rc;
-        n0 += nch;
     }
     return NEP_OK;
 }
@@ -385,6 +391,7 @@ int evaluate(nep_t* nep, const double* pos_dev)
     NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, 1.0 / nep->box[0], 1.0 / nep->box[1],
                                                1.0 / nep->box[2], nep->posq));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
+    NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
     NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
                                              nep->cA, nep->ncA, nep->cB, nep->ncB, nep->maskA, nep->disp_max));
     NEP_LAUNCH(NEP_K_CREV, k_crev<<<div_up(n, 256), 256, 0, st>>>(d, nep->cA, nep->ncA, nep->rev, nep->maskA, nep->cAr));
@@ -495,6 +502,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     d.NA = h->n_max_angular + 1; d.KA = h->basis_angular + 1;
     d.D = n_des(h); d.H = h->n_neurons;
     d.NRP = round_up4(d.NR); d.NAP = round_up4(d.NA); d.KRP = round_up4(d.KR);
+    d.KAR = 1 + round_up4(d.KA - 1);
     d.has4 = h->l_max_4b >= 2; d.has5 = h->l_max_5b >= 1; d.nblk = 4 + d.has4 + d.has5;
     d.rcR = (float)h->rc_radial; d.rcA = (float)h->rc_angular;
     d.rcR_inv = (float)(1.0 / h->rc_radial); d.rcA_inv = (float)(1.0 / h->rc_angular);
@@ -510,10 +518,31 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     const int T = d.T, TT = T * T;
     nep->KP = round_up4(d.KR);
     nep->strideR = (d.KR * d.NRP) | 1;
-    nep->strideA = (d.KA * d.NAP) | 1;
     nep->nch_max = 5;
     if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) nep->nch_max = v; }
-    std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f), cAt((size_t)TT * nep->strideA, 0.0f);
+    {   // angular passes: at most nch_max channels each, tables staged in shared memory; if a table would
+        // not fit there, passes of 4 channels read it from global memory (zero-padded surplus channels)
+        {
+            cudaDeviceProp prop;
+            if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); delete nep; return NEP_ERR_CUDA; }
+            nep->num_sms = prop.multiProcessorCount;
+        }
+        auto stride_of = [&](int nch) { return 4 * (((d.KAR * round_up4(nch)) / 4) | 1); };
+        const int npass = (d.NA + nep->nch_max - 1) / nep->nch_max;
+        const int base = d.NA / npass, rem = d.NA % npass;
+        nep->angular_tab_smem = sizeof(float) * (size_t)TT * stride_of(base + (rem ? 1 : 0)) <= kSmemTableMax;
+        int n0 = 0, off = 0;
+        nep->n_pass = 0;
+        while (n0 < d.NA) {
+            const int p = nep->n_pass++;
+            const int nch = nep->angular_tab_smem ? base + (p < rem ? 1 : 0) : 4;
+            nep->pass_n0[p] = n0; nep->pass_nch[p] = nch; nep->pass_off[p] = off; nep->pass_stride[p] = stride_of(nch);
+            off += TT * nep->pass_stride[p];
+            n0 += nch;
+        }
+    }
+    std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f);
+    std::vector<float> cAt((size_t)nep->pass_off[nep->n_pass - 1] + (size_t)TT * nep->pass_stride[nep->n_pass - 1], 0.0f);
     std::vector<float> cRq((size_t)d.NR * nep->KP, 0.0f);
     std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
     for (int tt = 0; tt < TT; ++tt) {
@@ -524,14 +553,18 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
                 cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
                 if (TT == 1) cRq[(size_t)nn * nep->KP + k] = v;
             }
-        for (int nn = 0; nn < d.NA; ++nn) {
-            const float* c = c_angular + ((size_t)tt * d.NA + nn) * d.KA;
-            double csum = 2.0 * (double)c[0];                      // csum'_n = 2 c_n0 + sum_{k>=1} c_nk
-            for (int k = 1; k < d.KA; ++k) {
-                cAt[(size_t)tt * nep->strideA + (size_t)(k - 1) * d.NAP + nn] = c[k];
-                csum += (double)c[k];
+        for (int p = 0; p < nep->n_pass; ++p) {
+            const int NCHP = round_up4(nep->pass_nch[p]);
+            float* tab = cAt.data() + nep->pass_off[p] + (size_t)tt * nep->pass_stride[p];
+            for (int a = 0; a < nep->pass_nch[p] && nep->pass_n0[p] + a < d.NA; ++a) {
+                const float* c = c_angular + ((size_t)tt * d.NA + nep->pass_n0[p] + a) * d.KA;
+                double csum = 2.0 * (double)c[0];                  // csum'_n = 2 c_n0 + sum_{k>=1} c_nk
+                for (int k = 1; k < d.KA; ++k) {
+                    tab[(size_t)k * NCHP + a] = c[k];
+                    csum += (double)c[k];
+                }
+                tab[a] = (float)csum;
             }
-            cAt[(size_t)tt * nep->strideA + (size_t)(d.KA - 1) * d.NAP + nn] = (float)csum;
         }
     }
     for (int m = 0; m < d.H; ++m)
@@ -557,6 +590,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     UPLOAD(mass_dev, vm);
 #undef UPLOAD
     rc = dev_alloc(nep, &nep->flags, 8);
+    if (rc == NEP_OK) rc = dev_alloc(nep, &nep->tile_ctr, 64);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 1);
     if (rc != NEP_OK) { nep_destroy(nep); return rc; }
     cudaMemset(nep->disp_max, 0, sizeof(unsigned));

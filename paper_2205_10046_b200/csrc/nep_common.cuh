@@ -30,6 +30,7 @@ struct NepDims {
     int T, NR, KR, NA, KA, D, H;
     int NRP, NAP;                // NR, NA rounded up to a multiple of 4 (row stride of the c tables)
     int KRP;                     // KR rounded up to 4 (row stride of the per-atom E table)
+    int KAR;                     // rows of an angular coefficient table: 1 + (KA - 1 rounded up to 4)
     int nblk, has4, has5;        // descriptor blocks after the radial one; 4-/5-body present
     float rcR, rcA, rcR_inv, rcA_inv, rcR2, rcA2;
     float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
@@ -56,9 +57,14 @@ struct nep_ctx {
     // model (device)
     float* cR_t;     // [T*T] x strideR: rows [k][NRP]   c_radial with the n-values of one k contiguous
     float* cR_q;     // [NR][KP]  (T == 1 only) zero-padded rows for k_radial1
-    float* cA_t;     // [T*T] x strideA: rows k = 1..KA-1 then csum' (see k_angular), NAP floats each
+    float* cA_t;     // per angular pass: [T*T] x pass_stride: KAR rows of round_up4(nch) floats (see k_angular)
+    int n_pass;              // angular passes (channels n0 .. n0+nch-1 each)
+    int pass_n0[16], pass_nch[16], pass_off[16], pass_stride[16];   // offsets / strides in floats
+    bool angular_tab_smem;   // tables staged in shared memory (else read from global memory)
+    int* tile_ctr;           // [64] device: dynamic tile counters of the angular kernels (zeroed per evaluation)
+    int num_sms;
     float* cR_e;     // [T(ti)][T(tj)][NR][KRP]  for the per-atom E table
-    int strideR, strideA;   // odd type-pair strides (floats) of cR_t / cA_t: bank-conflict-free lookups
+    int strideR;            // odd type-pair stride (floats) of cR_t: bank-conflict-free lookups
     int KP;                 // KR rounded up to a multiple of 4
     int nch_max;            // angular n-values per pass (<= NEP_NCH_MAX)
     float* w0p;      // [H][DP] rows padded with zeros to DP
@@ -224,22 +230,32 @@ struct BasisHead {
     float hfc_dx;         // (f_c / 2) * dx/dr
 };
 
+// f_c needs cos(pi t), f_c' needs sin(pi t), t = r/rc in [0,1).  With u = t - 1/2 in [-1/2, 1/2):
+// cos(pi t) = -sin(pi u), sin(pi t) = cos(pi u); both by minimax polynomials in u^2 (degree 9 / 10, error
+// < 1e-8 before rounding -- as good as fp32 allows), constants 1/4 and -pi/4 folded into the coefficients.
 template <bool WITH_DERIV>
 __device__ __forceinline__ BasisHead basis_head(float r, float rc_inv)
 {
     BasisHead b;
-    float t = r * rc_inv;
-    float y = t - 1.0f;
-    b.x = 2.0f * y * y - 1.0f;
+    const float t = r * rc_inv;
+    const float y = t - 1.0f;
+    b.x = fmaf(2.0f * y, y, -1.0f);
     b.two_x = 2.0f * b.x;
+    const float u = t - 0.5f, v = u * u;
+    float ps = fmaf(1.941441508e-02f, v, -1.495728214e-01f);       // sin(pi u) / (4 u)
+    ps = fmaf(ps, v, 6.375193808e-01f);
+    ps = fmaf(ps, v, -1.291927521e+00f);
+    ps = fmaf(ps, v, 7.853981600e-01f);
+    b.hfc = fmaf(-u, ps, 0.25f);                                   // (1 + cos(pi t)) / 4
     if (WITH_DERIV) {
-        float s, c;
-        sincospif(t, &s, &c);
-        b.hfc = 0.25f * c + 0.25f;
-        b.hdfc = -0.25f * 3.14159265358979323846f * rc_inv * s;
+        float pc = fmaf(1.916082836e-02f, v, -1.845193348e-01f);   // -(pi/4) cos(pi u)
+        pc = fmaf(pc, v, 1.048673055e+00f);
+        pc = fmaf(pc, v, -3.187702720e+00f);
+        pc = fmaf(pc, v, 3.875784535e+00f);
+        pc = fmaf(pc, v, -7.853981632e-01f);
+        b.hdfc = pc * rc_inv;                                      // -(pi / 4 rc) sin(pi t)
         b.hfc_dx = b.hfc * (4.0f * y * rc_inv);
     } else {
-        b.hfc = 0.25f * cospif(t) + 0.25f;
         b.hdfc = 0.0f;
         b.hfc_dx = 0.0f;
     }

@@ -331,33 +331,53 @@ __device__ __forceinline__ void q_from_S(const float* S, const NepCoef& C, float
     out[5] = C.c5[0] * s0 * s0 * s0 * s0 + C.c5[1] * s0 * s0 * p + C.c5[2] * p * p;
 }
 
-// The angular coefficient table, per type pair tp = ti*T + tj (stride `tab_stride`, odd, so that the
-// lanes of a warp -- which differ in tp -- hit different banks): rows r = 0..KA-2 hold c_{n,k=r+1},
-// row KA-1 holds csum'_n = 2 c_{n0} + sum_{k>=1} c_{nk}; NAP floats per row.  Then
-//   g_n(r) = (f_c/2) [ sum_{k>=1} c_nk T_k(x) + csum'_n ]                       (Eqs. 3-4)
+// The angular coefficient table of one pass (channels n0 .. n0+NCH-1), per type pair tp = ti*T + tj:
+// KAR rows of NCHP = round_up4(NCH) floats.  Row 0 holds csum'_n = 2 c_{n0} + sum_{k>=1} c_{nk}, row k
+// (1 <= k < KA) holds c_{nk}, rows KA..KAR-1 are zero (KAR - 1 is a multiple of 4 so that the k loop
+// unrolls by 4).  Then   g_n(r) = (f_c/2) [ csum'_n + sum_{k>=1} c_nk T_k(x) ]            (Eqs. 3-4)
+// The type-pair stride is an odd number of float4, so rows are 16-byte aligned (128-bit loads) and the
+// lanes of a warp -- which differ in tp -- fall into different bank groups.
 // SM = true: the table is staged in shared memory; false: read from global memory (huge tables).
 template <bool SM>
 __device__ __forceinline__ const float* stage_table(const float* __restrict__ tab_g, int count, float* sc)
 {
     if (SM) {
-        for (int t = threadIdx.x; t < count; t += blockDim.x) sc[t] = tab_g[t];
+        const float4* g4 = reinterpret_cast<const float4*>(tab_g);
+        float4* s4 = reinterpret_cast<float4*>(sc);
+        for (int t = threadIdx.x; t < count / 4; t += blockDim.x) s4[t] = g4[t];
         __syncthreads();
         return sc;
     }
     return tab_g;
 }
 
-// (a3)+(a4) S_nk = sum_j g_n(r_ij) b_k(r_hat_ij) for n = n0..n0+NCH-1, then the components.
-template <int NCH, bool SM>
-__global__ void __launch_bounds__(128)
-k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
-          const int* __restrict__ ncA, const float* __restrict__ cA_t, float* __restrict__ S_out,
-          float* __restrict__ q)
+template <int NCH>
+__device__ __forceinline__ void load_row(const float4* __restrict__ row, float* c)
 {
-    extern __shared__ float sc[];
-    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= D.n) return;
+#pragma unroll
+    for (int q4 = 0; q4 < (NCH + 3) / 4; ++q4) {
+        const float4 v = row[q4];
+        c[4 * q4 + 0] = v.x; c[4 * q4 + 1] = v.y; c[4 * q4 + 2] = v.z; c[4 * q4 + 3] = v.w;
+    }
+}
+
+// Warps take 32-atom tiles from a global counter (dynamic, in spatial order): the coefficient table is
+// staged once per resident block, and a warp that drew short neighbour lists simply takes the next tile.
+__device__ __forceinline__ int next_tile(int* __restrict__ ctr)
+{
+    int tile = 0;
+    if ((threadIdx.x & 31) == 0) tile = atomicAdd(ctr, 1);
+    return __shfl_sync(0xffffffffu, tile, 0);
+}
+
+// (a3)+(a4) S_nk = sum_j g_n(r_ij) b_k(r_hat_ij) for n = n0..n0+NCH-1, then the components.
+template <int NCH>
+__device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C, int n0, int tab_stride, const float* tab,
+                                             const int4* __restrict__ posq, const int* __restrict__ cA,
+                                             const int* __restrict__ ncA, float* __restrict__ S_out,
+                                             float* __restrict__ q, int s)
+{
+    constexpr int N4 = (NCH + 3) / 4;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
     float S[NCH][NEP_NUM_S];
@@ -365,27 +385,30 @@ k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__
     for (int a = 0; a < NCH; ++a)
 #pragma unroll
         for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = 0.0f;
-    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride + n0;
+    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride;
     PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
     while (w.next()) {
         float dx, dy, dz, r2;
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<false>(r, D.rcA_inv);
-        const float* c = tab_i + (size_t)w.pj.w * tab_stride;
-        float g[NCH];
-#pragma unroll
-        for (int a = 0; a < NCH; ++a) g[a] = 0.0f;
+        const float4* c4 = reinterpret_cast<const float4*>(tab_i + w.pj.w * tab_stride);
+        float g[4 * N4];
+        load_row<NCH>(c4, g);                              // csum'
         float Tkm1 = 1.0f, Tk = h.x;
-        for (int k = 1; k < D.KA; ++k) {
+        for (int r0 = 1; r0 < D.KAR; r0 += 4) {
 #pragma unroll
-            for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], Tk, g[a]);
-            const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-            Tkm1 = Tk; Tk = Tn;
-            c += D.NAP;
+            for (int u = 0; u < 4; ++u) {
+                float c[4 * N4];
+                load_row<NCH>(c4 + (r0 + u) * N4, c);
+#pragma unroll
+                for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], Tk, g[a]);
+                const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+                Tkm1 = Tk; Tk = Tn;
+            }
         }
 #pragma unroll
-        for (int a = 0; a < NCH; ++a) g[a] = (g[a] + c[a]) * h.hfc;
+        for (int a = 0; a < NCH; ++a) g[a] *= h.hfc;
         float b[NEP_NUM_S];
         angular_b(dx * rinv, dy * rinv, dz * rinv, b);
 #pragma unroll
@@ -393,19 +416,38 @@ k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__
 #pragma unroll
             for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = fmaf(g[a], b[k], S[a][k]);
     }
+    float* qa = q + (size_t)D.NR * n + s;                  // angular blocks: qa[(blk * NA + nn) * n]
+    float* Sp = S_out + (size_t)(n0 * NEP_NUM_S) * n + s;
 #pragma unroll
     for (int a = 0; a < NCH; ++a) {
         const int nn = n0 + a;
         if (nn < D.NA) {
             float out[6];
             q_from_S(S[a], C, out);
+            float* qp = qa + (size_t)nn * n;
+            const size_t blk = (size_t)D.NA * n;
 #pragma unroll
-            for (int l = 0; l < 4; ++l) q[(size_t)(D.NR + l * D.NA + nn) * n + s] = out[l];
-            if (D.has4) q[(size_t)(D.NR + 4 * D.NA + nn) * n + s] = out[4];
-            if (D.has5) q[(size_t)(D.NR + (4 + D.has4) * D.NA + nn) * n + s] = out[5];
+            for (int l = 0; l < 4; ++l) { *qp = out[l]; qp += blk; }
+            if (D.has4) { *qp = out[4]; qp += blk; }
+            if (D.has5) *qp = out[5];
 #pragma unroll
-            for (int k = 0; k < NEP_NUM_S; ++k) S_out[(size_t)(nn * NEP_NUM_S + k) * n + s] = S[a][k];
+            for (int k = 0; k < NEP_NUM_S; ++k) { *Sp = S[a][k]; Sp += n; }
         }
+    }
+}
+
+template <int NCH, bool SM>
+__global__ void __launch_bounds__(128)
+k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
+          const int* __restrict__ ncA, const float* __restrict__ cA_t, float* __restrict__ S_out,
+          float* __restrict__ q, int* __restrict__ tile_ctr)
+{
+    extern __shared__ __align__(16) float sc[];
+    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
+    const int ntile = (D.n + 31) >> 5;
+    for (int tile = next_tile(tile_ctr); tile < ntile; tile = next_tile(tile_ctr)) {
+        const int s = tile * 32 + (threadIdx.x & 31);
+        if (s < D.n) angular_atom<NCH>(D, C, n0, tab_stride, tab, posq, cA, ncA, S_out, q, s);
     }
 }
 
@@ -528,37 +570,41 @@ __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float 
 // g_n and g_n' from the table of k_angular:  with G0_n = sum_{k>=1} c_nk T_k + csum'_n and
 // G1_n = sum_{k>=1} c_nk T_k'(x):  g_n = (f_c/2) G0_n,  g_n' = (f_c'/2) G0_n + (f_c/2) x'(r) G1_n;
 // T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}'.
-template <int NCH, bool SM>
-__global__ void __launch_bounds__(128)
-k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
-                const int* __restrict__ cAr, const int* __restrict__ ncA, const float* __restrict__ cA_t,
-                const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf,
-                float4* __restrict__ fa)
+template <int NCH>
+__device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCoef& C, int n0, int accumulate, int tab_stride,
+                                                   const float* tab, const int4* __restrict__ posq,
+                                                   const int* __restrict__ cAr, const int* __restrict__ ncA,
+                                                   const float* __restrict__ S_in, const float* __restrict__ fp,
+                                                   float4* __restrict__ pf, float4* __restrict__ fa, int s)
 {
-    extern __shared__ float sc[];
-    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= D.n) return;
+    constexpr int N4 = (NCH + 3) / 4;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
     float G[NCH][NEP_NUM_S];
+    {
+        const float* fpa = fp + (size_t)D.NR * n + s;          // angular blocks: fpa[(blk * NA + nn) * n]
+        const size_t blk = (size_t)D.NA * n;
 #pragma unroll
-    for (int a = 0; a < NCH; ++a) {
-        const int nn = min(n0 + a, D.NA - 1);
-        float Sv[NEP_NUM_S], f3[4];
+        for (int a = 0; a < NCH; ++a) {
+            const int nn = min(n0 + a, D.NA - 1);
+            float Sv[NEP_NUM_S], f3[4];
+            const float* Sp = S_in + (size_t)(nn * NEP_NUM_S) * n + s;
 #pragma unroll
-        for (int k = 0; k < NEP_NUM_S; ++k) Sv[k] = S_in[(size_t)(nn * NEP_NUM_S + k) * n + s];
+            for (int k = 0; k < NEP_NUM_S; ++k) { Sv[k] = *Sp; Sp += n; }
+            const float* fq = fpa + (size_t)nn * n;
 #pragma unroll
-        for (int l = 0; l < 4; ++l) f3[l] = fp[(size_t)(D.NR + l * D.NA + nn) * n + s];
-        const float f4 = D.has4 ? fp[(size_t)(D.NR + 4 * D.NA + nn) * n + s] : 0.0f;
-        const float f5 = D.has5 ? fp[(size_t)(D.NR + (4 + D.has4) * D.NA + nn) * n + s] : 0.0f;
-        G_from_S(Sv, f3, f4, f5, C, G[a]);
-        if (n0 + a >= D.NA) {                              // padded channel of the global-table fallback
+            for (int l = 0; l < 4; ++l) { f3[l] = *fq; fq += blk; }
+            float f4 = 0.0f, f5 = 0.0f;
+            if (D.has4) { f4 = *fq; fq += blk; }
+            if (D.has5) f5 = *fq;
+            G_from_S(Sv, f3, f4, f5, C, G[a]);
+            if (n0 + a >= D.NA) {                              // padded channel of the global-table fallback
 #pragma unroll
-            for (int k = 0; k < NEP_NUM_S; ++k) G[a][k] = 0.0f;
+                for (int k = 0; k < NEP_NUM_S; ++k) G[a][k] = 0.0f;
+            }
         }
     }
-    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride + n0;
+    const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride;
     float sx = 0.0f, sy = 0.0f, sz = 0.0f;                 // sum_j dU_i/dr_ij
     PairWalk<NEP_SLOT_BITS> w(cAr, n, s, ncA[s], posq);
     while (w.next()) {
@@ -566,23 +612,28 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, co
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<true>(r, D.rcA_inv);
-        const float* c = tab_i + (size_t)w.pj.w * tab_stride;
-        float g[NCH], dg[NCH];
+        const float4* c4 = reinterpret_cast<const float4*>(tab_i + w.pj.w * tab_stride);
+        float g[4 * N4], dg[NCH];
+        load_row<NCH>(c4, g);                              // csum'
 #pragma unroll
-        for (int a = 0; a < NCH; ++a) { g[a] = 0.0f; dg[a] = 0.0f; }
+        for (int a = 0; a < NCH; ++a) dg[a] = 0.0f;
         {
             float Tkm1 = 1.0f, Tk = h.x, Dkm1 = 0.0f, Dk = 1.0f;      // T_0,T_1 ; T_0',T_1'
-            for (int k = 1; k < D.KA; ++k) {
+            for (int r0 = 1; r0 < D.KAR; r0 += 4) {
 #pragma unroll
-                for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
-                const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
-                const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-                Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
-                c += D.NAP;
+                for (int u = 0; u < 4; ++u) {
+                    float c[4 * N4];
+                    load_row<NCH>(c4 + (r0 + u) * N4, c);
+#pragma unroll
+                    for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
+                    const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
+                    const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+                    Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
+                }
             }
 #pragma unroll
             for (int a = 0; a < NCH; ++a) {
-                const float G0 = g[a] + c[a];
+                const float G0 = g[a];
                 g[a] = G0 * h.hfc;
                 dg[a] = fmaf(G0, h.hdfc, dg[a] * h.hfc_dx);
             }
@@ -635,6 +686,22 @@ k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, co
     }
     if (accumulate) { const float4 o = fa[s]; sx += o.x; sy += o.y; sz += o.z; }
     fa[s] = make_float4(sx, sy, sz, 0.0f);
+}
+
+template <int NCH, bool SM>
+__global__ void __launch_bounds__(128)
+k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
+                const int* __restrict__ cAr, const int* __restrict__ ncA, const float* __restrict__ cA_t,
+                const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf,
+                float4* __restrict__ fa, int* __restrict__ tile_ctr)
+{
+    extern __shared__ __align__(16) float sc[];
+    const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
+    const int ntile = (D.n + 31) >> 5;
+    for (int tile = next_tile(tile_ctr); tile < ntile; tile = next_tile(tile_ctr)) {
+        const int s = tile * 32 + (threadIdx.x & 31);
+        if (s < D.n) force_angular_atom<NCH>(D, C, n0, accumulate, tab_stride, tab, posq, cAr, ncA, S_in, fp, pf, fa, s);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
