@@ -67,9 +67,15 @@ def kernel_costs(h: W.Hyper, n_atoms: int, pairs_r: int, pairs_a: int, list_r: i
     # a7: g, g' (4 NA KA), A_k, B_k (4 x 24 NA), assembly of b_k / grad P_k (~500); per atom G_nk
     out["force_angular"] = (pairs_a * (4 * NA * KA + 4 * 24 * NA + 500) + n * 3 * 24 * NA,
                             n * (16 + 4 * 24 * NA + 4 * 6 * NA) + pairs_a * (4 + 12))
-    # a6+a8: radial partial forces both directions, sums; angular gather of own + reverse partial force
-    out["final"] = (pairs_r * (55 + 8 * KR + 4 * NR * KR) + pairs_a * 30,
-                    n * (16 + 4 + 8 * 13) + 4 * pairs_r + pairs_a * (4 + 1 + 2 * 12) + pairs_r * 4 * NR)
+    # a6: radial partial forces.  SURVEY.md 8(d) counts 55 + 8 KR + 4 NR KR per ordered pair for BOTH
+    # directions evaluated at atom i (Alg. 2); every direction is needed once only, so the method's
+    # minimum is one direction per ordered pair: 55 + 4 KR + 2 NR KR.  Bytes: position, own Fp_R, list
+    # entry, one 4-byte scalar delivered per pair, own sum.
+    out["force_radial"] = (pairs_r * (55 + 4 * KR + 2 * NR * KR),
+                           n * (16 + 4 * NR + 16 + 8) + pairs_r * (4 + 4))
+    # a8: gather of the delivered partial forces into F_i, W_i (~30 flops per pair)
+    out["final"] = (pairs_r * 30,
+                    n * (16 + 16 + 4 + 8 * 13) + 4 * pairs_r + pairs_a * 16 + (pairs_r - pairs_a) * 4)
     # per-step filter of the skin lists to the in-cutoff lists (~12 flops per listed pair)
     out["filter"] = (list_r * 12, n * 32 + 4 * list_r + 4 * pairs_r)
     out["quantize"] = (n * 9, n * (24 + 4 + 4 + 16))

@@ -88,6 +88,21 @@ int dev_alloc(nep_t* nep, T** p, size_t count)
 }
 #define NEP_TRY(x) do { int rc_ = (x); if (rc_ != NEP_OK) return rc_; } while (0)
 
+// Shared memory is carved out of the 228 KB that also hold the L1 cache, and the driver sizes the
+// carve-out for as many resident blocks as registers allow -- which can leave no L1 for the neighbour
+// gathers.  cap_smem limits it to the blocks that fit in `budget` bytes (at least one).
+template <typename K>
+int cap_smem(nep_t* nep, K kernel, size_t bytes_per_block, size_t budget)
+{
+    const size_t per = bytes_per_block + 1024;            // + the driver's 1 KB per block
+    size_t nb = budget / per;
+    if (nb < 1) nb = 1;
+    int pct = (int)((nb * per * 100 + 228 * 1024 - 1) / (228 * 1024));
+    if (pct > 100) pct = 100;
+    NEP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
+    return NEP_OK;
+}
+
 template <typename K>
 int allow_smem(nep_t* nep, K kernel, size_t bytes)
 {
@@ -102,9 +117,11 @@ int alloc_lists(nep_t* nep, int capA, int capS)
     NEP_TRY(dev_alloc(nep, &nep->listA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->rev, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->cA, (size_t)capA * n));
-    NEP_TRY(dev_alloc(nep, &nep->cAr, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->pf, (size_t)capA * n));
+    NEP_TRY(dev_alloc(nep, &nep->mA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->listS, (size_t)capS * n));
+    NEP_TRY(dev_alloc(nep, &nep->revS, (size_t)capS * n));
+    NEP_TRY(dev_alloc(nep, &nep->mB, (size_t)(capA + capS) * n));
     NEP_TRY(dev_alloc(nep, &nep->cB, (size_t)(capA + capS) * n));
     nep->capA = capA;
     nep->capS = capS;
@@ -127,18 +144,17 @@ int alloc_atoms(nep_t* nep, int64_t n)
     NEP_TRY(dev_alloc(nep, &nep->cntS, N));
     NEP_TRY(dev_alloc(nep, &nep->ncA, N));
     NEP_TRY(dev_alloc(nep, &nep->ncB, N));
-    NEP_TRY(dev_alloc(nep, &nep->maskA, N * ((1 << NEP_SLOT_BITS) / 64)));
     NEP_TRY(dev_alloc(nep, &nep->fa, N));
     NEP_TRY(dev_alloc(nep, &nep->q, N * d.D));
     NEP_TRY(dev_alloc(nep, &nep->fp, N * d.D));
     NEP_TRY(dev_alloc(nep, &nep->S, N * d.NA * NEP_NUM_S));
-    NEP_TRY(dev_alloc(nep, &nep->Et, N * d.T * d.KRP));
     NEP_TRY(dev_alloc(nep, &nep->U, N));
     NEP_TRY(dev_alloc(nep, &nep->e_out, N));
     NEP_TRY(dev_alloc(nep, &nep->f_out, 3 * N));
     NEP_TRY(dev_alloc(nep, &nep->w_out, 9 * N));
     nep->atom_cap = n;
     nep->capA = nep->capS = 0;      // list storage is tied to n: force a re-allocation
+    nep->mask_cap = 0;
     return NEP_OK;
 }
 
@@ -195,16 +211,28 @@ int build_lists(nep_t* nep, const double* pos_dev)
         NEP_CUDA(cudaStreamSynchronize(st));
         nep->maxA_skin = fl[2];
         nep->maxR_skin = fl[3];
-        if (!fl[0] && !fl[1]) break;
+        nep->maxS_skin = fl[4];
         if (fl[2] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours inside rc_angular + skin");
+        if (fl[4] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours between rc_angular + skin and rc_radial + skin");
+        if (!fl[0] && !fl[1]) break;
         if (attempt == 3) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "neighbour lists kept overflowing");
         int capA = nep->capA, capS = nep->capS;
         if (fl[0]) capA = fl[2] + 8 > 256 ? 256 : fl[2] + 8;
-        if (fl[1]) capS = fl[4] + 8;
+        if (fl[1]) capS = fl[4] + 8 > 256 ? 256 : fl[4] + 8;
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
-    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA, nep->listA, nep->cntA, nep->rev));
-    nep->d.maskW = nep->maxA_skin > 0 ? (nep->maxA_skin + 63) / 64 : 1;
+    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->listA, nep->cntA, nep->rev));
+    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->listS, nep->cntS, nep->revS));
+    {
+        const int longest = nep->maxA_skin > nep->maxS_skin ? nep->maxA_skin : nep->maxS_skin;
+        nep->d.maskW = longest > 0 ? (longest + 63) / 64 : 1;
+        nep->d.mrec = 4 * nep->d.maskW;
+        if ((int64_t)n * nep->d.mrec > nep->mask_cap) {
+            nep->mask_cap = 0;
+            NEP_TRY(dev_alloc(nep, &nep->mask, (size_t)n * nep->d.mrec));
+            nep->mask_cap = (int64_t)n * nep->d.mrec;
+        }
+    }
     nep->steps_since_build = 0;
     nep->have_lists = true;
     return NEP_OK;
@@ -213,11 +241,61 @@ int build_lists(nep_t* nep, const double* pos_dev)
 // ---- one evaluation of (a2)-(a8) into the internal output buffers ---------------------------------------
 const size_t kSmemTableMax = 96 * 1024;     // larger coefficient tables are read from global memory (L1)
 
-template <int KP>
-int launch_radial1(nep_t* nep)
+// register variants (few species): TT * KP <= 64 and a coefficient table small enough to stage
+const size_t kRegTableMax = 16 * 1024;
+
+template <int TT, int KP>
+int launch_radial_reg(nep_t* nep)
 {
     const NepDims& d = nep->d;
-    NEP_LAUNCH(NEP_K_RADIAL, k_radial1<KP><<<div_up(d.n, 128), 128, 0, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->cR_q, nep->q));
+    const size_t sm = sizeof(float) * (size_t)TT * TT * nep->strideR;
+    NEP_LAUNCH(NEP_K_RADIAL, (k_radial_reg<TT, KP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB,
+                                                                              nep->cR_t, nep->q)));
+    return NEP_OK;
+}
+
+template <int TT, int KP>
+int launch_force_radial_reg(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * (size_t)TT * TT * d.NR * KP;
+    NEP_LAUNCH(NEP_K_FORCE_RADIAL, (k_force_radial_reg<TT, KP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask,
+                                                                                          nep->fp, nep->cR_e, nep->mA, nep->mB, nep->fa)));
+    return NEP_OK;
+}
+
+// returns kNoVariant when (T, KP) has no register variant
+const int kNoVariant = 1;
+template <bool FORCE>
+int dispatch_radial_reg(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    if (d.T * nep->KP > 64 || d.T > 5) return kNoVariant;
+    if (sizeof(float) * (size_t)d.T * d.T * nep->strideR > kRegTableMax) return kNoVariant;
+    if (sizeof(float) * (size_t)d.T * d.T * d.NR * nep->KP > kRegTableMax) return kNoVariant;
+#define NEP_REG_CASE(TT, KPV)                                                                      \
+    if (d.T == TT && nep->KP == KPV) return FORCE ? launch_force_radial_reg<TT, KPV>(nep) : launch_radial_reg<TT, KPV>(nep);
+    NEP_REG_CASE(1, 4) NEP_REG_CASE(1, 8) NEP_REG_CASE(1, 12) NEP_REG_CASE(1, 16) NEP_REG_CASE(1, 20) NEP_REG_CASE(1, 24) NEP_REG_CASE(1, 28) NEP_REG_CASE(1, 32)
+    NEP_REG_CASE(2, 4) NEP_REG_CASE(2, 8) NEP_REG_CASE(2, 12) NEP_REG_CASE(2, 16) NEP_REG_CASE(2, 20) NEP_REG_CASE(2, 24) NEP_REG_CASE(2, 28) NEP_REG_CASE(2, 32)
+    NEP_REG_CASE(3, 4) NEP_REG_CASE(3, 8) NEP_REG_CASE(3, 12) NEP_REG_CASE(3, 16) NEP_REG_CASE(3, 20)
+    NEP_REG_CASE(4, 4) NEP_REG_CASE(4, 8) NEP_REG_CASE(4, 12) NEP_REG_CASE(4, 16)
+    NEP_REG_CASE(5, 4) NEP_REG_CASE(5, 8) NEP_REG_CASE(5, 12)
+#undef NEP_REG_CASE
+    return kNoVariant;
+}
+
+// block size of the kernels that keep per-thread tables in shared memory: 128 threads, or 32 when the
+// tables of 128 threads would not fit
+const size_t kSmemBlockMax = 200 * 1024;
+
+template <int KP, bool TAB_SM, int BS>
+int launch_radial_multi2(nep_t* nep, size_t sm)
+{
+    const NepDims& d = nep->d;
+    NEP_TRY(allow_smem(nep, k_radial_multi<KP, TAB_SM, BS>, sm));
+    NEP_TRY(cap_smem(nep, k_radial_multi<KP, TAB_SM, BS>, sm, nep->smem_budget));
+    NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, TAB_SM, BS><<<div_up(d.n, BS), BS, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
+                                                                                          nep->cB, nep->ncB, nep->cR_t, nep->q)));
     return NEP_OK;
 }
 
@@ -227,38 +305,16 @@ int launch_radial_multi(nep_t* nep)
     const NepDims& d = nep->d;
     const size_t tab_bytes = sizeof(float) * (size_t)d.T * d.T * nep->strideR;
     const bool tab_in_smem = tab_bytes <= kSmemTableMax;
-    int bs = 128;
-    auto smem = [&](int b) { return sizeof(float) * (size_t)d.T * KP * b + (tab_in_smem ? tab_bytes : 0); };
-    while (bs > 32 && smem(bs) > 160 * 1024) bs >>= 1;
-    const size_t sm = smem(bs);
-    if (tab_in_smem) {
-        NEP_TRY(allow_smem(nep, k_radial_multi<KP, true>, sm));
-        NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, true><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
-                                                                                        nep->cB, nep->ncB, nep->cR_t, nep->q)));
-    } else {
-        NEP_TRY(allow_smem(nep, k_radial_multi<KP, false>, sm));
-        NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, false><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
-                                                                                         nep->cB, nep->ncB, nep->cR_t, nep->q)));
-    }
-    return NEP_OK;
+    auto smem = [&](int b) { return sizeof(float) * (size_t)d.T * d.KR * b + (tab_in_smem ? tab_bytes : 0); };
+    if (smem(128) <= kSmemBlockMax / 2)
+        return tab_in_smem ? launch_radial_multi2<KP, true, 128>(nep, smem(128)) : launch_radial_multi2<KP, false, 128>(nep, smem(128));
+    if (smem(32) > kSmemBlockMax) return nep_fail(nep, NEP_ERR_INVALID_ARG, "n_types x basis_radial too large for shared memory");
+    return tab_in_smem ? launch_radial_multi2<KP, true, 32>(nep, smem(32)) : launch_radial_multi2<KP, false, 32>(nep, smem(32));
 }
 
 int dispatch_radial(nep_t* nep)
 {
-    const NepDims& d = nep->d;
-    if (d.T == 1) {
-        switch (nep->KP) {
-            case 4: return launch_radial1<4>(nep);
-            case 8: return launch_radial1<8>(nep);
-            case 12: return launch_radial1<12>(nep);
-            case 16: return launch_radial1<16>(nep);
-            case 20: return launch_radial1<20>(nep);
-            case 24: return launch_radial1<24>(nep);
-            case 28: return launch_radial1<28>(nep);
-            case 32: return launch_radial1<32>(nep);
-        }
-        return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
-    }
+    if (!nep->force_smem_radial) { const int rc = dispatch_radial_reg<false>(nep); if (rc != kNoVariant) return rc; }
     switch (nep->KP) {
         case 4: return launch_radial_multi<4>(nep);
         case 8: return launch_radial_multi<8>(nep);
@@ -299,7 +355,7 @@ int launch_angular(nep_t* nep, const NepCoef& C, int p, bool force_pass)
     } else {
         NEP_TRY(allow_smem(nep, k_force_angular<NCH, SM>, sm));
         NEP_TRY(persistent_grid(nep, k_force_angular<NCH, SM>, sm, &grid));
-        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, p > 0, stride, nep->posq, nep->cAr, nep->ncA, tab,
+        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, p > 0, stride, nep->posq, nep->cA, nep->ncA, nep->mask, tab,
                                                                                                  nep->S, nep->fp, nep->pf, nep->fa, nep->tile_ctr + 16 + p)));
     }
     return NEP_OK;
@@ -328,12 +384,11 @@ int launch_ann(nep_t* nep)
 {
     const NepDims& d = nep->d;
     int bs = 128;                                        // smaller blocks for networks whose weights fill shared memory
-    auto smem = [&](int b) { return sizeof(float) * ((size_t)d.H * DP + 2 * d.H + (size_t)(16 + d.H) * b); };
+    auto smem = [&](int b) { return sizeof(float) * ((size_t)d.H * DP + 2 * d.H + (size_t)d.H * b); };
     while (bs > 32 && smem(bs) > 110 * 1024) bs >>= 1;
     const size_t sm = smem(bs);
     NEP_TRY(allow_smem(nep, k_ann<DP>, sm));
-    NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->posq, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1,
-                                                        nep->cR_e, nep->fp, nep->U, nep->Et));
+    NEP_LAUNCH(NEP_K_ANN, k_ann<DP><<<div_up(d.n, bs), bs, sm, nep->stream>>>(d, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1, nep->fp, nep->U));
     return NEP_OK;
 }
 
@@ -358,28 +413,52 @@ int dispatch_ann(nep_t* nep)
     return nep_fail(nep, NEP_ERR_INVALID_ARG, "descriptor too long");
 }
 
-template <int NK4>
-int launch_final(nep_t* nep)
+template <int KP, bool TAB_SM, int BS>
+int launch_force_radial2(nep_t* nep, size_t sm)
 {
     const NepDims& d = nep->d;
-    NEP_LAUNCH(NEP_K_FINAL, k_final<NK4><<<div_up(d.n, 128), 128, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->Et,
-                                                            nep->pf, nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out));
+    NEP_TRY(allow_smem(nep, k_force_radial<KP, TAB_SM, BS>, sm));
+    NEP_TRY(cap_smem(nep, k_force_radial<KP, TAB_SM, BS>, sm, nep->smem_budget));
+    NEP_LAUNCH(NEP_K_FORCE_RADIAL, (k_force_radial<KP, TAB_SM, BS><<<div_up(d.n, BS), BS, sm, nep->stream>>>(d, nep->posq, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask,
+                                                                                                nep->fp, nep->cR_e, nep->mA, nep->mB, nep->fa)));
     return NEP_OK;
+}
+
+template <int KP>
+int launch_force_radial(nep_t* nep)
+{
+    const NepDims& d = nep->d;
+    const size_t tab_bytes = sizeof(float) * (size_t)d.T * d.T * d.NR * KP;
+    const bool tab_in_smem = tab_bytes <= kSmemTableMax;
+    auto smem = [&](int b) { return sizeof(float) * (size_t)round_up4(d.T * d.KR) * b + (tab_in_smem ? tab_bytes : 0); };
+    if (smem(128) <= kSmemBlockMax / 2)
+        return tab_in_smem ? launch_force_radial2<KP, true, 128>(nep, smem(128)) : launch_force_radial2<KP, false, 128>(nep, smem(128));
+    if (smem(32) > kSmemBlockMax) return nep_fail(nep, NEP_ERR_INVALID_ARG, "n_types x basis_radial too large for shared memory");
+    return tab_in_smem ? launch_force_radial2<KP, true, 32>(nep, smem(32)) : launch_force_radial2<KP, false, 32>(nep, smem(32));
+}
+
+int dispatch_force_radial(nep_t* nep)
+{
+    if (!nep->force_smem_radial) { const int rc = dispatch_radial_reg<true>(nep); if (rc != kNoVariant) return rc; }
+    switch (nep->KP) {
+        case 4: return launch_force_radial<4>(nep);
+        case 8: return launch_force_radial<8>(nep);
+        case 12: return launch_force_radial<12>(nep);
+        case 16: return launch_force_radial<16>(nep);
+        case 20: return launch_force_radial<20>(nep);
+        case 24: return launch_force_radial<24>(nep);
+        case 28: return launch_force_radial<28>(nep);
+        case 32: return launch_force_radial<32>(nep);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
 }
 
 int dispatch_final(nep_t* nep)
 {
-    switch (nep->d.KRP >> 2) {
-        case 1: return launch_final<1>(nep);
-        case 2: return launch_final<2>(nep);
-        case 3: return launch_final<3>(nep);
-        case 4: return launch_final<4>(nep);
-        case 5: return launch_final<5>(nep);
-        case 6: return launch_final<6>(nep);
-        case 7: return launch_final<7>(nep);
-        case 8: return launch_final<8>(nep);
-    }
-    return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
+    const NepDims& d = nep->d;
+    NEP_LAUNCH(NEP_K_FINAL, k_final<<<div_up(d.n, 256), 256, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->pf, nep->mA, nep->mB,
+                                                       nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out));
+    return NEP_OK;
 }
 
 int evaluate(nep_t* nep, const double* pos_dev)
@@ -392,13 +471,13 @@ int evaluate(nep_t* nep, const double* pos_dev)
                                                1.0 / nep->box[2], nep->posq));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
     NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
-    NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->listS, nep->cntS,
-                                             nep->cA, nep->ncA, nep->cB, nep->ncB, nep->maskA, nep->disp_max));
-    NEP_LAUNCH(NEP_K_CREV, k_crev<<<div_up(n, 256), 256, 0, st>>>(d, nep->cA, nep->ncA, nep->rev, nep->maskA, nep->cAr));
+    NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
+                                             nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
     NEP_TRY(dispatch_radial(nep));
     NEP_TRY(dispatch_angular(nep, C, false));
     NEP_TRY(dispatch_ann(nep));
     NEP_TRY(dispatch_angular(nep, C, true));
+    NEP_TRY(dispatch_force_radial(nep));
     NEP_TRY(dispatch_final(nep));
     nep->have_eval = true;
     return NEP_OK;
@@ -507,6 +586,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     d.rcR = (float)h->rc_radial; d.rcA = (float)h->rc_angular;
     d.rcR_inv = (float)(1.0 / h->rc_radial); d.rcA_inv = (float)(1.0 / h->rc_angular);
     d.rcR2 = d.rcR * d.rcR; d.rcA2 = d.rcA * d.rcA;
+    if (const char* e = getenv("NEP_DBG")) d.dbg = atoi(e);
     nep->DP = ann_tier(d.D);
     if (nep->DP < 0) { delete nep; return NEP_ERR_INVALID_ARG; }
     for (int t = 0; t < d.T; ++t) {
@@ -519,6 +599,9 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     nep->KP = round_up4(d.KR);
     nep->strideR = (d.KR * d.NRP) | 1;
     nep->nch_max = 5;
+    nep->smem_budget = 180 * 1024;
+    nep->force_smem_radial = getenv("NEP_RADIAL_SMEM") != nullptr;    // tests: exercise the shared-memory variants
+    if (const char* e = getenv("NEP_SMEM_KB")) { const int v = atoi(e); if (v >= 8 && v <= 227) nep->smem_budget = (size_t)v * 1024; }
     if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) nep->nch_max = v; }
     {   // angular passes: at most nch_max channels each, tables staged in shared memory; if a table would
         // not fit there, passes of 4 channels read it from global memory (zero-padded surplus channels)
@@ -543,7 +626,6 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     }
     std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f);
     std::vector<float> cAt((size_t)nep->pass_off[nep->n_pass - 1] + (size_t)TT * nep->pass_stride[nep->n_pass - 1], 0.0f);
-    std::vector<float> cRq((size_t)d.NR * nep->KP, 0.0f);
     std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
     for (int tt = 0; tt < TT; ++tt) {
         for (int nn = 0; nn < d.NR; ++nn)
@@ -551,7 +633,6 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
                 const float v = c_radial[((size_t)tt * d.NR + nn) * d.KR + k];
                 cRt[(size_t)tt * nep->strideR + (size_t)k * d.NRP + nn] = v;
                 cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
-                if (TT == 1) cRq[(size_t)nn * nep->KP + k] = v;
             }
         for (int p = 0; p < nep->n_pass; ++p) {
             const int NCHP = round_up4(nep->pass_nch[p]);
@@ -579,7 +660,6 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
         if (rc != NEP_OK) { nep_destroy(nep); return rc; }                                        \
     } while (0)
     UPLOAD(cR_t, cRt);
-    UPLOAD(cR_q, cRq);
     UPLOAD(cA_t, cAt);
     UPLOAD(cR_e, cRe);
     UPLOAD(w0p, w0p);
@@ -805,8 +885,8 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 
 // ---- measurement support ----------------------------------------------------------------------------------
 static const char* const kKernelNames[NEP_K_COUNT] = {
-    "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "crev", "radial",
-    "angular", "ann", "force_angular", "final", "kick_drift", "kick", "export"};
+    "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
+    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "export"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
 

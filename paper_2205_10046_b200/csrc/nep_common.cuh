@@ -18,7 +18,7 @@
 // Kernel ids for the optional per-kernel CUDA-event timing (nep_profile_*; bench.py's roofline leg).
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
-    NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_CREV, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FINAL,
+    NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FORCE_RADIAL, NEP_K_FINAL,
     NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_EXPORT, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
@@ -35,7 +35,9 @@ struct NepDims {
     float rcR, rcA, rcR_inv, rcA_inv, rcR2, rcA2;
     float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
     int capA, capS;              // storage rows of the skin lists (angular-range part, outer shell)
-    int maskW;                   // 64-bit words per atom of the in-cutoff mask over the angular skin slots
+    int maskW;                   // 64-bit words of one in-cutoff mask (covers the longest skin list)
+    int dbg;                     // NEP_DBG experiments (0 in production)
+    int mrec;                    // 64-bit words of an atom's mask record (4 maskW, see k_filter)
 };
 
 struct nep_ctx {
@@ -56,17 +58,18 @@ struct nep_ctx {
 
     // model (device)
     float* cR_t;     // [T*T] x strideR: rows [k][NRP]   c_radial with the n-values of one k contiguous
-    float* cR_q;     // [NR][KP]  (T == 1 only) zero-padded rows for k_radial1
     float* cA_t;     // per angular pass: [T*T] x pass_stride: KAR rows of round_up4(nch) floats (see k_angular)
     int n_pass;              // angular passes (channels n0 .. n0+nch-1 each)
     int pass_n0[16], pass_nch[16], pass_off[16], pass_stride[16];   // offsets / strides in floats
     bool angular_tab_smem;   // tables staged in shared memory (else read from global memory)
     int* tile_ctr;           // [64] device: dynamic tile counters of the angular kernels (zeroed per evaluation)
     int num_sms;
-    float* cR_e;     // [T(ti)][T(tj)][NR][KRP]  for the per-atom E table
+    float* cR_e;     // [T(ti)][T(tj)][NR][KRP]  for the per-atom E table of k_force_radial
     int strideR;            // odd type-pair stride (floats) of cR_t: bank-conflict-free lookups
     int KP;                 // KR rounded up to a multiple of 4
     int nch_max;            // angular n-values per pass (<= NEP_NCH_MAX)
+    size_t smem_budget;     // shared memory per SM that the table-in-smem kernels may carve out of L1
+    bool force_smem_radial; // NEP_RADIAL_SMEM set: use the shared-memory radial kernels even where a register variant exists
     float* w0p;      // [H][DP] rows padded with zeros to DP
     float* b0;       // [H]
     float* w1;       // [H]
@@ -87,7 +90,7 @@ struct nep_ctx {
     bool force_current;      // ... and it belongs to the positions md_step will continue from
     const double* force_pos_tag;
     int steps_since_build;
-    int maxA_skin, maxR_skin;   // list sizes of the last build (angular-range part; radial = A + shell)
+    int maxA_skin, maxR_skin, maxS_skin;   // list sizes of the last build (angular-range part; radial = A + shell; shell)
 
     // per-atom (device); "sorted" = internal spatial order, "orig" = caller's order
     int* type_orig;          // [n]
@@ -106,10 +109,11 @@ struct nep_ctx {
     int* listA;  int* cntA;  // [capA][n] sorted indices with |r| < rcA + skin
     int* listS;  int* cntS;  // [capS][n] rcA + skin <= |r| < rcR + skin
     unsigned char* rev;      // [capA][n] slot of i in j's listA
-    int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|skin slot with |r| < rcA
-    int* cAr;                // [capA][n] per step: packed (j<<8)|slot of i in j's cA column (k_angular)
-    unsigned long long* maskA;  // [n][maskW] per step: bit m set <=> skin slot m of listA is inside rcA
-    int* cB; int* ncB;       // [capA+capS][n] per step: j with rcA <= |r| < rcR
+    unsigned char* revS;     // [capS][n] slot of i in j's listS
+    int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|(slot of i in j's skin list) with |r| < rcA
+    unsigned long long* mask;   // [n][mrec] per step: in-cutoff masks over the skin slots (see k_filter)
+    int64_t mask_cap;           // allocated 64-bit words
+    int* cB; int* ncB;       // [capA+capS][n] per step: packed like cA, rcA <= |r| < rcR (listA part, then listS part)
     int* flags;              // [4] device: 0 overflow A, 1 overflow S, 2 max cntA, 3 max (cntA+cntS)
     unsigned* disp_max;      // [1] device: float bits of max displacement^2 since build
     int64_t atom_cap;        // allocated atoms
@@ -117,10 +121,11 @@ struct nep_ctx {
     float* q;                // [D][n]
     float* fp;               // [D][n]
     float* S;                // [NA*24][n]
-    float* Et;               // [n][T][KRP]  E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
     float* U;                // [n]
-    float4* pf;              // [capA][n] received angular partial forces: pf[m][i] = dU_j/dr_ji, j = cA[m][i]
-    float4* fa;              // [n] sum_j dU_i/dr_ij over the angular pairs of i
+    float4* pf;              // [capA][n] received from j = cA[m][i]: angular dU_j/dr_ji
+    float* mA;               // [capA][n] received from j = cA[m][i]: radial scalar m_ji
+    float* mB;               // [capA+capS][n] received from j = cB[m][i]: radial scalar m_ji
+    float4* fa;              // [n] sum_j dU_i/dr_ij (angular part from k_force_angular, radial added by k_force_radial)
     double* e_out;           // [n]    orig order
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]
@@ -205,6 +210,7 @@ static inline int nep_fail(nep_t* nep, int status, const char* msg)
 
 static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 static inline int round_up4(int a) { return (a + 3) & ~3; }
+__device__ __forceinline__ int round_up4_dev(int a) { return (a + 3) & ~3; }
 
 // ---------------------------------------------------------------------------------------------------
 // Pair geometry from quantised coordinates.  Positions are stored as 32-bit fractions of the box edge,

@@ -23,43 +23,99 @@ struct NepCoef {
 };
 
 // ---------------------------------------------------------------------------------------------------
-// Software-pipelined walk over one atom's neighbour entries  e_m = list[m*n + s], m = 0..cnt-1.
-// DECODE(e) gives the neighbour's sorted index.  Usage:
-//   PairWalk w(list, n, s, cnt, posq);  while (w.next()) { use w.e (entry), w.pj (neighbour posq) }
-template <int SHIFT>
+// Software-pipelined walk over one atom's compact entries  e_m = list[m*n + s] = (j << 8) | rs,
+// m = 0..cnt-1: the entry two pairs ahead and the neighbour's position one pair ahead are in flight while
+// the current pair is computed.  Usage:
+//   PairWalk<MODE> w(...);  while (w.next(D)) { w.j() neighbour, w.pj its posq, w.slot(D) delivery slot }
+// MODE 0: positions only.  MODE 1 (cA): also prefetches the neighbour's mask words of the 64-slot group
+// of rs, from which slot() = compact slot of this atom in the neighbour's cA column.  MODE 2 (cB): entries
+// m < nsplit came from listA, the others from listS (offset by the neighbour's count of outer-shell
+// listA entries).  Mask record of an atom (k_filter): 2 W 16-byte pairs, {A_w, O_w} for w < W, then
+// {S_w, count}.
+// DEPTH = how many pairs ahead the neighbour's position (and mask pair) is requested; the entries run one
+// further ahead.
+template <int MODE, int DEPTH = 1>
 struct PairWalk {
-    const int* __restrict__ list;
+    const int* __restrict__ lp;          // &list[(m + DEPTH + 1) * n + s]
     const int4* __restrict__ posq;
+    const ulonglong2* __restrict__ mask;
     size_t n;
-    int s, cnt, m;
-    int e, e1, e2;       // current entry, next, next-next
-    int4 pj, p1;         // current / next neighbour position
+    int cnt, m, nsplit;
+    int e;               // current entry
+    int4 pj;             // current neighbour position
+    ulonglong2 mw;       // current neighbour mask pair
+    int eq[DEPTH + 1];   // entries m+1 .. m+DEPTH+1
+    int4 pq[DEPTH];      // positions of m+1 .. m+DEPTH
+    ulonglong2 mq[DEPTH];
     __device__ __forceinline__ PairWalk(const int* __restrict__ list_, size_t n_, int s_, int cnt_,
-                                        const int4* __restrict__ posq_)
-        : list(list_), posq(posq_), n(n_), s(s_), cnt(cnt_), m(-1)
+                                        const int4* __restrict__ posq_, const NepDims& D,
+                                        const unsigned long long* __restrict__ mask_ = nullptr, int nsplit_ = 0)
+        : lp(list_ + s_), posq(posq_), mask(reinterpret_cast<const ulonglong2*>(mask_)), n(n_), cnt(cnt_), m(-1), nsplit(nsplit_)
     {
-        e1 = (cnt > 0) ? list[s] : 0;
-        e2 = (cnt > 1) ? list[n + s] : 0;
-        p1 = (cnt > 0) ? posq[e1 >> SHIFT] : make_int4(0, 0, 0, 0);
+#pragma unroll
+        for (int d = 0; d <= DEPTH; ++d) { eq[d] = (d < cnt) ? *lp : 0; lp += n; }
+#pragma unroll
+        for (int d = 0; d < DEPTH; ++d) {
+            pq[d] = make_int4(0, 0, 0, 0);
+            mq[d] = make_ulonglong2(0ull, 0ull);
+            if (d < cnt) fetch(eq[d], d, pq[d], mq[d], D);
+        }
     }
-    __device__ __forceinline__ bool next()
+    __device__ __forceinline__ void fetch(int ee, int mm, int4& p, ulonglong2& w, const NepDims& D)   // entry ee at position mm
+    {
+        const int j1 = ee >> NEP_SLOT_BITS;
+        p = posq[j1];
+        if (MODE >= 1) {
+            const int word = (ee & ((1 << NEP_SLOT_BITS) - 1)) >> 6;
+            w = mask[(size_t)j1 * (2 * D.maskW) + ((MODE == 2 && mm >= nsplit) ? D.maskW + word : word)];
+        }
+    }
+    __device__ __forceinline__ bool next(const NepDims& D)
     {
         if (++m >= cnt) return false;
-        e = e1; pj = p1;
-        e1 = e2;
-        if (m + 1 < cnt) p1 = posq[e1 >> SHIFT];
-        if (m + 2 < cnt) e2 = list[(size_t)(m + 2) * n + s];
+        e = eq[0]; pj = pq[0]; mw = mq[0];
+#pragma unroll
+        for (int d = 0; d < DEPTH; ++d) eq[d] = eq[d + 1];
+#pragma unroll
+        for (int d = 0; d + 1 < DEPTH; ++d) { pq[d] = pq[d + 1]; mq[d] = mq[d + 1]; }
+        if (m + DEPTH < cnt) fetch(eq[DEPTH - 1], m + DEPTH, pq[DEPTH - 1], mq[DEPTH - 1], D);
+        if (m + DEPTH + 1 < cnt) eq[DEPTH] = *lp;
+        lp += n;
         return true;
+    }
+    __device__ __forceinline__ int j() const { return e >> NEP_SLOT_BITS; }
+    // compact slot of this atom in the neighbour's column of the same list
+    __device__ __forceinline__ int slot(const NepDims& D) const
+    {
+        const int rs = e & ((1 << NEP_SLOT_BITS) - 1);
+        const bool fromS = (MODE == 2 && m >= nsplit);
+        const unsigned long long word = (MODE == 1 || fromS) ? mw.x : mw.y;
+        int cs = __popcll(word & ((1ull << (rs & 63)) - 1ull));
+        if (rs >> 6) {                                       // rare: more than 64 skin slots
+            const ulonglong2* rec = mask + (size_t)j() * (2 * D.maskW) + (fromS ? D.maskW : 0);
+            for (int w = 0; w < (rs >> 6); ++w) cs += __popcll((MODE == 1 || fromS) ? rec[w].x : rec[w].y);
+        }
+        if (fromS) cs += (int)mw.y;
+        return cs;
     }
 };
 
 // ---------------------------------------------------------------------------------------------------
+// Per-step compaction of the skin lists to this step's in-cutoff lists (removes the in-cutoff divergence
+// from every later kernel):
+//   cA[m][i] = (j << 8) | rs   pairs with r < rcA,            rs = slot of i in j's SKIN list (rev / revS)
+//   cB[m][i] = (j << 8) | rs   pairs with rcA <= r < rcR: first those of listA, then those of listS
+// and the mask record of atom i, 2 W 16-byte pairs (W = D.maskW words cover the longest skin list):
+//   pair w < W:   .x bit m: slot 64 w + m of listA is inside rcA;  .y: that slot is in the outer shell
+//   pair W + w:   .x bit m: slot 64 w + m of listS is inside rcR;  .y: number of outer-shell bits of listA
+// The slot of i in j's COMPACT column -- where i delivers dU_i/dr_ij to j -- is the number of set bits
+// below rs in the matching mask of j (PairWalk::slot), so no per-step reverse list is built.
 __global__ void __launch_bounds__(256)
 k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq_build,
-         const int* __restrict__ listA, const int* __restrict__ cntA,
-         const int* __restrict__ listS, const int* __restrict__ cntS,
+         const int* __restrict__ listA, const int* __restrict__ cntA, const unsigned char* __restrict__ rev,
+         const int* __restrict__ listS, const int* __restrict__ cntS, const unsigned char* __restrict__ revS,
          int* __restrict__ cA, int* __restrict__ ncA, int* __restrict__ cB, int* __restrict__ ncB,
-         unsigned long long* __restrict__ maskA, unsigned* __restrict__ disp_max)
+         unsigned long long* __restrict__ mask, unsigned* __restrict__ disp_max)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
@@ -71,83 +127,65 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
         if (r2 > 0.0f) atomicMax(disp_max, __float_as_uint(r2));
     }
     int na = 0, nb = 0;
+    ulonglong2* rec = reinterpret_cast<ulonglong2*>(mask) + (size_t)s * (2 * D.maskW);
     const int ca = cntA[s];
-    // maskA[s]: bit m <=> skin slot m is inside rcA this step.  The compact slot of skin slot m is the
-    // number of set bits below m, which is how a neighbour finds the slot of i in i's cA column.
-    unsigned long long mword = 0ull;
-    unsigned long long* mrow = maskA + (size_t)s * D.maskW;
-    for (int m0 = 0; m0 < ca; m0 += 4) {                 // 4 independent gathers in flight
-        int j[4]; int4 pj[4];
+    for (int w = 0; w < D.maskW; ++w) {
+        unsigned long long wa = 0ull, wb = 0ull;
+        const int mend = min(ca, 64 * (w + 1));
+        for (int m0 = 64 * w; m0 < mend; m0 += 4) {          // 4 independent gathers in flight
+            int j[4], rs[4]; int4 pj[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) j[u] = (m0 + u < ca) ? listA[(size_t)(m0 + u) * n + s] : s;
+            for (int u = 0; u < 4; ++u) {
+                const bool ok = m0 + u < mend;
+                j[u] = ok ? listA[(size_t)(m0 + u) * n + s] : s;
+                rs[u] = ok ? rev[(size_t)(m0 + u) * n + s] : 0;
+            }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+            for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (m0 + u < ca) {
-                float dx, dy, dz, r2;
-                pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                if (r2 < D.rcA2) {
-                    cA[(size_t)na * n + s] = (j[u] << NEP_SLOT_BITS) | (m0 + u); ++na;
-                    mword |= 1ull << ((m0 + u) & 63);
+            for (int u = 0; u < 4; ++u) {
+                if (m0 + u < mend) {
+                    float dx, dy, dz, r2;
+                    pair_vec(pi, pj[u], D, dx, dy, dz, r2);
+                    const int e = (j[u] << NEP_SLOT_BITS) | rs[u];
+                    if (r2 < D.rcA2) { cA[(size_t)na * n + s] = e; ++na; wa |= 1ull << ((m0 + u) & 63); }
+                    else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = e; ++nb; wb |= 1ull << ((m0 + u) & 63); }
                 }
-                else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j[u]; ++nb; }
             }
         }
-        if (((m0 + 4) & 63) == 0) { mrow[m0 >> 6] = mword; mword = 0ull; }     // word complete
+        rec[w] = make_ulonglong2(wa, wb);
     }
-    if (((ca + 3) & ~3) & 63) mrow[ca >> 6] = mword;     // last word not completed inside the loop
+    const unsigned long long nouter = (unsigned long long)nb;
     const int cs = cntS[s];
-    for (int m0 = 0; m0 < cs; m0 += 4) {
-        int j[4]; int4 pj[4];
+    for (int w = 0; w < D.maskW; ++w) {
+        unsigned long long ws = 0ull;
+        const int mend = min(cs, 64 * (w + 1));
+        for (int m0 = 64 * w; m0 < mend; m0 += 4) {
+            int j[4], rs[4]; int4 pj[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) j[u] = (m0 + u < cs) ? listS[(size_t)(m0 + u) * n + s] : s;
+            for (int u = 0; u < 4; ++u) {
+                const bool ok = m0 + u < mend;
+                j[u] = ok ? listS[(size_t)(m0 + u) * n + s] : s;
+                rs[u] = ok ? revS[(size_t)(m0 + u) * n + s] : 0;
+            }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+            for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (m0 + u < cs) {
-                float dx, dy, dz, r2;
-                pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = j[u]; ++nb; }
+            for (int u = 0; u < 4; ++u) {
+                if (m0 + u < mend) {
+                    float dx, dy, dz, r2;
+                    pair_vec(pi, pj[u], D, dx, dy, dz, r2);
+                    if (r2 < D.rcR2) {
+                        cB[(size_t)nb * n + s] = (j[u] << NEP_SLOT_BITS) | rs[u]; ++nb;
+                        ws |= 1ull << ((m0 + u) & 63);
+                    }
+                }
             }
         }
+        rec[D.maskW + w] = make_ulonglong2(ws, nouter);
     }
     ncA[s] = na;
     ncB[s] = nb;
-}
-
-// ---------------------------------------------------------------------------------------------------
-// cAr[m][i] = (j << 8) | (slot of i in j's cA column), j = cA[m][i]: the address at which atom i
-// delivers dU_i/dr_ij to atom j (k_force_angular).  That slot is the number of in-cutoff skin slots of j
-// below the skin slot of i in j's listA (rev, built with the lists): a popcount of j's mask.
-__global__ void __launch_bounds__(256)
-k_crev(NepDims D, const int* __restrict__ cA, const int* __restrict__ ncA, const unsigned char* __restrict__ rev,
-       const unsigned long long* __restrict__ maskA, int* __restrict__ cAr)
-{
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= D.n) return;
-    const size_t n = (size_t)D.n;
-    const int na = ncA[s];
-    for (int m0 = 0; m0 < na; m0 += 4) {                 // 4 independent dependent-load chains in flight
-        int e[4], rs[4];
-        unsigned long long mw[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) e[u] = (m0 + u < na) ? cA[(size_t)(m0 + u) * n + s] : 0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) rs[u] = (m0 + u < na) ? rev[(size_t)(e[u] & ((1 << NEP_SLOT_BITS) - 1)) * n + s] : 0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) mw[u] = (m0 + u < na) ? maskA[(size_t)(e[u] >> NEP_SLOT_BITS) * D.maskW + (rs[u] >> 6)] : 0ull;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (m0 + u < na) {
-                const int j = e[u] >> NEP_SLOT_BITS;
-                int cs = __popcll(mw[u] & ((1ull << (rs[u] & 63)) - 1ull));
-                for (int ww = 0; ww < (rs[u] >> 6); ++ww) cs += __popcll(maskA[(size_t)j * D.maskW + ww]);
-                cAr[(size_t)(m0 + u) * n + s] = (j << NEP_SLOT_BITS) | cs;
-            }
-        }
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -159,7 +197,7 @@ k_crev(NepDims D, const int* __restrict__ cA, const int* __restrict__ ncA, const
 
 // one pair's contribution to A_0..A_{K-1} held in registers (K compile-time)
 template <int KP>
-__device__ __forceinline__ void radial_accumulate(float r2, float rc_inv, float* A)
+__device__ __forceinline__ void radial_accumulate(float r2, float rc_inv, float* A, int KR = KP)
 {
     const float r = r2 * rsqrtf(r2);
     const BasisHead h = basis_head<false>(r, rc_inv);
@@ -168,103 +206,148 @@ __device__ __forceinline__ void radial_accumulate(float r2, float rc_inv, float*
     if (KP > 1) A[1] = fmaf(Tk, h.hfc, A[1]);
 #pragma unroll
     for (int k = 2; k < KP; ++k) {
-        const float Tn = fmaf(h.two_x, Tk, -Tkm1);
-        Tkm1 = Tk; Tk = Tn;
-        A[k] = fmaf(Tk, h.hfc, A[k]);
+        if (k < KP - 3 || k < KR) {                       // uniform: KP - 3 <= KR <= KP
+            const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+            Tkm1 = Tk; Tk = Tn;
+            A[k] = fmaf(Tk, h.hfc, A[k]);
+        }
     }
 }
 
-// single-species systems: accumulators in registers.  KP = KR rounded up to a multiple of 4 (the
-// surplus accumulators are finite and multiply zero-padded coefficients).
-template <int KP>
-__global__ void __launch_bounds__(128)
-k_radial1(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, const int* __restrict__ ncA,
-          const int* __restrict__ cB, const int* __restrict__ ncB, const float* __restrict__ cR_q,
-          float* __restrict__ q)
+// Few species (TT * KP <= 64): the per-type accumulators A[t][k] stay in registers -- no shared memory, so
+// the whole L1 serves the neighbour gathers and occupancy is set by registers alone.  The neighbour's
+// type selects the row with a 0/1 factor (TT * KR FMAs per pair, no branches).  KP = KR rounded up to 4.
+template <int TT, int KP>
+__device__ __forceinline__ void radial_accumulate_typed(float r2, float rc_inv, int KR, int tj, float (&A)[TT][KP])
 {
+    const float r = r2 * rsqrtf(r2);
+    const BasisHead h = basis_head<false>(r, rc_inv);
+    float v[KP];
+    v[0] = h.hfc;
+    float Tkm1 = 1.0f, Tk = h.x;
+    if (KP > 1) v[1] = Tk * h.hfc;
+#pragma unroll
+    for (int k = 2; k < KP; ++k) {
+        const float Tn = fmaf(h.two_x, Tk, -Tkm1);
+        Tkm1 = Tk; Tk = Tn;
+        v[k] = Tk * h.hfc;
+    }
+#pragma unroll
+    for (int t = 0; t < TT; ++t) {
+        const float sel = (TT == 1 || tj == t) ? 1.0f : 0.0f;
+#pragma unroll
+        for (int k = 0; k < KP; ++k)
+            if (k < KP - 3 || k < KR) A[t][k] = fmaf(sel, v[k], A[t][k]);
+    }
+}
+
+template <int TT, int KP>
+__global__ void __launch_bounds__(128)
+k_radial_reg(NepDims D, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
+             const int* __restrict__ ncA, const int* __restrict__ cB, const int* __restrict__ ncB,
+             const float* __restrict__ cR_t, float* __restrict__ q)
+{
+    extern __shared__ float sc[];                        // table [T*T] x tab_stride (rows [k][NRP])
+    for (int t = threadIdx.x; t < TT * TT * tab_stride; t += blockDim.x) sc[t] = cR_t[t];
+    __syncthreads();
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    float A[KP];
+    float A[TT][KP];
 #pragma unroll
-    for (int k = 0; k < KP; ++k) A[k] = 0.0f;
+    for (int t = 0; t < TT; ++t)
+#pragma unroll
+        for (int k = 0; k < KP; ++k) A[t][k] = 0.0f;
     {
-        PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
-        while (w.next()) {
+        PairWalk<0> w(cA, n, s, ncA[s], posq, D);
+        while (w.next(D)) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate<KP>(r2, D.rcR_inv, A);
+            radial_accumulate_typed<TT, KP>(r2, D.rcR_inv, D.KR, w.pj.w, A);
         }
     }
     {
-        PairWalk<0> w(cB, n, s, ncB[s], posq);
-        while (w.next()) {
+        PairWalk<0> w(cB, n, s, ncB[s], posq, D);
+        while (w.next(D)) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate<KP>(r2, D.rcR_inv, A);
+            radial_accumulate_typed<TT, KP>(r2, D.rcR_inv, D.KR, w.pj.w, A);
         }
     }
-    const float H = A[0];
-    A[0] = 2.0f * H;
+    // F_t,0 = 2 A_t,0 ; F_t,k = A_t,k + A_t,0 ; q_n = sum_t sum_k c[ti][t][n][k] F_t,k
 #pragma unroll
-    for (int k = 1; k < KP; ++k) A[k] += H;
-    for (int a = 0; a < D.NR; ++a) {                     // cR_q: [NR][KP] zero-padded (T == 1)
-        const float* c = cR_q + a * KP;
-        float acc = 0.0f;
+    for (int t = 0; t < TT; ++t) {
+        const float H = A[t][0];
+        A[t][0] = 2.0f * H;
 #pragma unroll
-        for (int k = 0; k < KP; ++k) acc = fmaf(__ldg(c + k), A[k], acc);
-        q[(size_t)a * n + s] = acc;
+        for (int k = 1; k < KP; ++k) A[t][k] += H;
+    }
+    float* qp = q + s;
+    for (int a0 = 0; a0 < D.NR; a0 += 4) {
+        float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+        for (int t = 0; t < TT; ++t) {
+            const float* c = sc + (size_t)(pi.w * TT + t) * tab_stride + a0;
+#pragma unroll
+            for (int k = 0; k < KP; ++k) {
+                if (k < KP - 3 || k < D.KR) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) acc[u] = fmaf(c[k * D.NRP + u], A[t][k], acc[u]);
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { if (a0 + u < D.NR) *qp = acc[u]; qp += n; }
     }
 }
 
 // any number of species: accumulators A[t][k] in shared memory, [t][k][thread] (conflict-free).  KP = KR
 // rounded up to a multiple of 4 is a compile-time constant so that the read-modify-write of one pair is
-// KP independent LDS, then the recurrence and FMAs, then KP STS (surplus terms are finite and meet
-// zero-padded coefficients).
-template <int KP>
-__device__ __forceinline__ void radial_accumulate_smem(float r2, float rc_inv, int BS, float* acc)
+// KR independent LDS, then the recurrence and FMAs, then KR STS; the block size is a compile-time
+// constant too, so that every shared-memory offset is an immediate.
+template <int KP, int BS>
+__device__ __forceinline__ void radial_accumulate_smem(float r2, float rc_inv, int KR, float* acc)
 {
     float A[KP];
 #pragma unroll
-    for (int k = 0; k < KP; ++k) A[k] = acc[k * BS];
-    radial_accumulate<KP>(r2, rc_inv, A);
+    for (int k = 0; k < KP; ++k) A[k] = (k < KP - 3 || k < KR) ? acc[k * BS] : 0.0f;
+    radial_accumulate<KP>(r2, rc_inv, A, KR);
 #pragma unroll
-    for (int k = 0; k < KP; ++k) acc[k * BS] = A[k];
+    for (int k = 0; k < KP; ++k) if (k < KP - 3 || k < KR) acc[k * BS] = A[k];
 }
 
-template <int KP, bool TAB_SM>
-__global__ void __launch_bounds__(128)
+template <int KP, bool TAB_SM, int BS>
+__global__ void __launch_bounds__(BS)
 k_radial_multi(NepDims D, int tab_stride, const int4* __restrict__ posq, const int* __restrict__ cA,
                const int* __restrict__ ncA, const int* __restrict__ cB, const int* __restrict__ ncB,
                const float* __restrict__ cR_t, float* __restrict__ q)
 {
-    extern __shared__ float sm[];                        // A[T][KP][BS], then table [T*T] x tab_stride
-    const int BS = blockDim.x;
-    float* sc = sm + (size_t)D.T * KP * BS;
+    extern __shared__ float sm[];                        // A[T][KR][BS], then table [T*T] x tab_stride
+    float* sc = sm + (size_t)D.T * D.KR * BS;
     if (TAB_SM) for (int t = threadIdx.x; t < D.T * D.T * tab_stride; t += BS) sc[t] = cR_t[t];
     float* my = sm + threadIdx.x;
-    for (int t = 0; t < D.T * KP; ++t) my[t * BS] = 0.0f;
+    for (int t = 0; t < D.T * D.KR; ++t) my[t * BS] = 0.0f;
     __syncthreads();
     const int s = blockIdx.x * BS + threadIdx.x;
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    const int tstride = KP * BS;
+    const int tstride = D.KR * BS;
     {
-        PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
-        while (w.next()) {
+        PairWalk<0> w(cA, n, s, ncA[s], posq, D);
+        while (w.next(D)) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate_smem<KP>(r2, D.rcR_inv, BS, my + w.pj.w * tstride);
+            radial_accumulate_smem<KP, BS>(r2, D.rcR_inv, D.KR, my + w.pj.w * tstride);
         }
     }
     {
-        PairWalk<0> w(cB, n, s, ncB[s], posq);
-        while (w.next()) {
+        PairWalk<0> w(cB, n, s, ncB[s], posq, D);
+        while (w.next(D)) {
             float dx, dy, dz, r2;
             pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            radial_accumulate_smem<KP>(r2, D.rcR_inv, BS, my + w.pj.w * tstride);
+            radial_accumulate_smem<KP, BS>(r2, D.rcR_inv, D.KR, my + w.pj.w * tstride);
         }
     }
     // q_n = sum_t sum_k c[ti][t][n][k] F_t,k ; table rows [tp][k][NRP], tp stride odd (conflict-free)
@@ -386,8 +469,8 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
 #pragma unroll
         for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = 0.0f;
     const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride;
-    PairWalk<NEP_SLOT_BITS> w(cA, n, s, ncA[s], posq);
-    while (w.next()) {
+    PairWalk<0> w(cA, n, s, ncA[s], posq, D);
+    while (w.next(D)) {
         float dx, dy, dz, r2;
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -453,24 +536,21 @@ k_angular(NepDims D, NepCoef C, int n0, int tab_stride, const int4* __restrict__
 
 // ---------------------------------------------------------------------------------------------------
 // (a5) U_i = sum_m w1_m tanh(sum_v w0_mv q_v - b0_m) - b1 and Fp_v = dU_i/dq_v   Eq. (1), Listing 1
-// (PAPER.md:52-56, 912-963).  Also the per-atom radial table E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k],
-// which turns the radial partial force of Eq. (21) into KR FMAs per pair and direction.
+// (PAPER.md:52-56, 912-963).
 template <int DP>
 __global__ void __launch_bounds__(128)
-k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, const float* __restrict__ w0p,
-      const float* __restrict__ b0, const float* __restrict__ w1, float b1, const float* __restrict__ cR_e,
-      float* __restrict__ fp, float* __restrict__ U, float* __restrict__ Et)
+k_ann(NepDims D, const float* __restrict__ q, const float* __restrict__ w0p, const float* __restrict__ b0,
+      const float* __restrict__ w1, float b1, float* __restrict__ fp, float* __restrict__ U)
 {
     // Two phases so that neither holds q and Fp in registers at once (occupancy): forward with q in
     // registers, leaving cf_m = w1_m (1 - tanh^2) in shared memory ([m][thread], conflict-free); backward
     // Fp_v = sum_m cf_m w0_mv eight components at a time.  Weight reads are warp-uniform (broadcast).
-    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H], Fp_R [16][BS], cf [H][BS]
+    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H], cf [H][BS]
     const int BS = blockDim.x;
     for (int t = threadIdx.x; t < D.H * DP; t += BS) sw[t] = w0p[t];
     float* sb0 = sw + D.H * DP;
     float* sw1 = sb0 + D.H;
-    float* sfp = sw1 + D.H;
-    float* scf = sfp + 16 * BS;
+    float* scf = sw1 + D.H;
     for (int t = threadIdx.x; t < D.H; t += BS) { sb0[t] = b0[t]; sw1[t] = w1[t]; }
     __syncthreads();
     const int s = blockIdx.x * BS + threadIdx.x;
@@ -497,7 +577,6 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
             mycf[m * BS] = w1m * (1.0f - x1 * x1);
         }
     }
-    float* myfp = sfp + threadIdx.x;
 #pragma unroll
     for (int d0 = 0; d0 < DP; d0 += 8) {
         float acc[8];
@@ -513,30 +592,10 @@ k_ann(NepDims D, const int4* __restrict__ posq, const float* __restrict__ q, con
             acc[6] = fmaf(cf, wb.z, acc[6]); acc[7] = fmaf(cf, wb.w, acc[7]);
         }
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
+        for (int u = 0; u < 8; ++u)
             if (d0 + u < D.D) fp[(size_t)(d0 + u) * n + s] = acc[u];
-            // the radial Fp_n go through shared memory so that the E-table loop below can be a run-time
-            // loop over n (NR <= 16 <= DP)
-            if (d0 + u < 16 && d0 + u < D.NR) myfp[(d0 + u) * BS] = acc[u];
-        }
     }
     U[s] = e - b1;
-    // E table (atom-major so that neighbours can gather a row with 128-bit loads)
-    const int ti = posq[s].w;
-    for (int t = 0; t < D.T; ++t) {
-        const float4* c = reinterpret_cast<const float4*>(cR_e + (size_t)((ti * D.T + t) * D.NR) * D.KRP);
-        float4* out = reinterpret_cast<float4*>(Et + ((size_t)s * D.T + t) * D.KRP);
-        for (int k4 = 0; k4 < D.KRP / 4; ++k4) {
-            float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            for (int a = 0; a < D.NR; ++a) {
-                const float f = myfp[a * BS];
-                const float4 cc = __ldg(c + a * (D.KRP / 4) + k4);
-                acc.x = fmaf(f, cc.x, acc.x); acc.y = fmaf(f, cc.y, acc.y);
-                acc.z = fmaf(f, cc.z, acc.z); acc.w = fmaf(f, cc.w, acc.w);
-            }
-            out[k4] = acc;
-        }
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -573,7 +632,8 @@ __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float 
 template <int NCH>
 __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCoef& C, int n0, int accumulate, int tab_stride,
                                                    const float* tab, const int4* __restrict__ posq,
-                                                   const int* __restrict__ cAr, const int* __restrict__ ncA,
+                                                   const int* __restrict__ cA, const int* __restrict__ ncA,
+                                                   const unsigned long long* __restrict__ mask,
                                                    const float* __restrict__ S_in, const float* __restrict__ fp,
                                                    float4* __restrict__ pf, float4* __restrict__ fa, int s)
 {
@@ -606,8 +666,8 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
     }
     const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride;
     float sx = 0.0f, sy = 0.0f, sz = 0.0f;                 // sum_j dU_i/dr_ij
-    PairWalk<NEP_SLOT_BITS> w(cAr, n, s, ncA[s], posq);
-    while (w.next()) {
+    PairWalk<1> w(cA, n, s, ncA[s], posq, D, mask);
+    while (w.next(D)) {
         float dx, dy, dz, r2;
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -680,7 +740,7 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         sx += out.x; sy += out.y; sz += out.z;
         // delivered to the receiver: row (slot of i in j's column) of atom j -- a fire-and-forget store
         // here instead of a dependent gather in k_final; only this thread ever touches that element
-        float4* dst = pf + (size_t)(w.e & ((1 << NEP_SLOT_BITS) - 1)) * n + (w.e >> NEP_SLOT_BITS);
+        float4* dst = pf + (size_t)w.slot(D) * n + w.j();
         if (accumulate) { const float4 o = *dst; out.x += o.x; out.y += o.y; out.z += o.z; }
         *dst = out;
     }
@@ -691,91 +751,297 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
 template <int NCH, bool SM>
 __global__ void __launch_bounds__(128)
 k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
-                const int* __restrict__ cAr, const int* __restrict__ ncA, const float* __restrict__ cA_t,
-                const float* __restrict__ S_in, const float* __restrict__ fp, float4* __restrict__ pf,
-                float4* __restrict__ fa, int* __restrict__ tile_ctr)
+                const int* __restrict__ cA, const int* __restrict__ ncA, const unsigned long long* __restrict__ mask,
+                const float* __restrict__ cA_t, const float* __restrict__ S_in, const float* __restrict__ fp,
+                float4* __restrict__ pf, float4* __restrict__ fa, int* __restrict__ tile_ctr)
 {
     extern __shared__ __align__(16) float sc[];
     const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
     const int ntile = (D.n + 31) >> 5;
     for (int tile = next_tile(tile_ctr); tile < ntile; tile = next_tile(tile_ctr)) {
         const int s = tile * 32 + (threadIdx.x & 31);
-        if (s < D.n) force_angular_atom<NCH>(D, C, n0, accumulate, tab_stride, tab, posq, cAr, ncA, S_in, fp, pf, fa, s);
+        if (s < D.n) force_angular_atom<NCH>(D, C, n0, accumulate, tab_stride, tab, posq, cA, ncA, mask, S_in, fp, pf, fa, s);
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// (a6)+(a8) forces and virials.
-//  radial: dU_i/dr_ij = [sum_k E^i[tj][k] f_k'(r)] u,  dU_j/dr_ji = -[sum_k E^j[ti][k] f_k'(r)] u
-//    f_k' = P_k + f_c'/2 with P_k = T_k f_c'/2 + T_k' (f_c/2) x':  P_0 = f_c'/2, P_1 = x f_c'/2 + (f_c/2) x',
-//    P_{k+1} = 2 x P_k - P_{k-1} + 2 (f_c/2) x' T_k   (from T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}')
-//  angular: sum_j dU_i/dr_ij was reduced by k_force_angular (fa); dU_j/dr_ji was delivered by atom j to
-//    row m of this atom's column (pf[m][i], j = cA[m][i]) -- coalesced reads, no gather, no atomics
-//  F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji)  (Eqs. 22-23);  W_i = sum_j r_ij (x) dU_j/dr_ji  (Eq. 24)
-// The row E^j[ti] of the next neighbour is fetched while the current pair is computed (NK4 = KRP/4
-// float4 registers), because that gather is the long-latency operation of this kernel.
+// (a6) radial partial forces, sender side.   dU_i/dr_ij = m_ij u_ij  (first term of Eq. (21)) with
+//   m_ij = sum_k E^i[tj][k] f_k'(r_ij),   E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
+// (an exact re-association of sum_n Fp_n g_n'(r_ij): KR FMAs per pair instead of NR x KR).
+//   f_k' = P_k + f_c'/2 with P_k = T_k f_c'/2 + T_k' (f_c/2) x':  P_0 = f_c'/2, P_1 = x f_c'/2 + (f_c/2) x',
+//   P_{k+1} = 2 x P_k - P_{k-1} + 2 (f_c/2) x' T_k   (from T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}')
+// The scalar m_ij is delivered to the receiver j (a fire-and-forget store; only this thread ever touches
+// that element): mA[slot][j] for the angular-range pairs, mB[slot][j] for the outer shell.  (Not into the
+// .w of pf: a 4-byte write into a sector that has left L2 costs a DRAM read-modify-write.)  The own sum  sum_j m_ij u_ij  is added to fa[i].
+// E^i lives in shared memory, [t][k][thread] (conflict-free), T x KR rows: as little as possible, because
+// shared memory is carved out of the L1 that serves the neighbour gathers.
+template <int KP, int BS>
+__device__ __forceinline__ float radial_m(float r, float rc_inv, int KR, const float* __restrict__ E)
+{
+    const BasisHead h = basis_head<true>(r, rc_inv);
+    const float c2 = 2.0f * h.hfc_dx;
+    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
+    float Ev[KP];
+#pragma unroll
+    for (int k = 0; k < KP; ++k) Ev[k] = (k < KP - 3 || k < KR) ? E[k * BS] : 0.0f;
+    float m0 = 0.0f, m1 = 0.0f;
+#pragma unroll
+    for (int k = 0; k < KP; ++k) {
+        if (k < KP - 3 || k < KR) {                   // uniform: KP - 3 <= KR <= KP
+            const float df = Pa + h.hdfc;             // f_k'
+            if (k & 1) m1 = fmaf(Ev[k], df, m1); else m0 = fmaf(Ev[k], df, m0);
+            const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
+            const float Tn = fmaf(h.two_x, Tb, -Ta);
+            Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
+        }
+    }
+    return m0 + m1;
+}
+
+// register variant for few species (TT * KP <= 64): E^i[t][k] in registers, all TT dot products per pair,
+// the neighbour's type selects one -- no shared memory beyond the staged coefficient table.
+template <int TT, int KP>
+__device__ __forceinline__ float radial_m_typed(float r, float rc_inv, int KR, int tj, const float (&E)[TT][KP])
+{
+    const BasisHead h = basis_head<true>(r, rc_inv);
+    const float c2 = 2.0f * h.hfc_dx;
+    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
+    float m[TT];
+#pragma unroll
+    for (int t = 0; t < TT; ++t) m[t] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < KP; ++k) {
+        if (k < KP - 3 || k < KR) {                   // uniform: KP - 3 <= KR <= KP
+            const float df = Pa + h.hdfc;             // f_k'
+#pragma unroll
+            for (int t = 0; t < TT; ++t) m[t] = fmaf(E[t][k], df, m[t]);
+            const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
+            const float Tn = fmaf(h.two_x, Tb, -Ta);
+            Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
+        }
+    }
+    float out = m[0];
+#pragma unroll
+    for (int t = 1; t < TT; ++t) out = (tj == t) ? m[t] : out;
+    return out;
+}
+
+template <int TT, int KP>
+__global__ void __launch_bounds__(128)
+k_force_radial_reg(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, const int* __restrict__ ncA,
+                   const int* __restrict__ cB, const int* __restrict__ ncB, const unsigned long long* __restrict__ mask,
+                   const float* __restrict__ fp, const float* __restrict__ cR_e, float* __restrict__ mA,
+                   float* __restrict__ mB, float4* __restrict__ fa)
+{
+    extern __shared__ __align__(16) float sc[];          // cR_e [T*T][NR][KP]
+    {
+        const int cnt4 = TT * TT * D.NR * (KP / 4);
+        for (int t = threadIdx.x; t < cnt4; t += blockDim.x) reinterpret_cast<float4*>(sc)[t] = reinterpret_cast<const float4*>(cR_e)[t];
+        __syncthreads();
+    }
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= D.n) return;
+    const size_t n = (size_t)D.n;
+    const int4 pi = posq[s];
+    float E[TT][KP];
+    {
+#pragma unroll
+        for (int t = 0; t < TT; ++t)
+#pragma unroll
+            for (int k = 0; k < KP; ++k) E[t][k] = 0.0f;
+        const float* fpa = fp + s;
+        for (int a = 0; a < D.NR; ++a) {
+            const float f = *fpa;
+            fpa += n;
+#pragma unroll
+            for (int t = 0; t < TT; ++t) {
+                const float4* c = reinterpret_cast<const float4*>(sc) + (size_t)((pi.w * TT + t) * D.NR + a) * (KP / 4);
+#pragma unroll
+                for (int k4 = 0; k4 < KP / 4; ++k4) {
+                    const float4 cc = c[k4];
+                    E[t][4 * k4 + 0] = fmaf(f, cc.x, E[t][4 * k4 + 0]); E[t][4 * k4 + 1] = fmaf(f, cc.y, E[t][4 * k4 + 1]);
+                    E[t][4 * k4 + 2] = fmaf(f, cc.z, E[t][4 * k4 + 2]); E[t][4 * k4 + 3] = fmaf(f, cc.w, E[t][4 * k4 + 3]);
+                }
+            }
+        }
+    }
+    float fx = 0.0f, fy = 0.0f, fz = 0.0f;
+    {
+        PairWalk<1> w(cA, n, s, ncA[s], posq, D, mask);
+        while (w.next(D)) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            const float rinv = rsqrtf(r2);
+            const float m = radial_m_typed<TT, KP>(r2 * rinv, D.rcR_inv, D.KR, w.pj.w, E);
+            const float mr = m * rinv;
+            fx = fmaf(mr, dx, fx); fy = fmaf(mr, dy, fy); fz = fmaf(mr, dz, fz);
+            mA[(size_t)w.slot(D) * n + w.j()] = m;
+        }
+    }
+    {
+        const int nsplit = (int)mask[(size_t)s * D.mrec + 2 * D.maskW + 1];
+        PairWalk<2> w(cB, n, s, ncB[s], posq, D, mask, nsplit);
+        while (w.next(D)) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            const float rinv = rsqrtf(r2);
+            const float m = radial_m_typed<TT, KP>(r2 * rinv, D.rcR_inv, D.KR, w.pj.w, E);
+            const float mr = m * rinv;
+            fx = fmaf(mr, dx, fx); fy = fmaf(mr, dy, fy); fz = fmaf(mr, dz, fz);
+            mB[(size_t)w.slot(D) * n + w.j()] = m;
+        }
+    }
+    float4 own = fa[s];
+    own.x += fx; own.y += fy; own.z += fz;
+    fa[s] = own;
+}
+
+template <int KP, bool TAB_SM, int BS>
+__global__ void __launch_bounds__(BS)
+k_force_radial(NepDims D, const int4* __restrict__ posq, const int* __restrict__ cA, const int* __restrict__ ncA,
+               const int* __restrict__ cB, const int* __restrict__ ncB, const unsigned long long* __restrict__ mask,
+               const float* __restrict__ fp, const float* __restrict__ cR_e, float* __restrict__ mA,
+               float* __restrict__ mB, float4* __restrict__ fa)
+{
+    extern __shared__ __align__(16) float sm[];          // E [T][KR][BS] (16-byte padded), then cR_e [T*T][NR][KP]
+    float* sc = sm + (size_t)round_up4_dev(D.T * D.KR) * BS;
+    if (TAB_SM) {
+        const int cnt4 = D.T * D.T * D.NR * (KP / 4);
+        for (int t = threadIdx.x; t < cnt4; t += BS) reinterpret_cast<float4*>(sc)[t] = reinterpret_cast<const float4*>(cR_e)[t];
+        __syncthreads();
+    }
+    const int s = blockIdx.x * BS + threadIdx.x;
+    if (s >= D.n) return;
+    const size_t n = (size_t)D.n;
+    const int4 pi = posq[s];
+    float* my = sm + threadIdx.x;
+    {   // E^i[t][k] from the radial components of Fp (re-read per neighbour type: L1 hits)
+        const float4* tab4 = reinterpret_cast<const float4*>(TAB_SM ? sc : cR_e);
+        for (int t = 0; t < D.T; ++t) {
+            const float4* c = tab4 + (size_t)((pi.w * D.T + t) * D.NR) * (KP / 4);
+            float4 acc[KP / 4];
+#pragma unroll
+            for (int k4 = 0; k4 < KP / 4; ++k4) acc[k4] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            const float* fpa = fp + s;
+            for (int a = 0; a < D.NR; ++a) {
+                const float f = *fpa;
+                fpa += n;
+#pragma unroll
+                for (int k4 = 0; k4 < KP / 4; ++k4) {
+                    const float4 cc = TAB_SM ? c[a * (KP / 4) + k4] : __ldg(c + a * (KP / 4) + k4);
+                    acc[k4].x = fmaf(f, cc.x, acc[k4].x); acc[k4].y = fmaf(f, cc.y, acc[k4].y);
+                    acc[k4].z = fmaf(f, cc.z, acc[k4].z); acc[k4].w = fmaf(f, cc.w, acc[k4].w);
+                }
+            }
+            float* e = my + (size_t)(t * D.KR) * BS;
+#pragma unroll
+            for (int k4 = 0; k4 < KP / 4; ++k4) {
+                const float v[4] = {acc[k4].x, acc[k4].y, acc[k4].z, acc[k4].w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (4 * k4 + u < KP - 3 || 4 * k4 + u < D.KR) e[(4 * k4 + u) * BS] = v[u];
+            }
+        }
+    }
+    const int tstride = D.KR * BS;
+    float fx = 0.0f, fy = 0.0f, fz = 0.0f;
+    {
+        PairWalk<1> w(cA, n, s, ncA[s], posq, D, mask);
+        while (w.next(D)) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            const float rinv = rsqrtf(r2);
+            const float m = radial_m<KP, BS>(r2 * rinv, D.rcR_inv, D.KR, my + w.pj.w * tstride);
+            const float mr = m * rinv;
+            fx = fmaf(mr, dx, fx); fy = fmaf(mr, dy, fy); fz = fmaf(mr, dz, fz);
+            mA[(size_t)w.slot(D) * n + w.j()] = m;
+        }
+    }
+    {
+        const int nsplit = (int)mask[(size_t)s * D.mrec + 2 * D.maskW + 1];
+        PairWalk<2> w(cB, n, s, ncB[s], posq, D, mask, nsplit);
+        while (w.next(D)) {
+            float dx, dy, dz, r2;
+            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
+            const float rinv = rsqrtf(r2);
+            const float m = radial_m<KP, BS>(r2 * rinv, D.rcR_inv, D.KR, my + w.pj.w * tstride);
+            const float mr = m * rinv;
+            fx = fmaf(mr, dx, fx); fy = fmaf(mr, dy, fy); fz = fmaf(mr, dz, fz);
+            mB[(size_t)w.slot(D) * n + w.j()] = m;
+        }
+    }
+    float4 own = fa[s];
+    own.x += fx; own.y += fy; own.z += fz;
+    fa[s] = own;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// (a8) forces and virials, receiver side.  Row m of this atom's columns holds what neighbour j = cA[m][i]
+// (or cB[m][i]) delivered: dU_j/dr_ji = pf[m][i].xyz - mA[m][i] u_ij  (angular part, radial scalar m_ji;
+// u_ji = -u_ij), resp. -mB[m][i] u_ij for the outer shell -- coalesced reads, no gather of partial
+// forces, no atomics.  fa[i] = sum_j dU_i/dr_ij (both parts).
+//   F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji)  (Eqs. 22-23);  W_i = sum_j r_ij (x) dU_j/dr_ji  (Eq. 24)
 struct FinalAcc {
     float fx, fy, fz, w[9];
 };
 
-__device__ __forceinline__ void virial_add(FinalAcc& acc, float dx, float dy, float dz, float px, float py, float pz)
+__device__ __forceinline__ void final_pair(FinalAcc& acc, float dx, float dy, float dz, float px, float py, float pz)
 {
+    acc.fx -= px; acc.fy -= py; acc.fz -= pz;
     acc.w[0] = fmaf(dx, px, acc.w[0]); acc.w[1] = fmaf(dx, py, acc.w[1]); acc.w[2] = fmaf(dx, pz, acc.w[2]);
     acc.w[3] = fmaf(dy, px, acc.w[3]); acc.w[4] = fmaf(dy, py, acc.w[4]); acc.w[5] = fmaf(dy, pz, acc.w[5]);
     acc.w[6] = fmaf(dz, px, acc.w[6]); acc.w[7] = fmaf(dz, py, acc.w[7]); acc.w[8] = fmaf(dz, pz, acc.w[8]);
 }
 
-// radial part of one pair; ei4 = row E^i[tj] (own atom, L1), ej = row E^j[ti] (prefetched registers)
-template <int NK4>
-__device__ __forceinline__ void final_radial_pair(const NepDims& D, float dx, float dy, float dz, float r2,
-                                                  const float4* __restrict__ ei4, const float4 (&ej)[NK4], FinalAcc& acc)
+// one list of one atom, four pairs at a time: the four entries of the next batch, then the four neighbour
+// positions and the four received records of this batch are in flight together (the kernel is bound by
+// memory latency, not arithmetic)
+template <bool ANG>
+__device__ __forceinline__ void final_walk(const NepDims& D, const int4& pi, const int4* __restrict__ posq,
+                                           const int* __restrict__ lp, const float* __restrict__ colm,
+                                           const float4* __restrict__ colp, int cnt, FinalAcc& acc)
 {
-    const float rinv = rsqrtf(r2), r = r2 * rinv;
-    const BasisHead h = basis_head<true>(r, D.rcR_inv);
-    const float c2 = 2.0f * h.hfc_dx;
-    float Ta = 1.0f, Tb = h.x, Pa = h.hdfc, Pb = fmaf(h.x, h.hdfc, h.hfc_dx);
-    float mi = 0.0f, mj = 0.0f;
+    const size_t n = (size_t)D.n;
+    int en[4];
 #pragma unroll
-    for (int k4 = 0; k4 < NK4; ++k4) {
-        const float4 a = __ldg(ei4 + k4), bq = ej[k4];
-        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {bq.x, bq.y, bq.z, bq.w};
+    for (int u = 0; u < 4; ++u) en[u] = (u < cnt) ? lp[(size_t)u * n] : 0;
+    for (int m0 = 0; m0 < cnt; m0 += 4) {
+        int4 pj[4]; float mv[4]; float4 pv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pj[u] = posq[en[u] >> NEP_SLOT_BITS];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            if (4 * k4 + u < D.KR) {                      // uniform: skips the padding of the last group
-                const float df = Pa + h.hdfc;             // f_k'
-                mi = fmaf(av[u], df, mi); mj = fmaf(bv[u], df, mj);
-                const float Pn = fmaf(h.two_x, Pb, fmaf(c2, Tb, -Pa));
-                const float Tn = fmaf(h.two_x, Tb, -Ta);
-                Pa = Pb; Pb = Pn; Ta = Tb; Tb = Tn;
+            if (m0 + u < cnt) {
+                mv[u] = colm[(size_t)(m0 + u) * n];
+                if (ANG) pv[u] = colp[(size_t)(m0 + u) * n];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) en[u] = (m0 + 4 + u < cnt) ? lp[(size_t)(m0 + 4 + u) * n] : 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (m0 + u < cnt) {
+                float dx, dy, dz, r2;
+                pair_vec(pi, pj[u], D, dx, dy, dz, r2);
+                const float rinv = rsqrtf(r2);
+                const float sr = -mv[u] * rinv;
+                if (ANG) final_pair(acc, dx, dy, dz, fmaf(sr, dx, pv[u].x), fmaf(sr, dy, pv[u].y), fmaf(sr, dz, pv[u].z));
+                else final_pair(acc, dx, dy, dz, sr * dx, sr * dy, sr * dz);
             }
         }
     }
-    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-    const float ft = mi + mj;                        // (dU_i/dr_ij - dU_j/dr_ji) = (mi + mj) u
-    acc.fx = fmaf(ft, ux, acc.fx); acc.fy = fmaf(ft, uy, acc.fy); acc.fz = fmaf(ft, uz, acc.fz);
-    virial_add(acc, dx, dy, dz, -mj * ux, -mj * uy, -mj * uz);   // dU_j/dr_ji
 }
 
-template <int NK4>
-__device__ __forceinline__ void load_erow(float4 (&e)[NK4], const float4* __restrict__ row)
-{
-#pragma unroll
-    for (int k4 = 0; k4 < NK4; ++k4) e[k4] = __ldg(row + k4);
-}
-
-template <int NK4>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(256)
 k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
         const int* __restrict__ cA, const int* __restrict__ ncA, const int* __restrict__ cB,
-        const int* __restrict__ ncB, const float* __restrict__ Et,
-        const float4* __restrict__ pf, const float4* __restrict__ fa, const float* __restrict__ U,
+        const int* __restrict__ ncB, const float4* __restrict__ pf, const float* __restrict__ mA, const float* __restrict__ mB,
+        const float4* __restrict__ fa, const float* __restrict__ U,
         double* __restrict__ e_out, double* __restrict__ f_out, double* __restrict__ w_out)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
-    const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    const int ti = pi.w;
     FinalAcc acc;
     {
         const float4 own = fa[s];
@@ -783,40 +1049,8 @@ k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
     }
 #pragma unroll
     for (int a = 0; a < 9; ++a) acc.w[a] = 0.0f;
-    const int na = ncA[s];
-    const int atomf4 = D.T * NK4;
-    const float4* Et4 = reinterpret_cast<const float4*>(Et);
-    const float4* Ei4 = Et4 + (size_t)s * atomf4;
-    const float4* Ej4 = Et4 + ti * NK4;                  // + j * atomf4: row E^j[ti]
-    float4 ecur[NK4], enext[NK4];
-    {   // angular-range pairs: radial part + the angular partial forces received from the neighbours
-        PairWalk<NEP_SLOT_BITS> w(cA, n, s, na, posq);
-        if (na > 0) load_erow<NK4>(enext, Ej4 + (size_t)(w.e1 >> NEP_SLOT_BITS) * atomf4);
-        while (w.next()) {
-            const float4 oth = pf[(size_t)w.m * n + s];
-#pragma unroll
-            for (int k4 = 0; k4 < NK4; ++k4) ecur[k4] = enext[k4];
-            if (w.m + 1 < na) load_erow<NK4>(enext, Ej4 + (size_t)(w.e1 >> NEP_SLOT_BITS) * atomf4);
-            float dx, dy, dz, r2;
-            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            final_radial_pair<NK4>(D, dx, dy, dz, r2, Ei4 + w.pj.w * NK4, ecur, acc);
-            acc.fx -= oth.x; acc.fy -= oth.y; acc.fz -= oth.z;
-            virial_add(acc, dx, dy, dz, oth.x, oth.y, oth.z);
-        }
-    }
-    {   // outer shell: radial part only
-        const int nb = ncB[s];
-        PairWalk<0> w(cB, n, s, nb, posq);
-        if (nb > 0) load_erow<NK4>(enext, Ej4 + (size_t)w.e1 * atomf4);
-        while (w.next()) {
-#pragma unroll
-            for (int k4 = 0; k4 < NK4; ++k4) ecur[k4] = enext[k4];
-            if (w.m + 1 < nb) load_erow<NK4>(enext, Ej4 + (size_t)w.e1 * atomf4);
-            float dx, dy, dz, r2;
-            pair_vec(pi, w.pj, D, dx, dy, dz, r2);
-            final_radial_pair<NK4>(D, dx, dy, dz, r2, Ei4 + w.pj.w * NK4, ecur, acc);
-        }
-    }
+    final_walk<true>(D, pi, posq, cA + s, mA + s, pf + s, ncA[s], acc);
+    final_walk<false>(D, pi, posq, cB + s, mB + s, nullptr, ncB[s], acc);
     const size_t i = (size_t)perm[s];
     if (e_out) e_out[i] = (double)U[s];
     if (f_out) { f_out[3 * i + 0] = (double)acc.fx; f_out[3 * i + 1] = (double)acc.fy; f_out[3 * i + 2] = (double)acc.fz; }

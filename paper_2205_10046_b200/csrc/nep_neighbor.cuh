@@ -10,7 +10,7 @@
 //   4. one thread per atom walks the 5x5x5 stencil cells, tests candidates in fp32 and resolves
 //      anything inside a guard band around a cutoff with the exact fp64 predicate of reading A8, so
 //      the sets equal an fp64 brute force bit for bit
-//   5. reverse index: slot of i in j's angular list (for the scatter-free gather of Eq. 22-24)
+//   5. reverse index: slot of i in j's list, for both lists (where i delivers dU_i/dr_ij to j, Eq. 22-24)
 // The angular-range list (|r| < rcA+skin) and the outer shell (rcA+skin <= |r| < rcR+skin) are stored
 // disjointly; the radial list is their union.
 #pragma once
@@ -241,7 +241,7 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
 }
 
 // ---- 5. reverse index -----------------------------------------------------------------------------------
-__global__ void k_build_rev(int n, int capA, const int* __restrict__ listA, const int* __restrict__ cntA,
+__global__ void k_build_rev(int n, const int* __restrict__ listA, const int* __restrict__ cntA,
                             unsigned char* __restrict__ rev)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
