@@ -586,7 +586,6 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     d.rcR = (float)h->rc_radial; d.rcA = (float)h->rc_angular;
     d.rcR_inv = (float)(1.0 / h->rc_radial); d.rcA_inv = (float)(1.0 / h->rc_angular);
     d.rcR2 = d.rcR * d.rcR; d.rcA2 = d.rcA * d.rcA;
-    if (const char* e = getenv("NEP_DBG")) d.dbg = atoi(e);
     nep->DP = ann_tier(d.D);
     if (nep->DP < 0) { delete nep; return NEP_ERR_INVALID_ARG; }
     for (int t = 0; t < d.T; ++t) {

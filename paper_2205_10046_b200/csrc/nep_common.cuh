@@ -36,7 +36,6 @@ struct NepDims {
     float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
     int capA, capS;              // storage rows of the skin lists (angular-range part, outer shell)
     int maskW;                   // 64-bit words of one in-cutoff mask (covers the longest skin list)
-    int dbg;                     // NEP_DBG experiments (0 in production)
     int mrec;                    // 64-bit words of an atom's mask record (4 maskW, see k_filter)
 };
 

@@ -3,15 +3,21 @@
 // One thread per atom in the internal spatial order (tile-major Morton order of the cells, so that a
 // warp's 32 atoms and their neighbours are a compact blob and the neighbour gathers hit L1).  Per-atom
 // arrays are stored [component][atom] so that a warp reads/writes 128 contiguous bytes per component.
-// Every pair loop is software-pipelined: the index two pairs ahead and the position one pair ahead
+// Every pair loop is software-pipelined: the entry two pairs ahead and the position one pair ahead
 // are in flight while the current pair is computed.  Kernels per evaluation:
-//   k_filter              skin lists -> this step's in-cutoff lists (removes the in-cutoff divergence)
-//   k_radial1<KP> / k_radial_multi   Eqs. (2)-(5) radial descriptor via per-type basis sums
+//   k_filter              skin lists -> this step's in-cutoff lists + in-cutoff masks (removes the
+//                         in-cutoff divergence from every later kernel)
+//   k_radial_reg<T,KP> / k_radial_multi<KP,..>   Eqs. (2)-(5) radial descriptor via per-type basis sums
+//                         (accumulators in registers for few species, else in shared memory)
 //   k_angular<NCH,SM>     Eq. (12), (13)-(19) angular sums (24*NCH accumulators in registers) + components
-//   k_ann<DP>             Eq. (1) / Listing 1; also E^i[t][k] = sum_n Fp_n c^R[ti][t][n][k]
-//   k_force_angular<NCH,SM>  last three terms of Eq. (21): dU_i/dr_ij for every angular pair
-//   k_final               first term of Eq. (21) for both directions via the E tables; Eqs. (22)-(24):
-//                         scatter-free gather of dU_j/dr_ji through the reverse index
+//   k_ann<DP>             Eq. (1) / Listing 1: U_i and Fp = dU_i/dq
+//   k_force_angular<NCH,SM>  last three terms of Eq. (21): dU_i/dr_ij of every angular pair, delivered to j
+//   k_force_radial_reg<T,KP> / k_force_radial<KP,..>   first term of Eq. (21): m_ij of every pair, delivered to j
+//   k_final               Eqs. (22)-(24): each atom streams what its neighbours delivered (scatter-free on
+//                         the read side, no atomics anywhere)
+// "Delivered": the sender i stores into row (compact slot of i in j's column) of atom j; that slot is a
+// popcount over j's in-cutoff mask below the skin slot of i in j's list (reverse index built with the
+// lists), computed inline from a 16-byte gather.
 #pragma once
 #include "nep_common.cuh"
 

@@ -4,8 +4,11 @@ Empty neighbourhoods (one atom; a dilute gas where most atoms see nobody), a dim
 not fill a warp or a block, atoms exactly on the box faces and outside [0, L), a box of exactly the
 minimum legal size, list overflow beyond the 256-slot limit, zero-step md_step, the host-buffer entry
 points (nep_compute_host / md_run_host) against the device ones, model variants without the 4-/5-body
-blocks and with the largest supported basis sizes.
+blocks and with the largest supported basis sizes, skin lists longer than 64 and 128 slots (multi-word
+in-cutoff masks), more species than the register kernels take, and the shared-memory variants of the
+radial kernels (NEP_RADIAL_SMEM).
 """
+import os
 from dataclasses import replace
 
 import numpy as np
@@ -155,6 +158,55 @@ def test_hyperparameter_extremes(pkg, oracle_mod, nr, na, kr, ka, H, T):
     cfg = replace(base, hyper=hy, masses=tuple([24.0, 27.0, 64.0][:T]), species_rule="random" if T > 1 else "single")
     s, p = W.make_system(cfg), W.make_params(cfg, "stress")
     run_both(pkg, oracle_mod, hy, p, s.masses, s.pos, s.types, s.box, skin=0.0)
+
+
+def _dense_cubic(seed, cells, a, n_types):
+    """simple-cubic lattice with Gaussian displacements: a dense periodic system (1 / a^3 atoms per A^3)"""
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 903, seed]))
+    g = np.stack(np.meshgrid(*[np.arange(cells)] * 3, indexing="ij"), axis=-1).reshape(-1, 3).astype(np.float64)
+    pos = (g + 0.5) * a + rng.normal(0.0, 0.08, size=g.shape)
+    box = np.array([cells * a] * 3)
+    return np.mod(pos, box), rng.integers(0, n_types, size=len(pos)).astype(np.int32), box
+
+
+@pytest.mark.parametrize("a,expect_words", [(1.75, 2), (1.45, 3)])
+def test_skin_lists_longer_than_one_mask_word(pkg, oracle_mod, a, expect_words):
+    """More than 64 (a = 1.75 A) and more than 128 (a = 1.45 A) neighbours inside rc_angular + skin and in
+    the shell up to rc_radial + skin: the in-cutoff masks take several 64-bit words and the delivery slot
+    is a popcount across words."""
+    cfg = W.get_config(3, (4, 4, 3))
+    hy = replace(cfg.hyper, rc_radial=5.0, rc_angular=4.0)
+    cells = int(np.ceil(12.2 / a))
+    pos, types, box = _dense_cubic(1, cells, a, hy.n_types)
+    p = W.make_params(replace(cfg, hyper=hy))
+    nep = pkg.NEP(hy, p, cfg.masses, device=0)
+    nep.nep_neighbors(torch.tensor(pos, device="cuda:0"), torch.tensor(types, device="cuda:0"), box, 1.0)
+    assert (nep.nep_max_neighbors(1) + 63) // 64 >= expect_words
+    nep.close()
+    run_both(pkg, oracle_mod, hy, p, cfg.masses, pos, types, box, skin=1.0)
+
+
+def test_more_species_than_the_register_kernels_take(pkg, oracle_mod):
+    """Seven species: the radial kernels with per-type tables in shared memory."""
+    base = W.get_config(2, (3, 3, 3))
+    hy = W.Hyper(n_types=7, rc_radial=6.0, rc_angular=4.0, n_max_radial=4, n_max_angular=4, basis_radial=8,
+                 basis_angular=8, n_neurons=20)
+    cfg = replace(base, hyper=hy, masses=tuple(20.0 + 3.0 * t for t in range(7)), species_rule="random")
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    run_both(pkg, oracle_mod, hy, p, s.masses, s.pos, s.types, s.box, skin=0.5)
+
+
+@pytest.mark.parametrize("idx,cells", [(0, None), (2, (3, 3, 3)), (3, (4, 4, 3))])
+def test_shared_memory_radial_variants(pkg, oracle_mod, idx, cells):
+    """The configurations' species counts have register variants of the radial kernels; NEP_RADIAL_SMEM
+    (read at nep_create) selects the shared-memory ones, which must agree with the oracle as well."""
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    os.environ["NEP_RADIAL_SMEM"] = "1"
+    try:
+        run_both(pkg, oracle_mod, cfg.hyper, p, s.masses, s.pos, s.types, s.box, skin=0.3 if cells else cfg.skin)
+    finally:
+        del os.environ["NEP_RADIAL_SMEM"]
 
 
 def test_md_step_zero_steps_and_state_errors(pkg):
