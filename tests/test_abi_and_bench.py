@@ -78,14 +78,17 @@ def test_replica_aggregation_gloo_world2():
 
 
 def test_cost_model_matches_survey_table():
-    """cfg 0/1/3 radial pair 161 + 307 flops, angular pair 420 + 1,160 + 30."""
+    """cfg 0/1/3 radial pair 161 + 307 flops, angular pair 420 + 1,160 + 30.  The 307
+    are BOTH directions of a pair evaluated at one atom (Alg. 2); every direction is needed once, so the
+    model charges one direction per ordered pair, 55 + (307 - 55) / 2 = 181, and the 30-flop gather for
+    every radial pair (an angular pair is one)."""
     sys.path.insert(0, ROOT)
     import bench
     import workloads as W
     h = W.get_config(3).hyper
     c = bench.kernel_costs(h, 0, 1, 0, 0, 0)
-    assert c["radial"][0] == 161 and c["final"][0] == 307
-    c = bench.kernel_costs(h, 0, 0, 1, 0, 0)
+    assert c["radial"][0] == 161 and c["force_radial"][0] == 55 + (307 - 55) // 2 and c["final"][0] == 30
+    c = bench.kernel_costs(h, 0, 1, 1, 0, 0)
     assert c["angular"][0] == 420 and c["force_angular"][0] == 1160 and c["final"][0] == 30
 
 
