@@ -219,3 +219,32 @@ def md(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int, 
     if rc != 0:
         raise MemoryError("oracle allocation failed")
     return pos, vel, ep, ek
+
+
+# ---- outputs derived from what the path already computes --------------
+def latent(params, q):
+    """Latent-space vector of every atom: "an N_neu-dimensional space spanned by the vectors
+    whose components are the product of the states of the hidden-layer neurons and the connection weights
+    between them and the output layer":  latent[i][mu] = w1[mu] * tanh(sum_nu w0[mu][nu] q[i][nu] - b0[mu])
+    with the hidden-layer state of Eq. (1).  q: [n][D] fp64 descriptors."""
+    w0, b0, w1 = _d(params.w0), _d(params.b0), _d(params.w1)
+    q = _d(q)
+    n, H = q.shape[0], w0.shape[0]
+    out = np.zeros((n, H))
+    for i in range(n):
+        for mu in range(H):
+            out[i, mu] = w1[mu] * np.tanh(np.dot(w0[mu], q[i]) - b0[mu])
+    return out
+
+
+def heat_current(virial, vel):
+    """Per-atom heat current J_i = W_i . v_i, Eq. (25), with the 9-component virial of
+    Eq. (24) in the layout W[3a+b] (reading A9), i.e. J_i^a = sum_b W_i^{ab} v_i^b; and the total
+    J = sum_i J_i, Eq. (26).  Returns (J_atom[n][3], J_total[3]); units eV * Angstrom / fs."""
+    W, v = _d(virial), _d(vel)
+    n = W.shape[0]
+    ja = np.zeros((n, 3))
+    for i in range(n):
+        for a in range(3):
+            ja[i, a] = W[i, 3 * a + 0] * v[i, 0] + W[i, 3 * a + 1] * v[i, 1] + W[i, 3 * a + 2] * v[i, 2]
+    return ja, ja.sum(axis=0)

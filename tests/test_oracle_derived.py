@@ -1,0 +1,100 @@
+"""Pins of the oracle's derived outputs (CPU only): the latent-space vector and the heat
+current (Eqs. 25-26).  Each is checked against something other than its own formula:
+
+  * latent: a hand case; sum_mu latent_mu - b1 = U_i with U_i from the C network of Listing 1 (another
+    code path); tanh bounds |latent_mu| <= |w1_mu|; the latent vector of the full pipeline reproduces the
+    site energies the oracle's compute() returns
+  * heat current: Eq. (25)'s second form on a dimer with dU_1/dr_10 from finite differences of atom 1's
+    own site energy; rigid translation v_i = v0: J = (sum_i W_i) v0 = -(dE/d eps) v0 with the strain
+    derivative by finite differences; J is linear in v and invariant to the order of atoms
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+
+
+def test_latent_hand_case(oracle_mod):
+    class P:
+        w0 = np.array([[0.5, -1.0], [2.0, 0.25]]); b0 = np.array([0.1, -0.2]); w1 = np.array([3.0, -0.5]); b1 = np.array([0.7])
+    q = np.array([[1.0, 2.0]])
+    lat = oracle_mod.latent(P, q)
+    # neuron 0: tanh(0.5 - 2.0 - 0.1) = tanh(-1.6); neuron 1: tanh(2.0 + 0.5 + 0.2) = tanh(2.7)
+    assert lat[0, 0] == pytest.approx(3.0 * -0.9216685544064713, rel=1e-14)
+    assert lat[0, 1] == pytest.approx(-0.5 * 0.9910074536781176, rel=1e-14)
+
+
+def test_latent_sums_to_site_energy(oracle_mod):
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    e, f, w, q, fp, S = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box, want_internals=True)
+    lat = oracle_mod.latent(p, q)
+    assert lat.shape == (len(s.pos), cfg.hyper.n_neurons)
+    np.testing.assert_allclose(lat.sum(axis=1) - float(p.b1[0]), e, rtol=1e-12, atol=1e-13)
+    assert (np.abs(lat) <= np.abs(np.asarray(p.w1, dtype=np.float64))[None, :] + 1e-15).all()
+    # and against the C network of Listing 1, atom by atom
+    for i in (0, 17, 53):
+        ui, _ = oracle_mod.ann(p.w0, p.b0, p.w1, p.b1, q[i])
+        assert lat[i].sum() - float(p.b1[0]) == pytest.approx(ui, rel=1e-12, abs=1e-13)
+
+
+def test_heat_current_dimer_second_form_of_eq25(oracle_mod):
+    """J_0 = r_01 (dU_1/dr_10 . v_0), Eq. (25) second line, with dU_1/dr_10 = dU_1/dr_0 by central
+    differences of atom 1's own site energy -- no virial involved."""
+    cfg = W.get_config(2)
+    hyper, p = cfg.hyper, W.make_params(cfg, "stress")
+    pos = np.array([[0.0, 0.0, 0.0], [1.1, 1.7, -0.9]])
+    vel = np.array([[0.013, -0.004, 0.009], [-0.002, 0.011, 0.005]])
+    types = np.array([0, 1], dtype=np.int32)
+    box = np.array([40.0, 40.0, 40.0])
+    e, f, w = oracle_mod.compute(hyper, p, pos, types, box, pbc=(0, 0, 0))
+    ja, jt = oracle_mod.heat_current(w, vel)
+    h = 1e-5
+    dU = np.zeros((2, 3))          # dU[0] = dU_1/dr_0 = dU_1/dr_10 ; dU[1] = dU_0/dr_1 = dU_0/dr_01
+    for a in range(3):
+        for mover, owner in ((0, 1), (1, 0)):
+            pp, pm = pos.copy(), pos.copy()
+            pp[mover, a] += h; pm[mover, a] -= h
+            dU[mover, a] = (oracle_mod.compute(hyper, p, pp, types, box, pbc=(0, 0, 0))[0][owner]
+                            - oracle_mod.compute(hyper, p, pm, types, box, pbc=(0, 0, 0))[0][owner]) / (2 * h)
+    r01 = pos[1] - pos[0]
+    np.testing.assert_allclose(ja[0], r01 * np.dot(dU[0], vel[0]), rtol=1e-6, atol=1e-12)
+    np.testing.assert_allclose(ja[1], -r01 * np.dot(dU[1], vel[1]), rtol=1e-6, atol=1e-12)
+    np.testing.assert_allclose(jt, ja[0] + ja[1], rtol=1e-15)
+
+
+def test_heat_current_rigid_translation_is_strain_derivative(oracle_mod):
+    """v_i = v0 for all i: J = (sum_i W_i) v0, and sum_i W_i = -dE/d eps (reading A7), the latter by finite
+    differences of the total energy under the six strains of an open cluster."""
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    hyper, p = cfg.hyper, W.make_params(cfg, "stress")
+    pos, types = W.random_cluster(5, 14, hyper.n_types, 5.5, min_dist=1.5)
+    box = np.array([60.0, 60.0, 60.0])
+    e, f, w = oracle_mod.compute(hyper, p, pos, types, box, pbc=(0, 0, 0))
+    v0 = np.array([0.007, -0.012, 0.004])
+    ja, jt = oracle_mod.heat_current(w, np.tile(v0, (len(pos), 1)))
+    h = 1e-5
+    dE = np.zeros((3, 3))
+    for a in range(3):
+        for b in range(3):
+            eps = np.zeros((3, 3)); eps[a, b] = h
+            Ep = oracle_mod.compute(hyper, p, pos @ (np.eye(3) + eps).T, types, box, pbc=(0, 0, 0))[0].sum()
+            Em = oracle_mod.compute(hyper, p, pos @ (np.eye(3) - eps).T, types, box, pbc=(0, 0, 0))[0].sum()
+            dE[a, b] = (Ep - Em) / (2 * h)
+    np.testing.assert_allclose(jt, -dE @ v0, rtol=2e-5, atol=1e-10)
+
+
+def test_heat_current_linear_and_order_independent(oracle_mod):
+    rng = np.random.default_rng(7)
+    w = rng.normal(size=(23, 9)); v1 = rng.normal(size=(23, 3)); v2 = rng.normal(size=(23, 3))
+    j1, t1 = oracle_mod.heat_current(w, v1)
+    j2, t2 = oracle_mod.heat_current(w, v2)
+    j3, t3 = oracle_mod.heat_current(w, 2.0 * v1 - 3.0 * v2)
+    np.testing.assert_allclose(j3, 2.0 * j1 - 3.0 * j2, rtol=1e-12, atol=1e-12)
+    perm = rng.permutation(23)
+    jp, tp = oracle_mod.heat_current(w[perm], v1[perm])
+    np.testing.assert_allclose(jp, j1[perm], rtol=0, atol=0)
+    np.testing.assert_allclose(tp, t1, rtol=1e-12, atol=1e-12)
+    # a transposed virial must NOT give the same current (guards the W[3a+b] layout)
+    jt_, _ = oracle_mod.heat_current(w.reshape(-1, 3, 3).transpose(0, 2, 1).reshape(-1, 9), v1)
+    assert np.abs(jt_ - j1).max() > 1e-3
