@@ -146,11 +146,27 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
                 const double box[9], double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin,
                 double* energy_host, double* force_host, double* virial_host);
 
-/* ---- test hooks (internals of the last evaluation, caller's atom order) ---------------------------
- * q_dev [n][D] descriptor, fp_dev [n][D] dU_i/dq_v, S_dev [n][NA][24] sums of Eq. (12).
- * fp32; any pointer may be NULL.  Do not synchronise.                                                 */
+/* ---- descriptor / latent-vector export and test hooks (last evaluation, caller's atom order) -------
+ * nep_get_descriptors: q_dev [n][D] descriptor vector q_i^v of Eq. (1) in the order of DESIGN.md reading
+ *   A2 (what PYNEP's 'descriptor' property returns), fp_dev [n][D] dU_i/dq_v
+ *   (PAPER.md:901).  nep_get_angular_sums: S_dev [n][NA][24] sums of Eq. (12) (test hook).
+ * nep_get_latent: latent_dev [n][H], the latent-space vector of PAPER.md:484 -- component mu is the state
+ *   of hidden neuron mu times its weight to the output layer, w1_mu tanh(sum_v w0_mu,v q_v - b0_mu), so
+ *   that sum_mu latent[i][mu] - b1 = U_i.
+ * All fp32 device buffers owned by the caller; any pointer of the first two calls may be NULL.
+ * NEP_ERR_STATE before the first evaluation.  Do not synchronise.                                     */
 int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev);
 int nep_get_angular_sums(nep_t* nep, float* S_dev);
+int nep_get_latent(nep_t* nep, float* latent_dev);
+
+/* ---- heat current, Eqs. (25)-(26) ------------------------------------------------
+ * J_i = W_i . v_i with the per-atom virial W_i of the last evaluation (Eq. (24), layout W[3a+b]):
+ * j_atom_dev [n][3] gets J_i^a = sum_b W_i^{ab} v_i^b, j_total_dev [3] gets J = sum_i J_i (reduced in a
+ * fixed order: bitwise reproducible).  vel_dev [n][3] Angstrom/fs in the caller's atom order, which must be
+ * the velocities that belong to the evaluated positions (after md_step: the vel_dev it was given).
+ * fp64 device buffers owned by the caller; either output may be NULL, not both.  Units eV Angstrom / fs.
+ * NEP_ERR_STATE before the first evaluation.  Does not synchronise.                                    */
+int nep_heat_current(nep_t* nep, const double* vel_dev, double* j_atom_dev, double* j_total_dev);
 
 /* ---- measurement support (bench.py) ---------------------------------------------------------------
  * nep_launch_count: kernel launches the handle has enqueued so far (bench.py's gpu_launches).

@@ -19,7 +19,8 @@ _lib = None
 exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
-    "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums",
+    "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
+    "nep_heat_current",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
@@ -90,6 +91,10 @@ def load_library():
     L.nep_get_descriptors.argtypes = [vp, vp, vp]
     L.nep_get_angular_sums.restype = C.c_int
     L.nep_get_angular_sums.argtypes = [vp, vp]
+    L.nep_get_latent.restype = C.c_int
+    L.nep_get_latent.argtypes = [vp, vp]
+    L.nep_heat_current.restype = C.c_int
+    L.nep_heat_current.argtypes = [vp, vp, vp, vp]
     L.nep_launch_count.restype = i64
     L.nep_launch_count.argtypes = [vp]
     L.nep_pair_counts.restype = C.c_int
@@ -257,6 +262,23 @@ class NEP:
         S = torch.empty((self.n, self.hyper.n_max_angular + 1, 24), dtype=torch.float32, device=f"cuda:{self.device}")
         self._check(self._L.nep_get_angular_sums(self._h_ptr, C.c_void_p(S.data_ptr())))
         return S
+
+    def nep_get_latent(self):
+        """[n][H] latent-space vectors of the last evaluation."""
+        torch = self._torch
+        lat = torch.empty((self.n, self.hyper.n_neurons), dtype=torch.float32, device=f"cuda:{self.device}")
+        self._check(self._L.nep_get_latent(self._h_ptr, C.c_void_p(lat.data_ptr())))
+        return lat
+
+    def nep_heat_current(self, vel):
+        """(J_atom [n][3], J_total [3]) of Eqs. (25)-(26) from the last evaluation's virial and `vel`."""
+        torch = self._torch
+        n, dev = self.n, f"cuda:{self.device}"
+        ja = torch.empty((n, 3), dtype=torch.float64, device=dev)
+        jt = torch.empty(3, dtype=torch.float64, device=dev)
+        self._check(self._L.nep_heat_current(self._h_ptr, self._dev(vel, torch.float64, 3 * n),
+                                             C.c_void_p(ja.data_ptr()), C.c_void_p(jt.data_ptr())))
+        return ja, jt
 
     def nep_launch_count(self) -> int:
         return int(self._L.nep_launch_count(self._h_ptr))

@@ -527,6 +527,16 @@ int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
     return NEP_OK;
 }
 
+template <int DP>
+int launch_latent(nep_t* nep, float* latent_dev)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H);
+    NEP_TRY(allow_smem(nep, k_latent<DP>, sm));
+    NEP_LAUNCH(NEP_K_EXPORT, k_latent<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->perm, nep->q, nep->w0p, nep->b0, nep->w1, latent_dev));
+    return NEP_OK;
+}
+
 }  // namespace
 
 // =======================================================================================================
@@ -812,6 +822,44 @@ int nep_get_angular_sums(nep_t* nep, float* S_dev)
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
     if (S_dev) { NEP_LAUNCH(NEP_K_EXPORT, k_export_rows<<<div_up(n, 128), 128, 0, nep->stream>>>(n, nep->d.NA * NEP_NUM_S, nep->perm, nep->S, S_dev)); }
+    return NEP_OK;
+}
+
+// ---- derived outputs ----------------------------------------------------
+int nep_get_latent(nep_t* nep, float* latent_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!latent_dev) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    switch (nep->DP) {
+        case 24: return launch_latent<24>(nep, latent_dev);
+        case 40: return launch_latent<40>(nep, latent_dev);
+        case 56: return launch_latent<56>(nep, latent_dev);
+        case 72: return launch_latent<72>(nep, latent_dev);
+        case 88: return launch_latent<88>(nep, latent_dev);
+        case 104: return launch_latent<104>(nep, latent_dev);
+        case 120: return launch_latent<120>(nep, latent_dev);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "descriptor too long");
+}
+
+int nep_heat_current(nep_t* nep, const double* vel_dev, double* j_atom_dev, double* j_total_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!vel_dev || (!j_atom_dev && !j_total_dev)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    const int nb = div_up(n, 256);
+    if (nb > nep->heat_cap) {
+        nep->heat_cap = 0;
+        NEP_TRY(dev_alloc(nep, &nep->heat_partial, 3 * (size_t)nb + 3));
+        nep->heat_cap = nb;
+    }
+    NEP_LAUNCH(NEP_K_EXPORT, k_heat_current<<<nb, 256, 0, nep->stream>>>(n, nep->w_out, vel_dev, j_atom_dev, nep->heat_partial));
+    double* tot = j_total_dev ? j_total_dev : nep->heat_partial + 3 * (size_t)nb;
+    NEP_LAUNCH(NEP_K_EXPORT, k_heat_total<<<1, 256, 0, nep->stream>>>(nb, nep->heat_partial, tot));
     return NEP_OK;
 }
 

@@ -129,6 +129,9 @@ struct nep_ctx {
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]
 
+    double* heat_partial;    // [3 * blocks + 3] block partials of the total heat current (nep_heat_current)
+    int heat_cap;
+
     // staging of the host-buffer entry points (device copies of the caller's host arrays)
     double* h_pos; double* h_vel; int* h_type;
     int64_t h_cap;

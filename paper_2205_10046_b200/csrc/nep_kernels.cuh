@@ -1078,6 +1078,96 @@ __global__ void k_export_rows(int n, int ncomp, const int* __restrict__ perm, co
 }
 
 // ---------------------------------------------------------------------------------------------------
+// latent-space vector of every atom,
+//   latent[i][mu] = w1_mu tanh(sum_v w0_mu,v q_v - b0_mu)      (hidden-layer state of Eq. (1) times w1)
+// from the descriptors of the last evaluation; output [n][H] fp32 in the caller's atom order.  One thread
+// per atom with q in registers, weights staged in shared memory (warp-uniform reads), as in k_ann.
+template <int DP>
+__global__ void __launch_bounds__(128)
+k_latent(NepDims D, const int* __restrict__ perm, const float* __restrict__ q, const float* __restrict__ w0p,
+         const float* __restrict__ b0, const float* __restrict__ w1, float* __restrict__ out)
+{
+    extern __shared__ float sw[];                       // w0p [H][DP], b0 [H], w1 [H]
+    for (int t = threadIdx.x; t < D.H * DP; t += blockDim.x) sw[t] = w0p[t];
+    float* sb0 = sw + D.H * DP;
+    float* sw1 = sb0 + D.H;
+    for (int t = threadIdx.x; t < D.H; t += blockDim.x) { sb0[t] = b0[t]; sw1[t] = w1[t]; }
+    __syncthreads();
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= D.n) return;
+    const size_t n = (size_t)D.n;
+    float qv[DP];
+#pragma unroll
+    for (int d = 0; d < DP; ++d) qv[d] = (d < D.D) ? q[(size_t)d * n + s] : 0.0f;
+    float* row = out + (size_t)perm[s] * D.H;
+    for (int m = 0; m < D.H; ++m) {
+        const float4* w = reinterpret_cast<const float4*>(sw + m * DP);
+        float a0 = -sb0[m], a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+#pragma unroll
+        for (int d4 = 0; d4 < DP / 4; ++d4) {
+            const float4 ww = w[d4];
+            a0 = fmaf(ww.x, qv[4 * d4 + 0], a0); a1 = fmaf(ww.y, qv[4 * d4 + 1], a1);
+            a2 = fmaf(ww.z, qv[4 * d4 + 2], a2); a3 = fmaf(ww.w, qv[4 * d4 + 3], a3);
+        }
+        row[m] = sw1[m] * tanhf((a0 + a1) + (a2 + a3));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// per-atom heat current J_i = W_i . v_i, Eq. (25), and the total J = sum_i J_i,
+// Eq. (26), from the per-atom virial of the last evaluation (W[3a+b], caller's order,
+// fp64) and the caller's velocities: J_i^a = sum_b W_i^{ab} v_i^b.  The total is reduced in a fixed
+// order (block partials, then one block), so it is reproducible run to run.
+__global__ void __launch_bounds__(256)
+k_heat_current(int n, const double* __restrict__ w, const double* __restrict__ vel, double* __restrict__ j_atom,
+               double* __restrict__ partial)
+{
+    __shared__ double sh[3][256];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double j[3] = {0.0, 0.0, 0.0};
+    if (i < n) {
+        const double* W = w + 9 * (size_t)i;
+        const double vx = vel[3 * (size_t)i + 0], vy = vel[3 * (size_t)i + 1], vz = vel[3 * (size_t)i + 2];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) j[a] = W[3 * a + 0] * vx + W[3 * a + 1] * vy + W[3 * a + 2] * vz;
+        if (j_atom) { j_atom[3 * (size_t)i + 0] = j[0]; j_atom[3 * (size_t)i + 1] = j[1]; j_atom[3 * (size_t)i + 2] = j[2]; }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] = j[a];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) partial[3 * (size_t)blockIdx.x + threadIdx.x] = sh[threadIdx.x][0];
+}
+
+__global__ void __launch_bounds__(256)
+k_heat_total(int nblocks, const double* __restrict__ partial, double* __restrict__ j_total)
+{
+    __shared__ double sh[3][256];
+    double j[3] = {0.0, 0.0, 0.0};
+    for (int b = threadIdx.x; b < nblocks; b += 256) {     // fixed assignment of partials to threads
+#pragma unroll
+        for (int a = 0; a < 3; ++a) j[a] += partial[3 * (size_t)b + a];
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] = j[a];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) j_total[threadIdx.x] = sh[threadIdx.x][0];
+}
+
+// ---------------------------------------------------------------------------------------------------
 // (a9) velocity-Verlet pieces, caller's atom order, fp64 state.
 __global__ void k_kick_drift(int n, double half_dt_conv, double dt, const int* __restrict__ type,
                              const double* __restrict__ mass, const double* __restrict__ f,

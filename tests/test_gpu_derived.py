@@ -1,0 +1,113 @@
+"""GPU-vs-oracle parity of the derived outputs, through the C ABI (-m gpu):
+the latent-space vector (nep_get_latent) and the heat current (Eqs. 25-26, nep_heat_current).
+
+Tolerances, derived from the arithmetic: a latent component is w1_mu tanh(a) with a an fp32 dot product of
+D terms, so |d latent| <= |w1_mu| (|da| + eps) with |da| ~ D eps max|w0 q|: asserted as 2e-5 of the largest
+|latent| component (the same block-relative bar the descriptors use).  The heat current is a contraction
+of the fp32-accumulated virial (parity bar 1e-4 relative, reading A14) with fp64 velocities in fp64:
+per atom ||dJ_i|| <= 1e-4 max(||W_i||, median ||W||) ||v_i||; the contraction itself must be exact fp64 on
+the GPU's own virial (1e-14), the total equal to the fp64 sum of the GPU's J_i (1e-12), and within
+1e-4 (sum_i ||J_i|| / sqrt(n) + ||J||) of the oracle's total (independent per-atom errors add in quadrature).
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2205_10046_b200 as p
+    p.load_library()
+    return p
+
+
+CASES = [(0, None, 0.0), (2, (4, 4, 3), 1.0), (3, (7, 6, 5), 1.0), (4, (9, 8, 7), 1.0)]
+
+
+@pytest.mark.parametrize("kind", ["baseline", "stress"])
+@pytest.mark.parametrize("idx,cells,skin", CASES)
+def test_latent_vector(pkg, oracle_mod, idx, cells, skin, kind):
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s, p = W.make_system(cfg), W.make_params(cfg, kind)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    e, f, w = nep.nep_compute(pos)
+    lat = nep.nep_get_latent().cpu().numpy().astype(np.float64)
+    eo, fo, wo, qo, fpo, So = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box, want_internals=True)
+    lo = oracle_mod.latent(p, qo)
+    assert lat.shape == lo.shape == (len(s.pos), cfg.hyper.n_neurons)
+    assert np.abs(lat - lo).max() <= 2e-5 * np.abs(lo).max()
+    # the defining property, on the GPU's own numbers: sum_mu latent - b1 = U_i
+    assert np.abs(lat.sum(axis=1) - float(p.b1[0]) - e.cpu().numpy()).max() <= 1e-5
+    nep.close()
+
+
+@pytest.mark.parametrize("kind", ["baseline", "stress"])
+@pytest.mark.parametrize("idx,cells,skin", CASES)
+def test_heat_current(pkg, oracle_mod, idx, cells, skin, kind):
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s, p = W.make_system(cfg), W.make_params(cfg, kind)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    e, f, w = nep.nep_compute(pos)
+    ja, jt = nep.nep_heat_current(vel)
+    ja, jt, wg = ja.cpu().numpy(), jt.cpu().numpy(), w.cpu().numpy()
+    eo, fo, wo = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box)
+    jo, jto = oracle_mod.heat_current(wo, s.vel)
+    wn = np.linalg.norm(wo, axis=1)
+    vn = np.linalg.norm(s.vel, axis=1)
+    bound = 1e-4 * np.maximum(wn, np.median(wn)) * vn
+    assert (np.linalg.norm(ja - jo, axis=1) <= bound + 1e-18).all()
+    # the contraction itself is exact fp64 on the GPU's own virial (same summation order as Eq. 25 written out)
+    jself, _ = oracle_mod.heat_current(wg, s.vel)
+    assert np.abs(ja - jself).max() <= 1e-14 * max(np.abs(jself).max(), 1e-300)
+    # total: fixed-order fp64 reduction of the GPU's J_i; against the oracle within the virial bar
+    assert np.abs(jt - ja.sum(axis=0)).max() <= 1e-12 * np.abs(ja).sum()
+    assert np.linalg.norm(jt - jto) <= 1e-4 * np.linalg.norm(jo, axis=1).sum() / np.sqrt(len(jo)) + 1e-4 * np.linalg.norm(jto)
+    nep.close()
+
+
+def test_heat_current_after_md_and_reproducible(pkg, oracle_mod):
+    """After md_step the virial belongs to the final positions and vel_dev holds the matching velocities;
+    two calls give bitwise identical totals (fixed reduction order)."""
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 1.0)
+    nep.md_step(pos, vel, cfg.dt_fs, 5, cfg.rebuild_every, 1.0)
+    ja1, jt1 = nep.nep_heat_current(vel)
+    ja2, jt2 = nep.nep_heat_current(vel)
+    assert torch.equal(jt1, jt2) and torch.equal(ja1, ja2)
+    eo, fo, wo = oracle_mod.compute(cfg.hyper, p, pos.cpu().numpy(), s.types, s.box)
+    jo, jto = oracle_mod.heat_current(wo, vel.cpu().numpy())
+    wn = np.linalg.norm(wo, axis=1)
+    bound = 1e-4 * np.maximum(wn, np.median(wn)) * np.linalg.norm(vel.cpu().numpy(), axis=1)
+    assert (np.linalg.norm(ja1.cpu().numpy() - jo, axis=1) <= bound + 1e-18).all()
+    nep.close()
+
+
+def test_derived_outputs_need_an_evaluation(pkg):
+    cfg = W.get_config(0)
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 0.0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_get_latent()
+    assert ei.value.status == -5
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_heat_current(torch.tensor(s.vel, device="cuda:0"))
+    assert ei.value.status == -5
+    nep.close()
