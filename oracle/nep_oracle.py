@@ -248,3 +248,38 @@ def heat_current(virial, vel):
         for a in range(3):
             ja[i, a] = W[i, 3 * a + 0] * v[i, 0] + W[i, 3 * a + 1] * v[i, 1] + W[i, 3 * a + 2] * v[i, 2]
     return ja, ja.sum(axis=0)
+
+
+# ---- a second ensemble (NVT, Berendsen thermostat) ------------------------
+# Unit constants of DESIGN.md reading A10 (CODATA; pinned against scipy.constants in tests/test_oracle_derived.py)
+ACC_CONV = 9.648533212e-3      # (eV/Angstrom/amu) -> Angstrom/fs^2
+KB_EV_PER_K = 8.617333262e-5
+
+
+def kinetic_temperature(vel, masses_per_atom) -> float:
+    """T = sum_i m_i v_i^2 / (3 N k_B) with 3N degrees of freedom (readings A10, A15)."""
+    v, m = _d(vel), _d(masses_per_atom)
+    return float((m[:, None] * v * v).sum() / ACC_CONV / (3.0 * len(m) * KB_EV_PER_K))
+
+
+def md_berendsen(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int,
+                 t_start: float, t_stop: float, tau_fs: float, pbc=(1, 1, 1)):
+    """NVT with the Berendsen thermostat (named PAPER.md:318, `nvt_ber` PAPER.md:602; Berendsen et al.,
+    ref. 75 PAPER.md:1220; the paper prints no equation: DESIGN.md reading A15).  Each step is one
+    velocity-Verlet step of md() above (kick-drift-kick, forces at the new positions), after which all
+    velocities are scaled by  lambda = sqrt(1 + (dt / tau) (T_target / T - 1)),  T the kinetic temperature
+    of the just-updated velocities; T_target of step s = 1..n_steps is t_start + (t_stop - t_start) s / n_steps.
+    Returns (pos, vel, T_before[n_steps], T_after[n_steps]) -- temperatures before / after each rescale."""
+    pos, vel = _d(pos).copy(), _d(vel).copy()
+    m_atom = _d(masses)[np.ascontiguousarray(types, dtype=np.int32)]
+    t_before = np.zeros(n_steps)
+    t_after = np.zeros(n_steps)
+    for s in range(1, n_steps + 1):
+        pos, vel, _, _ = md(hyper, params, pos, vel, types, masses, box, dt_fs, 1, pbc=pbc)
+        T = kinetic_temperature(vel, m_atom)
+        t_target = t_start + (t_stop - t_start) * s / n_steps
+        lam = np.sqrt(1.0 + (dt_fs / tau_fs) * (t_target / T - 1.0)) if T > 0.0 else 1.0
+        vel = vel * lam
+        t_before[s - 1] = T
+        t_after[s - 1] = kinetic_temperature(vel, m_atom)
+    return pos, vel, t_before, t_after

@@ -98,3 +98,60 @@ def test_heat_current_linear_and_order_independent(oracle_mod):
     # a transposed virial must NOT give the same current (guards the W[3a+b] layout)
     jt_, _ = oracle_mod.heat_current(w.reshape(-1, 3, 3).transpose(0, 2, 1).reshape(-1, 9), v1)
     assert np.abs(jt_ - j1).max() > 1e-3
+
+
+# ------------------------------------------------------------------ Berendsen NVT (reading A15)
+def test_oracle_unit_constants_from_codata(oracle_mod):
+    from scipy import constants as sc
+    conv = sc.e / sc.physical_constants["atomic mass constant"][0] * 1e-10
+    assert oracle_mod.ACC_CONV == pytest.approx(conv, rel=2e-9)
+    assert oracle_mod.KB_EV_PER_K == pytest.approx(sc.k / sc.e, rel=1e-9)
+    cfg = W.get_config(0)
+    s = W.make_system(cfg)        # workloads draws exactly cfg.temperature with its own constants
+    assert oracle_mod.kinetic_temperature(s.vel, s.masses[s.types]) == pytest.approx(cfg.temperature, rel=5e-9)
+
+
+def _zero_model(cfg):
+    """all parameters zero: U_i = 0, no forces -- free particles"""
+    p = W.make_params(cfg)
+    for name in ("c_radial", "c_angular", "w0", "b0", "w1", "b1"):
+        getattr(p, name)[...] = 0.0
+    return p
+
+
+def test_berendsen_free_particles_closed_form(oracle_mod):
+    """No forces: velocity-Verlet leaves T unchanged, so T_{k+1} = T_k + (dt/tau)(T0 - T_k) exactly, i.e.
+    T_k = T0 + (T_init - T0) (1 - dt/tau)^k; positions advance with the velocity of each step."""
+    cfg = W.get_config(0)
+    s, p = W.make_system(cfg), _zero_model(cfg)
+    dt, tau, T0, n = 2.0, 50.0, 450.0, 12
+    pos, vel, tb, ta = oracle_mod.md_berendsen(cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box, dt, n, T0, T0, tau)
+    k = np.arange(1, n + 1)
+    np.testing.assert_allclose(ta, T0 + (cfg.temperature - T0) * (1.0 - dt / tau) ** k, rtol=1e-12)
+    np.testing.assert_allclose(tb[1:], ta[:-1], rtol=1e-13)
+    lam = np.sqrt(np.concatenate([[cfg.temperature], ta[:-1]]) ** -1 * ta)          # per-step scale factors
+    scale_before = np.concatenate([[1.0], np.cumprod(lam)[:-1]])                  # velocity used in step k's drift
+    np.testing.assert_allclose(pos, s.pos + dt * s.vel * scale_before.sum(), rtol=0, atol=1e-11)
+    np.testing.assert_allclose(vel, s.vel * np.prod(lam), rtol=1e-13, atol=0)
+
+
+def test_berendsen_limits_and_one_step_identity(oracle_mod):
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    args = (cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box)
+    m_atom = s.masses[s.types]
+    # tau -> infinity: the NVE trajectory of the pinned integrator
+    pos_n, vel_n, _, _ = oracle_mod.md(*args, 1.0, 6)
+    pos_b, vel_b, tb, ta = oracle_mod.md_berendsen(*args, 1.0, 6, 900.0, 900.0, 1e30)
+    np.testing.assert_allclose(pos_b, pos_n, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(vel_b, vel_n, rtol=0, atol=1e-14)
+    # one step: T_after - T_before = (dt/tau)(T_target - T_before), T_before from the NVE step alone
+    pos1, vel1, _, _ = oracle_mod.md(*args, 1.0, 1)
+    t_nve = oracle_mod.kinetic_temperature(vel1, m_atom)
+    _, vel_b1, tb1, ta1 = oracle_mod.md_berendsen(*args, 1.0, 1, 100.0, 900.0, 20.0)     # target of step 1 of 1 = t_stop
+    assert tb1[0] == pytest.approx(t_nve, rel=1e-13)
+    assert ta1[0] - tb1[0] == pytest.approx((1.0 / 20.0) * (900.0 - t_nve), rel=1e-10)
+    np.testing.assert_allclose(vel_b1 / vel1, np.sqrt(ta1[0] / tb1[0]), rtol=1e-12)     # a pure rescale
+    # tau = dt: the target is hit exactly; the ramp is linear in the step number
+    _, _, tb2, ta2 = oracle_mod.md_berendsen(*args, 1.0, 4, 300.0, 700.0, 1.0)
+    np.testing.assert_allclose(ta2, [400.0, 500.0, 600.0, 700.0], rtol=1e-12)
