@@ -120,6 +120,17 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
 int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs,
             int32_t n_steps, int32_t rebuild_every, double skin);
 
+/* ---- NVT: velocity-Verlet + Berendsen thermostat (named PAPER.md:318, `nvt_ber` PAPER.md:602, ref. 75;
+ * equation per DESIGN.md reading A15).  As md_step, and after the second half kick of every step all
+ * velocities are scaled by lambda = sqrt(1 + (dt_fs / tau_fs) (T_target / T - 1)), T = sum m v^2 / (3 n k_B),
+ * T_target of step s = 1..n_steps = t_start_K + (t_stop_K - t_start_K) s / n_steps.  The kinetic-energy sum
+ * is reduced on the device in a fixed order; no host round trip.  NEP_ERR_INVALID_ARG if tau_fs <= 0 or a
+ * temperature < 0.  nep_last_temperature: T before the rescale and lambda of the last thermostatted step
+ * (host scalars; synchronises; NEP_ERR_STATE if there was none).                                        */
+int md_step_nvt_berendsen(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps,
+                          int32_t rebuild_every, double skin, double t_start_K, double t_stop_K, double tau_fs);
+int nep_last_temperature(nep_t* nep, double* t_before_host, double* lambda_host);
+
 /* Results of the most recent internal evaluation (the one md_step ended with, or nep_compute):
  * same layouts as nep_compute; any pointer may be NULL.  Does not synchronise.                        */
 int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* virial_dev);

@@ -14,6 +14,7 @@
 namespace {
 
 const double kAccConv = 9.648533212e-3;   // (eV/Angstrom/amu) -> Angstrom/fs^2 (reading A10)
+const double kBoltzmann = 8.617333262e-5; // eV/K (reading A10)
 
 struct HostCoef { NepCoef c; };
 
@@ -759,11 +760,20 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
     return nep_get_last(nep, energy_dev, force_dev, virial_dev);
 }
 
-int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin)
+// thermostat of md_loop: none (NVE) or Berendsen (reading A15)
+struct Thermostat {
+    bool on;
+    double t_start, t_stop, tau_fs;
+};
+
+static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
+                   double skin, const Thermostat& th)
 {
     if (!nep) return NEP_ERR_INVALID_ARG;
     if (!pos_dev || !vel_dev || n_steps < 0 || rebuild_every < 1 || !(skin >= 0.0) || !(dt_fs == dt_fs))
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad md_step argument");
+    if (th.on && (!(th.tau_fs > 0.0) || !(th.t_start >= 0.0) || !(th.t_stop >= 0.0)))
+        return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad thermostat argument");
     if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
@@ -778,15 +788,55 @@ int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t 
     if (!nep->force_current || nep->force_pos_tag != pos_dev) NEP_TRY(evaluate(nep, pos_dev));
     const double hdt = 0.5 * dt_fs * kAccConv;
     const int TB = 256;
+    const int nb = div_up(n, 256);
+    if (th.on && nb + 2 > nep->thermo_cap) {
+        nep->thermo_cap = 0;
+        NEP_TRY(dev_alloc(nep, &nep->thermo, (size_t)nb + 2));
+        nep->thermo_cap = nb + 2;
+    }
     for (int s = 0; s < n_steps; ++s) {
         NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
         NEP_TRY(evaluate(nep, pos_dev));
         NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
+        if (th.on) {
+            const double t_target = th.t_start + (th.t_stop - th.t_start) * (double)(s + 1) / (double)n_steps;
+            double* lam = nep->thermo + (nep->thermo_cap - 2);
+            NEP_LAUNCH(NEP_K_THERMOSTAT, k_mv2_partial<<<nb, 256, 0, st>>>(n, nep->type_orig, nep->mass_dev, vel_dev, nep->thermo));
+            NEP_LAUNCH(NEP_K_THERMOSTAT, k_berendsen_lambda<<<1, 256, 0, st>>>(nb, nep->thermo, 1.0 / (kAccConv * 3.0 * (double)n * kBoltzmann),
+                                                                              dt_fs / th.tau_fs, t_target, lam));
+            NEP_LAUNCH(NEP_K_THERMOSTAT, k_scale_velocities<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(3 * n, lam, vel_dev));
+        }
     }
     nep->force_current = true;
     nep->force_pos_tag = pos_dev;
+    return NEP_OK;
+}
+
+int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin)
+{
+    const Thermostat none = {false, 0.0, 0.0, 0.0};
+    return md_loop(nep, pos_dev, vel_dev, dt_fs, n_steps, rebuild_every, skin, none);
+}
+
+int md_step_nvt_berendsen(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
+                          double skin, double t_start_K, double t_stop_K, double tau_fs)
+{
+    const Thermostat th = {true, t_start_K, t_stop_K, tau_fs};
+    return md_loop(nep, pos_dev, vel_dev, dt_fs, n_steps, rebuild_every, skin, th);
+}
+
+int nep_last_temperature(nep_t* nep, double* t_before_host, double* lambda_host)
+{
+    if (!nep || (!t_before_host && !lambda_host)) return NEP_ERR_INVALID_ARG;
+    if (!nep->thermo || nep->thermo_cap < 2) return nep_fail(nep, NEP_ERR_STATE, "no thermostatted step yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    double v[2];
+    NEP_CUDA(cudaMemcpyAsync(v, nep->thermo + (nep->thermo_cap - 2), sizeof(v), cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    if (lambda_host) *lambda_host = v[0];
+    if (t_before_host) *t_before_host = v[1];
     return NEP_OK;
 }
 
@@ -933,7 +983,7 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 // ---- measurement support ----------------------------------------------------------------------------------
 static const char* const kKernelNames[NEP_K_COUNT] = {
     "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
-    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "export"};
+    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
 

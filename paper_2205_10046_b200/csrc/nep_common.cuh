@@ -19,7 +19,7 @@
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
     NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FORCE_RADIAL, NEP_K_FINAL,
-    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_EXPORT, NEP_K_COUNT
+    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
 
@@ -129,6 +129,8 @@ struct nep_ctx {
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]
 
+    double* thermo;          // [blocks] partials of sum m v^2, then {lambda, T before the rescale} of the last step
+    int thermo_cap;
     double* heat_partial;    // [3 * blocks + 3] block partials of the total heat current (nep_heat_current)
     int heat_cap;
 

@@ -1188,3 +1188,55 @@ __global__ void k_kick(int n, double half_dt_conv, const int* __restrict__ type,
     if (t >= 3 * n) return;
     vel[t] += half_dt_conv * (f[t] / mass[type[t / 3]]);
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Berendsen thermostat (reading A15), applied after the second half
+// kick: sum_i m_i v_i^2 by block partials and one final block (fixed order: reproducible), then
+// v *= lambda, lambda = sqrt(1 + (dt/tau) (T_target / T - 1)), T = sum m v^2 / (conv 3 N k_B); all on the
+// device, no host round trip.
+__global__ void __launch_bounds__(256)
+k_mv2_partial(int n, const int* __restrict__ type, const double* __restrict__ mass, const double* __restrict__ vel,
+              double* __restrict__ partial)
+{
+    __shared__ double sh[256];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double a = 0.0;
+    if (i < n) {
+        const double vx = vel[3 * (size_t)i + 0], vy = vel[3 * (size_t)i + 1], vz = vel[3 * (size_t)i + 2];
+        a = mass[type[i]] * (vx * vx + vy * vy + vz * vz);
+    }
+    sh[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+// one block: total of the partials -> scale factor lambda in out[0], temperature before the rescale in out[1]
+__global__ void __launch_bounds__(256)
+k_berendsen_lambda(int nblocks, const double* __restrict__ partial, double inv_conv_3nkb, double dt_over_tau,
+                   double t_target, double* __restrict__ out)
+{
+    __shared__ double sh[256];
+    double a = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 256) a += partial[b];
+    sh[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double T = sh[0] * inv_conv_3nkb;
+        out[0] = T > 0.0 ? sqrt(1.0 + dt_over_tau * (t_target / T - 1.0)) : 1.0;
+        out[1] = T;
+    }
+}
+
+__global__ void k_scale_velocities(int n3, const double* __restrict__ lambda, double* __restrict__ vel)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n3) vel[t] *= lambda[0];
+}

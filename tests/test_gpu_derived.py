@@ -111,3 +111,51 @@ def test_derived_outputs_need_an_evaluation(pkg):
         nep.nep_heat_current(torch.tensor(s.vel, device="cuda:0"))
     assert ei.value.status == -5
     nep.close()
+
+
+# ------------------------------------------------------------------ Berendsen NVT
+@pytest.mark.parametrize("idx,cells,skin,kind", [(0, None, 0.0, "baseline"), (3, (7, 6, 5), 1.0, "stress"), (2, (4, 4, 3), 1.0, "stress")])
+def test_berendsen_nvt_trajectory(pkg, oracle_mod, idx, cells, skin, kind):
+    """10 thermostatted steps with a temperature ramp against the oracle's md_berendsen: fp64 state, fp32 forces.
+    Tolerances as the NVE trajectory test (1e-7 A, 1e-9 A/fs) scaled by the stress set's stronger forces; the
+    temperature before the last rescale and its lambda to 1e-9 relative (a fixed-order fp64 reduction)."""
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s, p = W.make_system(cfg), W.make_params(cfg, kind)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    n_steps, t0, t1, tau = 10, 500.0, 800.0, 25.0
+    nep.md_step_nvt_berendsen(pos, vel, cfg.dt_fs, n_steps, cfg.rebuild_every, skin, t0, t1, tau)
+    po, vo, tb, ta = oracle_mod.md_berendsen(cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box, cfg.dt_fs, n_steps, t0, t1, tau)
+    tol = 1.0 if kind == "baseline" else 30.0
+    assert np.abs(pos.cpu().numpy() - po).max() < 1e-7 * tol
+    assert np.abs(vel.cpu().numpy() - vo).max() < 1e-9 * tol
+    t_last, lam = nep.nep_last_temperature()
+    assert t_last == pytest.approx(tb[-1], rel=1e-7)
+    assert lam == pytest.approx(np.sqrt(ta[-1] / tb[-1]), rel=1e-8)
+    m = s.masses[s.types]
+    assert oracle_mod.kinetic_temperature(vel.cpu().numpy(), m) == pytest.approx(ta[-1], rel=1e-7)
+    nep.close()
+
+
+def test_berendsen_nvt_reaches_target_and_rejects_bad_arguments(pkg, oracle_mod):
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 1.0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_last_temperature()
+    assert ei.value.status == -5
+    for bad in ((300.0, 300.0, 0.0), (-1.0, 300.0, 10.0), (300.0, -5.0, 10.0)):
+        with pytest.raises(pkg.NepError) as ei:
+            nep.md_step_nvt_berendsen(pos, vel, 1.0, 1, 10, 1.0, *bad)
+        assert ei.value.status == -1
+    # tau = dt: every step lands exactly on its target; 150 steps with tau = 20 fs hold 600 K within 10 % (the random model keeps exchanging kinetic and potential energy)
+    nep.md_step_nvt_berendsen(pos, vel, 1.0, 3, 10, 1.0, 600.0, 600.0, 1.0)
+    m = s.masses[s.types]
+    assert oracle_mod.kinetic_temperature(vel.cpu().numpy(), m) == pytest.approx(600.0, rel=1e-10)
+    nep.md_step_nvt_berendsen(pos, vel, 1.0, 150, 10, 1.0, 600.0, 600.0, 20.0)
+    assert abs(oracle_mod.kinetic_temperature(vel.cpu().numpy(), m) - 600.0) < 60.0
+    assert nep.nep_max_displacement() < 0.5
+    nep.close()
