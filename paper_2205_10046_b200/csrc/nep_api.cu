@@ -114,6 +114,9 @@ int allow_smem(nep_t* nep, K kernel, size_t bytes)
 // ---- allocation ----------------------------------------------------------------------------------------
 int alloc_lists(nep_t* nep, int capA, int capS)
 {
+    capA = (capA + 7) & ~7; capS = (capS + 7) & ~7;     // rows of the atom-major copy: whole 32-byte sectors
+    if (capA > 256) capA = 256;
+    if (capS > 256) capS = 256;
     const size_t n = (size_t)nep->n;
     NEP_TRY(dev_alloc(nep, &nep->listA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->rev, (size_t)capA * n));
@@ -121,6 +124,7 @@ int alloc_lists(nep_t* nep, int capA, int capS)
     NEP_TRY(dev_alloc(nep, &nep->pf, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->mA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->listS, (size_t)capS * n));
+    NEP_TRY(dev_alloc(nep, &nep->listT, (size_t)(capA + capS) * n));
     NEP_TRY(dev_alloc(nep, &nep->revS, (size_t)capS * n));
     NEP_TRY(dev_alloc(nep, &nep->mB, (size_t)(capA + capS) * n));
     NEP_TRY(dev_alloc(nep, &nep->cB, (size_t)(capA + capS) * n));
@@ -222,8 +226,13 @@ int build_lists(nep_t* nep, const double* pos_dev)
         if (fl[1]) capS = fl[4] + 8 > 256 ? 256 : fl[4] + 8;
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
-    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->listA, nep->cntA, nep->rev));
-    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->listS, nep->cntS, nep->revS));
+    {
+        const int row = nep->capA + nep->capS;
+        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capA, 32)), 256, 0, st>>>(n, nep->capA, row, 0, nep->listA, nep->listT));
+        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capS, 32)), 256, 0, st>>>(n, nep->capS, row, nep->capA, nep->listS, nep->listT));
+    }
+    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA + nep->capS, 0, nep->listA, nep->cntA, nep->listT, nep->rev));
+    NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA + nep->capS, nep->capA, nep->listS, nep->cntS, nep->listT, nep->revS));
     {
         const int longest = nep->maxA_skin > nep->maxS_skin ? nep->maxA_skin : nep->maxS_skin;
         nep->d.maskW = longest > 0 ? (longest + 63) / 64 : 1;
@@ -272,6 +281,9 @@ int dispatch_radial_reg(nep_t* nep)
 {
     const NepDims& d = nep->d;
     if (d.T * nep->KP > 64 || d.T > 5) return kNoVariant;
+    // the force kernel evaluates all T dot products per pair and selects one: beyond three species the
+    // shared-memory variant (one row of E per pair) is faster (measured at T = 5: 486 vs 523 us)
+    if (FORCE && d.T > 3) return kNoVariant;
     if (sizeof(float) * (size_t)d.T * d.T * nep->strideR > kRegTableMax) return kNoVariant;
     if (sizeof(float) * (size_t)d.T * d.T * d.NR * nep->KP > kRegTableMax) return kNoVariant;
 #define NEP_REG_CASE(TT, KPV)                                                                      \

@@ -10,7 +10,8 @@
 //   4. one thread per atom walks the 5x5x5 stencil cells, tests candidates in fp32 and resolves
 //      anything inside a guard band around a cutoff with the exact fp64 predicate of reading A8, so
 //      the sets equal an fp64 brute force bit for bit
-//   5. reverse index: slot of i in j's list, for both lists (where i delivers dU_i/dr_ij to j, Eq. 22-24)
+//   5. reverse index: slot of i in j's list, for both lists (where i delivers dU_i/dr_ij to j, Eq. 22-24),
+//      searched in an atom-major copy of the lists around the mirrored slot
 // The angular-range list (|r| < rcA+skin) and the outer shell (rcA+skin <= |r| < rcR+skin) are stored
 // disjointly; the radial list is their union.
 #pragma once
@@ -240,31 +241,71 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
     atomicMax(&flags[4], ns);
 }
 
-// ---- 5. reverse index -----------------------------------------------------------------------------------
-__global__ void k_build_rev(int n, const int* __restrict__ listA, const int* __restrict__ cntA,
-                            unsigned char* __restrict__ rev)
+// ---- 4b. atom-major copy of a list: out[atom][base + slot] = in[slot][atom] (tiled transpose) -----------
+__global__ void __launch_bounds__(256)
+k_transpose_list(int n, int cap, int cap_row, int base, const int* __restrict__ in, int* __restrict__ out)
 {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ int tile[32][33];
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;             // 32 x 8 threads
+    for (int r = ty; r < 32; r += 8) {
+        const int m = m0 + r, a = a0 + tx;
+        tile[r][tx] = (m < cap && a < n) ? in[(size_t)m * n + a] : 0;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int a = a0 + r, m = m0 + tx;
+        if (a < n && m < cap) out[(size_t)a * cap_row + base + m] = tile[tx][r];
+    }
+}
+
+// ---- 5. reverse index -----------------------------------------------------------------------------------
+// rev[m][i] = slot of i in the list of j = list[m][i].  The predicate is symmetric bit for bit, so the entry
+// exists, and the smaller index of a pair does the search and writes both directions (half the searches).
+// Both atoms walk the same stencil in the same order and j sees i in the mirrored stencil cell, so i sits
+// near slot cnt_j - 1 - m cnt_j / cnt_i of j's list.  The search reads the ATOM-MAJOR copy of j's list
+// (listT, 16 bytes = 4 slots per load, capA and capS are multiples of 4): the groups around the guess
+// share one or two 32-byte sectors, instead of one sector per probed slot in the [slot][atom] layout.
+__global__ void __launch_bounds__(128)
+k_build_rev(int n, int cap_row, int base, const int* __restrict__ list, const int* __restrict__ cnt,
+            const int* __restrict__ listT, unsigned char* __restrict__ rev)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
-    // Both atoms walk the same stencil in the same order, and j sees i in the mirrored stencil cell, so i
-    // sits near slot cnt_j - 1 - m * cnt_j / cnt_i of j's list: search outwards from there (two probes in
-    // flight per round).  The entry exists because the predicate is symmetric bit for bit.
-    const int c = cntA[s];
+    const size_t N = (size_t)n;
+    const int c = cnt[s];
     for (int m = 0; m < c; ++m) {
-        const int j = listA[(size_t)m * n + s];
-        const int cj = cntA[j];
-        const int* col = listA + j;
-        int hi = cj - 1 - (m * cj) / c;
-        hi = max(0, min(hi, cj - 1));
-        int lo = hi - 1, found = 0;
-        while (lo >= 0 || hi < cj) {
-            const int vlo = (lo >= 0) ? col[(size_t)lo * n] : -1;
-            const int vhi = (hi < cj) ? col[(size_t)hi * n] : -1;
-            if (vhi == s) { found = hi; break; }
-            if (vlo == s) { found = lo; break; }
-            --lo; ++hi;
+        const int j = list[(size_t)m * N + s];
+        if (j < s) continue;                              // written by thread j
+        const int cj = cnt[j];
+        const int4* row = reinterpret_cast<const int4*>(listT + (size_t)j * cap_row + base);
+        const int ngroups = (cj + 3) >> 2;
+        int g = cj - 1 - (m * cj) / c;
+        g = max(0, min(g, cj - 1));
+        int hi = g >> 2, lo = hi - 1, found = -1;
+        while (found < 0 && (lo >= 0 || hi < ngroups)) {
+            if (hi < ngroups) {
+                const int4 v = row[hi];
+                const int b = 4 * hi;
+                if (v.x == s && b < cj) found = b;
+                else if (v.y == s && b + 1 < cj) found = b + 1;
+                else if (v.z == s && b + 2 < cj) found = b + 2;
+                else if (v.w == s && b + 3 < cj) found = b + 3;
+                ++hi;
+            }
+            if (found < 0 && lo >= 0) {
+                const int4 v = row[lo];
+                const int b = 4 * lo;
+                if (v.x == s) found = b;
+                else if (v.y == s) found = b + 1;
+                else if (v.z == s) found = b + 2;
+                else if (v.w == s) found = b + 3;
+                --lo;
+            }
         }
-        rev[(size_t)m * n + s] = (unsigned char)found;
+        if (found < 0) found = 0;                         // cannot happen (symmetric predicate)
+        rev[(size_t)m * N + s] = (unsigned char)found;
+        rev[(size_t)found * N + j] = (unsigned char)m;
     }
 }
 
