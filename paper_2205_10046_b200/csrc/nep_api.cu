@@ -405,6 +405,23 @@ int launch_ann(nep_t* nep)
     return NEP_OK;
 }
 
+// tensor-core variant (3xTF32): descriptor tiers up to 72, weights + per-warp tiles within 100 KB of shared memory
+template <int DP>
+int launch_ann_tc(nep_t* nep, bool* done)
+{
+    const NepDims& d = nep->d;
+    const int HP = (d.H + 7) & ~7;
+    const size_t sm = sizeof(float) * ((size_t)2 * HP * ann_stride_fwd(DP) + (size_t)2 * HP * ann_stride_bwd(DP) + 2 * HP + (size_t)4 * 32 * (HP + 4));
+    *done = false;
+    if (sm > 100 * 1024) return NEP_OK;
+    NEP_TRY(allow_smem(nep, k_ann_tc<DP>, sm));
+    int grid = 0;
+    NEP_TRY(persistent_grid(nep, k_ann_tc<DP>, sm, &grid));
+    NEP_LAUNCH(NEP_K_ANN, k_ann_tc<DP><<<grid, 128, sm, nep->stream>>>(d, HP, nep->q, nep->w0p, nep->b0, nep->w1, nep->b1, nep->fp, nep->U, nep->tile_ctr + 32));
+    *done = true;
+    return NEP_OK;
+}
+
 int ann_tier(int D)
 {
     const int tiers[] = {24, 40, 56, 72, 88, 104, 120};
@@ -414,6 +431,17 @@ int ann_tier(int D)
 
 int dispatch_ann(nep_t* nep)
 {
+    if (!nep->ann_fp32) {
+        bool done = false;
+        int rc = NEP_OK;
+        switch (nep->DP) {
+            case 24: rc = launch_ann_tc<24>(nep, &done); break;
+            case 40: rc = launch_ann_tc<40>(nep, &done); break;
+            case 56: rc = launch_ann_tc<56>(nep, &done); break;
+            case 72: rc = launch_ann_tc<72>(nep, &done); break;
+        }
+        if (rc != NEP_OK || done) return rc;
+    }
     switch (nep->DP) {
         case 24: return launch_ann<24>(nep);
         case 40: return launch_ann<40>(nep);
@@ -622,6 +650,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     nep->strideR = (d.KR * d.NRP) | 1;
     nep->nch_max = 5;
     nep->smem_budget = 180 * 1024;
+    nep->ann_fp32 = getenv("NEP_ANN_FP32") != nullptr;                // tests / comparison: the fp32-FMA network kernel
     nep->force_smem_radial = getenv("NEP_RADIAL_SMEM") != nullptr;    // tests: exercise the shared-memory variants
     if (const char* e = getenv("NEP_SMEM_KB")) { const int v = atoi(e); if (v >= 8 && v <= 227) nep->smem_budget = (size_t)v * 1024; }
     if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) nep->nch_max = v; }

@@ -605,6 +605,155 @@ k_ann(NepDims D, const float* __restrict__ q, const float* __restrict__ w0p, con
 }
 
 // ---------------------------------------------------------------------------------------------------
+// (a5) on the tensor cores.  The network is the one dense contraction of the path: z[atoms x H] = q w0^T
+// and Fp[atoms x D] = cf w0.  One warp takes a 32-atom tile; mma.sync m16n8k8 TF32 with fp32 accumulation
+// and the 3xTF32 split (x = hi + lo, both TF32; acc += lo*hi + hi*lo + hi*hi), which keeps ~fp32 accuracy
+// (a plain TF32 product would miss the 1e-5 eV bar by two orders of magnitude).  Weights are split once
+// per block into shared memory, in two layouts whose row strides make the B-fragment reads of the forward
+// (stride = 12 mod 32) and of the backward pass (stride = 8 mod 32) bank-conflict-free; cf passes through
+// a per-warp shared tile (C-fragment layout -> A-fragment layout).  Fragment layouts: PTX ISA, mma.m16n8k8.
+__device__ __forceinline__ void tf32_split(float x, unsigned& hi, unsigned& lo)
+{
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
+    const float r = x - __uint_as_float(hi);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(r));
+}
+
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const unsigned (&a)[4], unsigned b0, unsigned b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+__host__ __device__ __forceinline__ int ann_stride_fwd(int DP) { return DP + ((12 - DP % 32) + 32) % 32; }
+__host__ __device__ __forceinline__ int ann_stride_bwd(int DP) { return DP + ((8 - DP % 32) + 32) % 32; }
+
+template <int DP>
+__global__ void __launch_bounds__(128)
+k_ann_tc(NepDims D, int HP, const float* __restrict__ q, const float* __restrict__ w0p, const float* __restrict__ b0,
+         const float* __restrict__ w1, float b1, float* __restrict__ fp, float* __restrict__ U, int* __restrict__ tile_ctr)
+{
+    constexpr int KT = DP / 8;
+    const int SF = ann_stride_fwd(DP), SB = ann_stride_bwd(DP), SC = HP + 4;
+    extern __shared__ __align__(16) unsigned smu[];
+    unsigned* wfh = smu;                       // [HP][SF] hi, forward layout
+    unsigned* wfl = wfh + HP * SF;             // [HP][SF] lo
+    unsigned* wbh = wfl + HP * SF;             // [HP][SB] hi, backward layout
+    unsigned* wbl = wbh + HP * SB;             // [HP][SB] lo
+    float* sb0 = reinterpret_cast<float*>(wbl + HP * SB);   // [HP]
+    float* sw1 = sb0 + HP;                                   // [HP]
+    float* scf = sw1 + HP + (threadIdx.x >> 5) * 32 * SC;    // this warp's cf tile [32][SC]
+    for (int t = threadIdx.x; t < HP * DP; t += blockDim.x) {
+        const int m = t / DP, d = t - m * DP;
+        unsigned hi, lo;
+        tf32_split(m < D.H ? w0p[m * DP + d] : 0.0f, hi, lo);
+        wfh[m * SF + d] = hi; wfl[m * SF + d] = lo;
+        wbh[m * SB + d] = hi; wbl[m * SB + d] = lo;
+    }
+    for (int t = threadIdx.x; t < HP; t += blockDim.x) { sb0[t] = t < D.H ? b0[t] : 0.0f; sw1[t] = t < D.H ? w1[t] : 0.0f; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, g = lane >> 2, t4 = lane & 3;
+    const size_t n = (size_t)D.n;
+    const int ntile = (D.n + 31) >> 5, NT = HP >> 3;
+    for (int tile = next_tile(tile_ctr); tile < ntile; tile = next_tile(tile_ctr)) {
+        const int s0 = tile * 32;
+        // A fragments of q (rows = atoms, cols = descriptor components), split once
+        unsigned ah[2][KT][4], al[2][KT][4];
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int a = s0 + mt * 16 + g + (r & 1) * 8, d = kt * 8 + t4 + (r >> 1) * 4;
+                    const float v = (a < D.n && d < D.D) ? q[(size_t)d * n + a] : 0.0f;
+                    tf32_split(v, ah[mt][kt][r], al[mt][kt][r]);
+                }
+        float e[2][2] = {{0.0f, 0.0f}, {0.0f, 0.0f}};      // [m-tile][row g / g+8] partial energies
+        for (int nt = 0; nt < NT; ++nt) {
+            float c[2][4];
+            {
+                const float nb0 = -sb0[nt * 8 + 2 * t4], nb1 = -sb0[nt * 8 + 2 * t4 + 1];
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) { c[mt][0] = nb0; c[mt][1] = nb1; c[mt][2] = nb0; c[mt][3] = nb1; }
+            }
+            const unsigned* bh = wfh + (nt * 8 + g) * SF + t4;
+            const unsigned* bl = wfl + (nt * 8 + g) * SF + t4;
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                const unsigned h0 = bh[kt * 8], h1 = bh[kt * 8 + 4], l0 = bl[kt * 8], l1 = bl[kt * 8 + 4];
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) {
+                    mma_tf32(c[mt], al[mt][kt], h0, h1);
+                    mma_tf32(c[mt], ah[mt][kt], l0, l1);
+                    mma_tf32(c[mt], ah[mt][kt], h0, h1);
+                }
+            }
+            const float w1a = sw1[nt * 8 + 2 * t4], w1b = sw1[nt * 8 + 2 * t4 + 1];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                const float x0 = tanhf(c[mt][0]), x1 = tanhf(c[mt][1]), x2 = tanhf(c[mt][2]), x3 = tanhf(c[mt][3]);
+                e[mt][0] = fmaf(w1a, x0, fmaf(w1b, x1, e[mt][0]));
+                e[mt][1] = fmaf(w1a, x2, fmaf(w1b, x3, e[mt][1]));
+                float* r0 = scf + (mt * 16 + g) * SC + nt * 8 + 2 * t4;
+                *reinterpret_cast<float2*>(r0) = make_float2(w1a * (1.0f - x0 * x0), w1b * (1.0f - x1 * x1));
+                *reinterpret_cast<float2*>(r0 + 8 * SC) = make_float2(w1a * (1.0f - x2 * x2), w1b * (1.0f - x3 * x3));
+            }
+        }
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                float v = e[mt][h];
+                v += __shfl_xor_sync(0xffffffffu, v, 1);
+                v += __shfl_xor_sync(0xffffffffu, v, 2);
+                const int a = s0 + mt * 16 + g + h * 8;
+                if (t4 == 0 && a < D.n) U[a] = v - b1;
+            }
+        __syncwarp();
+        // backward: Fp[atoms x DP] = cf[atoms x HP] w0[HP x DP]
+        float f[2][KT][4];
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int dt = 0; dt < KT; ++dt)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) f[mt][dt][r] = 0.0f;
+        for (int kt = 0; kt < NT; ++kt) {
+            unsigned ch[2][4], cl[2][4];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+                    tf32_split(scf[(mt * 16 + g + (r & 1) * 8) * SC + kt * 8 + t4 + (r >> 1) * 4], ch[mt][r], cl[mt][r]);
+            const unsigned* bh = wbh + (kt * 8 + t4) * SB + g;
+            const unsigned* bl = wbl + (kt * 8 + t4) * SB + g;
+#pragma unroll
+            for (int dt = 0; dt < KT; ++dt) {
+                const unsigned h0 = bh[dt * 8], h1 = bh[dt * 8 + 4 * SB], l0 = bl[dt * 8], l1 = bl[dt * 8 + 4 * SB];
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) {
+                    mma_tf32(f[mt][dt], cl[mt], h0, h1);
+                    mma_tf32(f[mt][dt], ch[mt], l0, l1);
+                    mma_tf32(f[mt][dt], ch[mt], h0, h1);
+                }
+            }
+        }
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int dt = 0; dt < KT; ++dt)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int a = s0 + mt * 16 + g + (r >> 1) * 8, d = dt * 8 + 2 * t4 + (r & 1);
+                    if (a < D.n && d < D.D) fp[(size_t)d * n + a] = f[mt][dt][r];
+                }
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // G_nk = dU_i/dS_nk from Fp and S (chain rule through Eqs. (13)-(19)).
 __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float f4, float f5, const NepCoef& C, float* G)
 {

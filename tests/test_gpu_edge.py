@@ -209,6 +209,35 @@ def test_shared_memory_radial_variants(pkg, oracle_mod, idx, cells):
         del os.environ["NEP_RADIAL_SMEM"]
 
 
+@pytest.mark.parametrize("idx,cells", [(3, (4, 4, 3)), (4, (5, 5, 5))])
+def test_network_kernel_variants_agree(pkg, oracle_mod, idx, cells):
+    """The network runs on the tensor cores (3xTF32, k_ann_tc) where the shapes allow; NEP_ANN_FP32 (read at
+    nep_create) selects the fp32-FMA kernel.  Both must meet the oracle, and each other to fp32 round-off."""
+    cfg = W.get_config(idx, cells)
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    out = {}
+    for variant in ("tc", "fp32"):
+        if variant == "fp32":
+            os.environ["NEP_ANN_FP32"] = "1"
+        try:
+            nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+            dpos = torch.tensor(s.pos, device="cuda:0")
+            nep.nep_neighbors(dpos, torch.tensor(s.types, device="cuda:0"), s.box, 0.3)
+            e, f, w = nep.nep_compute(dpos)
+            q, fp = nep.nep_get_descriptors()
+            out[variant] = (e.cpu().numpy(), fp.cpu().numpy())
+            nep.close()
+        finally:
+            os.environ.pop("NEP_ANN_FP32", None)
+    eo, fo, wo, qo, fpo, So = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box, want_internals=True)
+    for variant in out:
+        e, fp = out[variant]
+        assert np.abs(e - eo).max() <= 1e-5
+        assert np.abs(fp - fpo).max() <= 2e-5 * np.abs(fpo).max()
+    assert np.abs(out["tc"][0] - out["fp32"][0]).max() <= 2e-6
+    assert np.abs(out["tc"][1] - out["fp32"][1]).max() <= 4e-6 * np.abs(fpo).max()
+
+
 def test_md_step_zero_steps_and_state_errors(pkg):
     cfg = W.get_config(0)
     s, p = W.make_system(cfg), W.make_params(cfg)
