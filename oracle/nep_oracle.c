@@ -253,22 +253,49 @@ void onep_ann(int D, int H, const double* w0, const double* b0, const double* w1
     *energy = e - b1[0];
 }
 
-/* ---- O1: minimum image + neighbour predicate (reading A8) -----------------------------
- * each component: d = (r_j - r_i) - L * rint((r_j - r_i)/L) on periodic axes;
+/* ---- O1: minimum image + neighbour predicate (readings A8, A8t) -----------------------
+ * The cell is box[9] = rows a, b, c (lattice vectors).
+ * Orthorhombic cell (all off-diagonal elements zero), reading A8, literally:
+ *   each component: d = (r_j - r_i) - L * rint((r_j - r_i)/L) on periodic axes.
+ * General (triclinic) cell, reading A8t: t = r_j - r_i; fractional s_k = (t_x Hinv[x][k] + t_y Hinv[y][k])
+ *   + t_z Hinv[z][k] with Hinv the inverse of H = box by cofactors; n_k = rint(s_k) on periodic lattice
+ *   directions; d = ((t - n_a a) - n_b b) - n_c c.  This is the nearest image whenever |d| is below half the
+ *   smallest perpendicular width of the cell, which the harness guarantees for every cutoff it uses.
  * d2 = (dx*dx + dy*dy) + dz*dz in IEEE fp64 without contraction; neighbour iff d2 < rc*rc (strict). */
-static void min_image(const double* ri, const double* rj, const double box[3], const int32_t pbc[3], double d[3])
+static void inverse3(const double H[9], double inv[9])
 {
-    for (int a = 0; a < 3; ++a) {
-        double t = rj[a] - ri[a];
-        if (pbc[a]) t = t - box[a] * rint(t / box[a]);
-        d[a] = t;
+    const double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+    const double det = (H[0] * c00 + H[1] * c01) + H[2] * c02;
+    inv[0] = c00 / det; inv[1] = (H[2] * H[7] - H[1] * H[8]) / det; inv[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+    inv[3] = c01 / det; inv[4] = (H[0] * H[8] - H[2] * H[6]) / det; inv[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+    inv[6] = c02 / det; inv[7] = (H[1] * H[6] - H[0] * H[7]) / det; inv[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+}
+
+static void min_image(const double* ri, const double* rj, const double box[9], const int32_t pbc[3], double d[3])
+{
+    const int diagonal = box[1] == 0.0 && box[2] == 0.0 && box[3] == 0.0 && box[5] == 0.0 && box[6] == 0.0 && box[7] == 0.0;
+    if (diagonal) {
+        for (int a = 0; a < 3; ++a) {
+            double t = rj[a] - ri[a];
+            if (pbc[a]) t = t - box[4 * a] * rint(t / box[4 * a]);
+            d[a] = t;
+        }
+        return;
     }
+    double inv[9], t[3], nk[3];
+    inverse3(box, inv);
+    for (int a = 0; a < 3; ++a) t[a] = rj[a] - ri[a];
+    for (int k = 0; k < 3; ++k) {
+        const double sk = (t[0] * inv[k] + t[1] * inv[3 + k]) + t[2] * inv[6 + k];    /* row vector times Hinv */
+        nk[k] = pbc[k] ? rint(sk) : 0.0;
+    }
+    for (int a = 0; a < 3; ++a) d[a] = ((t[a] - nk[0] * box[a]) - nk[1] * box[3 + a]) - nk[2] * box[6 + a];
 }
 static double dist2(const double d[3]) { return (d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]; }
 
 /* brute force list: count[i], list[i*cap + m]; entries beyond cap are counted but not stored.
  * returns the largest count (so the caller can detect cap overflow).                               */
-int64_t onep_neighbors(int64_t n, const double* pos, const double box[3], const int32_t pbc[3],
+int64_t onep_neighbors(int64_t n, const double* pos, const double box[9], const int32_t pbc[3],
                        double rc, int32_t* count, int32_t* list, int64_t cap)
 {
     int64_t maxc = 0;
@@ -292,7 +319,7 @@ int64_t onep_neighbors(int64_t n, const double* pos, const double box[3], const 
 }
 
 /* neighbours of a chosen subset of atoms only (O(n_sel * N)); used for sampled full-size parity.   */
-int64_t onep_neighbors_of(int64_t n, const double* pos, const double box[3], const int32_t pbc[3],
+int64_t onep_neighbors_of(int64_t n, const double* pos, const double box[9], const int32_t pbc[3],
                           double rc, int64_t n_sel, const int64_t* sel, int32_t* count, int32_t* list, int64_t cap)
 {
     int64_t maxc = 0;
@@ -325,7 +352,7 @@ int64_t onep_neighbors_of(int64_t n, const double* pos, const double box[3], con
  * Returns 0, or -1 on allocation failure.                                                           */
 typedef struct { int32_t j; double d[3]; double r; } pair_t;
 
-static pair_t* build_pairs(int64_t n, const double* pos, const double box[3], const int32_t pbc[3],
+static pair_t* build_pairs(int64_t n, const double* pos, const double box[9], const int32_t pbc[3],
                            double rc, int64_t** first_out)
 {
     int64_t* first = (int64_t*)malloc(sizeof(int64_t) * (size_t)(n + 1));
@@ -371,7 +398,7 @@ static pair_t* build_pairs(int64_t n, const double* pos, const double box[3], co
 int onep_compute(const onep_hyper* h,
                  const double* c_radial, const double* c_angular,
                  const double* w0, const double* b0, const double* w1, const double* b1,
-                 int64_t n, const double* pos, const int32_t* type, const double box[3], const int32_t pbc[3],
+                 int64_t n, const double* pos, const int32_t* type, const double box[9], const int32_t pbc[3],
                  double* energy, double* force, double* virial,
                  double* q_out, double* fp_out, double* S_out)
 {
@@ -530,7 +557,7 @@ int onep_md(const onep_hyper* h,
             const double* c_radial, const double* c_angular,
             const double* w0, const double* b0, const double* w1, const double* b1,
             int64_t n, double* pos, double* vel, const int32_t* type, const double* mass_amu,
-            const double box[3], const int32_t pbc[3], double dt_fs, int32_t n_steps,
+            const double box[9], const int32_t pbc[3], double dt_fs, int32_t n_steps,
             double* e_pot, double* e_kin)
 {
     const double conv = 9.648533212e-3;

@@ -148,13 +148,21 @@ def ann(w0, b0, w1, b1, q):
     return e.value, fp
 
 
+def _box9(box) -> np.ndarray:
+    """The cell as 9 numbers, rows = lattice vectors a, b, c; three numbers mean an orthorhombic cell."""
+    b = np.asarray(box, dtype=np.float64)
+    if b.size == 3:
+        b = np.diag(b.reshape(3))
+    return np.ascontiguousarray(b.reshape(9))
+
+
 def _pbc(pbc) -> np.ndarray:
     return np.ascontiguousarray(pbc, dtype=np.int32)
 
 
 def neighbors(pos, box, rc: float, pbc=(1, 1, 1), cap: Optional[int] = None):
     """Brute-force neighbour sets: returns (count[n], list[n][cap]); grows cap until nothing is cut."""
-    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    pos, box, pbc = _d(pos), _box9(box), _pbc(pbc)
     n = pos.shape[0]
     cap = cap or 64
     while True:
@@ -167,7 +175,7 @@ def neighbors(pos, box, rc: float, pbc=(1, 1, 1), cap: Optional[int] = None):
 
 
 def neighbors_of(pos, box, rc: float, sel, pbc=(1, 1, 1), cap: int = 256):
-    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    pos, box, pbc = _d(pos), _box9(box), _pbc(pbc)
     sel = np.ascontiguousarray(sel, dtype=np.int64)
     n, ns = pos.shape[0], sel.shape[0]
     while True:
@@ -184,7 +192,7 @@ def compute(hyper, params, pos, types, box, pbc=(1, 1, 1), want_internals: bool 
     """Energy[n], force[n][3], virial[n][9] (+ q[n][D], fp[n][D], S[n][NA][24] if want_internals).
     `params` holds fp32 arrays; they are widened to fp64 here, unchanged in value."""
     h = OracleHyper.from_hyper(hyper)
-    pos, box, pbc = _d(pos), _d(box), _pbc(pbc)
+    pos, box, pbc = _d(pos), _box9(box), _pbc(pbc)
     types = np.ascontiguousarray(types, dtype=np.int32)
     n = pos.shape[0]
     cr, ca, w0, b0, w1, b1 = map(_d, (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1))
@@ -208,7 +216,7 @@ def md(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int, 
     """Velocity-Verlet NVE; returns (pos, vel, e_pot[n_steps+1], e_kin[n_steps+1]) (copies)."""
     h = OracleHyper.from_hyper(hyper)
     pos, vel = _d(pos).copy(), _d(vel).copy()
-    box, pbc, masses = _d(box), _pbc(pbc), _d(masses)
+    box, pbc, masses = _box9(box), _pbc(pbc), _d(masses)
     types = np.ascontiguousarray(types, dtype=np.int32)
     cr, ca, w0, b0, w1, b1 = map(_d, (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1))
     ep = np.zeros(n_steps + 1)

@@ -155,3 +155,79 @@ def test_berendsen_limits_and_one_step_identity(oracle_mod):
     # tau = dt: the target is hit exactly; the ramp is linear in the step number
     _, _, tb2, ta2 = oracle_mod.md_berendsen(*args, 1.0, 4, 300.0, 700.0, 1.0)
     np.testing.assert_allclose(ta2, [400.0, 500.0, 600.0, 700.0], rtol=1e-12)
+
+
+# ------------------------------------------------------------------ triclinic cells (reading A8t)
+def _brute_force_images(pos, H, rc):
+    """the plain definition: j is a neighbour of i iff some lattice image of j is closer than rc"""
+    n = len(pos)
+    shifts = np.array([[i, j, k] for i in (-2, -1, 0, 1, 2) for j in (-2, -1, 0, 1, 2) for k in (-2, -1, 0, 1, 2)], dtype=np.float64) @ H
+    sets = []
+    for i in range(n):
+        d = pos[None, :, :] - pos[i][None, None, :] + shifts[:, None, :]
+        close = ((d * d).sum(axis=2) < rc * rc).any(axis=0)
+        close[i] = False
+        sets.append(set(np.nonzero(close)[0].tolist()))
+    return sets
+
+
+def test_triclinic_neighbours_equal_lattice_image_search(oracle_mod):
+    cfg = W.get_config(3, cells=(4, 4, 4))
+    s = W.make_system(cfg)
+    pos, H = W.sheared(s, 0.31, -0.17, 0.23)
+    rc = 6.0
+    assert W.perpendicular_widths(H).min() >= 2 * rc
+    cnt, lst = oracle_mod.neighbors(pos, H, rc)
+    want = _brute_force_images(pos, H, rc)
+    assert sum(len(w) for w in want) > 50 * len(pos)
+    for i in range(len(pos)):
+        assert set(lst[i, :cnt[i]].tolist()) == want[i]
+    # positions shifted by arbitrary lattice vectors: the same sets
+    rng = np.random.default_rng(3)
+    pos2 = pos + rng.integers(-3, 4, size=(len(pos), 3)).astype(np.float64) @ H
+    cnt2, lst2 = oracle_mod.neighbors(pos2, H, rc)
+    for i in range(len(pos)):
+        assert set(lst2[i, :cnt2[i]].tolist()) == want[i]
+
+
+def test_triclinic_description_of_an_orthorhombic_lattice(oracle_mod):
+    """The cell (a, b + a, c - 2b) spans the same lattice as (a, b, c): the same periodic structure, so every
+    per-atom energy, force and virial must equal the orthorhombic (pinned) result."""
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    H0 = np.diag(s.box)
+    H1 = np.array([H0[0], H0[1] + H0[0], H0[2] - 2 * H0[1]])
+    hy = cfg.hyper
+    # cutoffs within half the smallest perpendicular width of the skewed cell
+    from dataclasses import replace
+    w = W.perpendicular_widths(H1).min()
+    hy = replace(hy, rc_radial=min(hy.rc_radial, 0.49 * w), rc_angular=min(hy.rc_angular, 0.4 * w))
+    e0, f0, w0 = oracle_mod.compute(hy, p, s.pos, s.types, s.box)
+    e1, f1, w1 = oracle_mod.compute(hy, p, s.pos, s.types, H1)
+    np.testing.assert_allclose(e1, e0, rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(f1, f0, rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(w1, w0, rtol=1e-10, atol=1e-12)
+
+
+def test_triclinic_forces_and_shear_virial_by_finite_differences(oracle_mod):
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    pos, H = W.sheared(s, 0.12, -0.08, 0.1)
+    from dataclasses import replace
+    w = W.perpendicular_widths(H).min()
+    hy = replace(cfg.hyper, rc_radial=min(cfg.hyper.rc_radial, 0.49 * w), rc_angular=min(cfg.hyper.rc_angular, 0.4 * w))
+    E = lambda x, B: oracle_mod.compute(hy, p, x, s.types, B)[0].sum()
+    e, f, wv = oracle_mod.compute(hy, p, pos, s.types, H)
+    h = 1e-4
+    for i, a in ((0, 0), (17, 1), (53, 2)):
+        pp, pm = pos.copy(), pos.copy()
+        pp[i, a] += h; pm[i, a] -= h
+        assert f[i, a] == pytest.approx(-(E(pp, H) - E(pm, H)) / (2 * h), rel=2e-6, abs=1e-8)
+    np.testing.assert_allclose(f.sum(axis=0), 0.0, atol=1e-10)
+    wtot = wv.sum(axis=0).reshape(3, 3)
+    h = 1e-5
+    for a, b in ((0, 1), (1, 0), (0, 2), (2, 1), (1, 1)):      # periodic cell: shear strains included
+        eps = np.zeros((3, 3)); eps[a, b] = h
+        Fp, Fm = (np.eye(3) + eps).T, (np.eye(3) - eps).T
+        dE = (E(pos @ Fp, H @ Fp) - E(pos @ Fm, H @ Fm)) / (2 * h)
+        assert wtot[a, b] == pytest.approx(-dE, rel=5e-6, abs=1e-8)

@@ -215,3 +215,19 @@ def random_cluster(seed: int, n: int, n_types: int, extent: float, min_dist: flo
             pts.append(p)
     types = rng.integers(0, n_types, size=n).astype(np.int32)
     return np.array(pts), types
+
+
+def sheared(system: "System", xy: float, xz: float, yz: float):
+    """A genuinely triclinic copy of an orthorhombic system: positions and cell mapped by r' = r F with
+    F = [[1,0,0],[xy,1,0],[xz,yz,1]] (row vectors).  Returns (pos', box'[3][3]) with rows a', b', c'."""
+    F = np.array([[1.0, 0.0, 0.0], [xy, 1.0, 0.0], [xz, yz, 1.0]])
+    return np.ascontiguousarray(system.pos @ F), np.diag(system.box) @ F
+
+
+def perpendicular_widths(box33) -> np.ndarray:
+    """Distances between opposite faces of the cell with rows a, b, c."""
+    H = np.asarray(box33, dtype=np.float64).reshape(3, 3)
+    vol = abs(np.linalg.det(H))
+    a, b, c = H
+    return np.array([vol / np.linalg.norm(np.cross(b, c)), vol / np.linalg.norm(np.cross(c, a)),
+                     vol / np.linalg.norm(np.cross(a, b))])
