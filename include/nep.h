@@ -43,8 +43,8 @@ typedef struct {
 typedef enum {
     NEP_OK = 0,
     NEP_ERR_INVALID_ARG = -1,        /* null pointer, value out of the ranges above, n <= 0, cap too small */
-    NEP_ERR_BOX_TOO_SMALL = -2,      /* a box edge < 2 (rc_radial + skin): minimum image would break      */
-    NEP_ERR_UNSUPPORTED_BOX = -3,    /* non-orthorhombic box (off-diagonal elements != 0)                 */
+    NEP_ERR_BOX_TOO_SMALL = -2,      /* a perpendicular width < 2 (rc_radial + skin): minimum image breaks */
+    NEP_ERR_UNSUPPORTED_BOX = -3,    /* degenerate or left-handed cell (det of the row vectors <= 0)      */
     NEP_ERR_NEIGHBOR_OVERFLOW = -4,  /* a list outgrew its storage and regrowing failed (never truncated) */
     NEP_ERR_STATE = -5,              /* compute / md_step before nep_neighbors, or hook before compute    */
     NEP_ERR_CUDA = -6,               /* a CUDA runtime call failed (text in nep_last_error)               */
@@ -78,10 +78,15 @@ int nep_num_descriptors(const nep_hyper_t* h);
  * Cell-binned construction of the radial and angular neighbour lists NN^R/NL^R, NN^A/NL^A
  * (construction itself is not described by the paper).
  *   pos_dev  [n][3] fp64 positions (need not be wrapped into the box);  type_dev [n] int32 in [0,T);
- *   box      HOST, 9 doubles, row vectors a,b,c; must be orthorhombic (only box[0], box[4], box[8] != 0);
+ *   box      HOST, 9 doubles: the cell's lattice vectors a, b, c as rows (Angstrom), right-handed
+ *            (det > 0); orthorhombic or general (triclinic).  Every perpendicular width of the cell must
+ *            be >= 2 (rc_radial + skin) (NEP_ERR_BOX_TOO_SMALL), so that the minimum image is unique;
  *   skin     >= 0: lists hold every pair with |r_ij| < r_c + skin (Verlet skin).
- * Membership (reading A8): with d = (r_j - r_i) - L*rint((r_j - r_i)/L) per axis in IEEE fp64,
- * j is a neighbour of i iff (dx*dx + dy*dy) + dz*dz < (r_c+skin)*(r_c+skin) -- evaluated exactly so, so
+ * Membership.  Orthorhombic cell (all off-diagonal elements zero), reading A8: with
+ * d = (r_j - r_i) - L*rint((r_j - r_i)/L) per axis in IEEE fp64, j is a neighbour of i iff
+ * (dx*dx + dy*dy) + dz*dz < (r_c+skin)*(r_c+skin).  General cell, reading A8t: t = r_j - r_i,
+ * n_k = rint((t_x Hinv[x][k] + t_y Hinv[y][k]) + t_z Hinv[z][k]), d = ((t - n_a a) - n_b b) - n_c c, same
+ * test.  Both are evaluated exactly so (fp64, no contraction) for every candidate near a cutoff, so
  * the sets equal a brute-force fp64 search bit for bit.  The list order within an atom is unspecified
  * but deterministic.  Copies the types; synchronises (reads back list sizes; regrows and rebuilds on
  * overflow).  n <= 16,777,216.                                                                        */

@@ -174,12 +174,13 @@ int build_lists(nep_t* nep, const double* pos_dev)
     P.ncx = nep->ncell[0]; P.ncy = nep->ncell[1]; P.ncz = nep->ncell[2];
     P.ntx = nep->ntile[0]; P.nty = nep->ntile[1];
     P.hx = P.hy = P.hz = 2;
-    P.Lx = nep->box[0]; P.Ly = nep->box[1]; P.Lz = nep->box[2];
-    P.inv_Lx = 1.0 / P.Lx; P.inv_Ly = 1.0 / P.Ly; P.inv_Lz = 1.0 / P.Lz;
-    P.sx = nep->d.sx; P.sy = nep->d.sy; P.sz = nep->d.sz;
+    CellInv inv;
+    for (int a = 0; a < 9; ++a) { P.H[a] = nep->H[a]; P.Hinv[a] = nep->Hinv[a]; P.h[a] = nep->d.h[a]; inv.m[a] = nep->Hinv[a]; }
+    P.tri = nep->d.tri;
     P.cutA2_d = acut * acut; P.cutR2_d = rcut * rcut;
     P.cutA2 = (float)P.cutA2_d; P.cutR2 = (float)P.cutR2_d;
-    const double Lmax = fmax(P.Lx, fmax(P.Ly, P.Lz));
+    double Lmax = 0.0;                                   // |a| + |b| + |c| bounds every component's scale
+    for (int k = 0; k < 3; ++k) Lmax += sqrt(P.H[3 * k] * P.H[3 * k] + P.H[3 * k + 1] * P.H[3 * k + 1] + P.H[3 * k + 2] * P.H[3 * k + 2]);
     // fp32/quantisation error of r^2 is < 2 r (3 L 2^-32 + r 2^-22); the band is ~100x wider
     P.guardR = (float)(1e-4 * P.cutR2_d + 64.0 * Lmax * rcut / 4294967296.0);
     P.guardA = (float)(1e-4 * P.cutA2_d + 64.0 * Lmax * acut / 4294967296.0);
@@ -196,11 +197,11 @@ int build_lists(nep_t* nep, const double* pos_dev)
     }
     NEP_LAUNCH(NEP_K_SCATTER, k_scatter<<<div_up(n, TB), TB, 0, st>>>(n, nep->cell_of, nep->rank_in_cell, nep->cell_start, nep->perm));
     NEP_LAUNCH(NEP_K_SORT_CELLS, k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm));
-    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, P.inv_Lx, P.inv_Ly, P.inv_Lz, nep->posq));
+    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
     NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
 
     if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
-        const double rho = (double)n / (P.Lx * P.Ly * P.Lz);
+        const double rho = (double)n / nep->volume;
         const double vA = 4.0 / 3.0 * 3.14159265358979 * acut * acut * acut, vR = 4.0 / 3.0 * 3.14159265358979 * rcut * rcut * rcut;
         int capA = (int)(rho * vA * 1.25) + 12, capS = (int)(rho * (vR - vA) * 1.25) + 12;
         if (capA > 256) capA = 256;
@@ -508,8 +509,9 @@ int evaluate(nep_t* nep, const double* pos_dev)
     const NepDims& d = nep->d;
     const int n = d.n;
     cudaStream_t st = nep->stream;
-    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, 1.0 / nep->box[0], 1.0 / nep->box[1],
-                                               1.0 / nep->box[2], nep->posq));
+    CellInv inv;
+    for (int a = 0; a < 9; ++a) inv.m[a] = nep->Hinv[a];
+    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
     NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
     NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
@@ -527,19 +529,36 @@ int evaluate(nep_t* nep, const double* pos_dev)
 int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
 {
     if (n <= 0 || n > NEP_MAX_ATOMS || !box || !(skin >= 0.0)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad n, box or skin");
+    // cell rows a, b, c; inverse by cofactors; perpendicular widths w_k = 1 / |column k of Hinv|
+    const double* H = box;
     for (int a = 0; a < 9; ++a)
-        if (a % 4 != 0 && box[a] != 0.0) return nep_fail(nep, NEP_ERR_UNSUPPORTED_BOX, "only orthorhombic boxes are supported");
-    const double L[3] = {box[0], box[4], box[8]};
+        if (!(H[a] == H[a]) || fabs(H[a]) > 1e12) return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad box");
+    const double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+    const double det = (H[0] * c00 + H[1] * c01) + H[2] * c02;
+    if (!(det > 0.0)) return nep_fail(nep, NEP_ERR_UNSUPPORTED_BOX, "the cell vectors a, b, c must form a right-handed, non-degenerate cell");
+    double inv[9];
+    inv[0] = c00 / det; inv[1] = (H[2] * H[7] - H[1] * H[8]) / det; inv[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+    inv[3] = c01 / det; inv[4] = (H[0] * H[8] - H[2] * H[6]) / det; inv[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+    inv[6] = c02 / det; inv[7] = (H[1] * H[6] - H[0] * H[7]) / det; inv[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+    double width[3];
+    for (int k = 0; k < 3; ++k) width[k] = 1.0 / sqrt(inv[k] * inv[k] + inv[3 + k] * inv[3 + k] + inv[6 + k] * inv[6 + k]);
     const double rcut = nep->h.rc_radial + skin;
-    for (int a = 0; a < 3; ++a)
-        if (!(L[a] >= 2.0 * rcut)) return nep_fail(nep, NEP_ERR_BOX_TOO_SMALL, "box edge < 2 (rc_radial + skin)");
+    for (int k = 0; k < 3; ++k)
+        if (!(width[k] >= 2.0 * rcut)) return nep_fail(nep, NEP_ERR_BOX_TOO_SMALL, "a perpendicular width of the cell < 2 (rc_radial + skin)");
     const bool same_n = (n == nep->n);
     nep->skin = skin;
+    nep->volume = det;
+    nep->d.tri = 0;
+    for (int a = 0; a < 9; ++a) {
+        nep->H[a] = H[a];
+        nep->Hinv[a] = inv[a];
+        nep->d.h[a] = (float)(H[a] / 4294967296.0);
+        if (a % 4 != 0 && H[a] != 0.0) nep->d.tri = 1;
+    }
     int64_t nc = 1;
     const double cell_min = 0.5 * rcut * (1.0 + 1e-6);
-    for (int a = 0; a < 3; ++a) {
-        nep->box[a] = L[a];
-        int c = (int)floor(L[a] / cell_min);
+    for (int a = 0; a < 3; ++a) {                       // cells are slabs in fractional space: thickness width / nc
+        int c = (int)floor(width[a] / cell_min);
         if (c < 1) c = 1;
         if (c > 1024) c = 1024;
         nep->ncell[a] = c;
@@ -547,9 +566,6 @@ int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
         nc *= 4 * (int64_t)nep->ntile[a];
     }
     nep->n_cells = nc;
-    nep->d.sx = (float)(L[0] / 4294967296.0);
-    nep->d.sy = (float)(L[1] / 4294967296.0);
-    nep->d.sz = (float)(L[2] / 4294967296.0);
     if (!same_n || n > nep->atom_cap) {
         nep->n = n;
         nep->d.n = (int)n;
@@ -589,7 +605,7 @@ const char* nep_status_string(int status)
         case NEP_OK: return "ok";
         case NEP_ERR_INVALID_ARG: return "invalid argument";
         case NEP_ERR_BOX_TOO_SMALL: return "box too small for the cutoff (minimum image)";
-        case NEP_ERR_UNSUPPORTED_BOX: return "unsupported (non-orthorhombic) box";
+        case NEP_ERR_UNSUPPORTED_BOX: return "unsupported box (degenerate or left-handed cell)";
         case NEP_ERR_NEIGHBOR_OVERFLOW: return "neighbour list overflow";
         case NEP_ERR_STATE: return "call out of order";
         case NEP_ERR_CUDA: return "CUDA error";
@@ -821,7 +837,8 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
     cudaStream_t st = nep->stream;
     if (skin != nep->skin) {
         // a different skin takes effect at once: lists are rebuilt for the current positions
-        const double box9[9] = {nep->box[0], 0, 0, 0, nep->box[1], 0, 0, 0, nep->box[2]};
+        double box9[9];
+        for (int a = 0; a < 9; ++a) box9[a] = nep->H[a];
         NEP_TRY(setup_system(nep, nep->n, box9, skin));
         NEP_TRY(build_lists(nep, pos_dev));
         nep->force_current = false;

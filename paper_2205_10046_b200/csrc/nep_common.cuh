@@ -33,7 +33,8 @@ struct NepDims {
     int KAR;                     // rows of an angular coefficient table: 1 + (KA - 1 rounded up to 4)
     int nblk, has4, has5;        // descriptor blocks after the radial one; 4-/5-body present
     float rcR, rcA, rcR_inv, rcA_inv, rcR2, rcA2;
-    float sx, sy, sz;            // L / 2^32: quantised coordinate unit -> Angstrom
+    float h[9];                  // cell rows a, b, c times 2^-32: quantised fractional units -> Angstrom
+    int tri;                     // the cell has off-diagonal elements (general 3x3 product in pair_vec)
     int capA, capS;              // storage rows of the skin lists (angular-range part, outer shell)
     int maskW;                   // 64-bit words of one in-cutoff mask (covers the longest skin list)
     int mrec;                    // 64-bit words of an atom's mask record (4 maskW, see k_filter)
@@ -80,7 +81,8 @@ struct nep_ctx {
 
     // system
     int64_t n;
-    double box[3];
+    double H[9], Hinv[9];    // cell rows a, b, c (Angstrom) and the inverse (fractional s = r Hinv)
+    double volume;
     double skin;
     int ncell[3];
     int ntile[3];            // 4-cell tiles per axis
@@ -219,16 +221,23 @@ static inline int round_up4(int a) { return (a + 3) & ~3; }
 __device__ __forceinline__ int round_up4_dev(int a) { return (a + 3) & ~3; }
 
 // ---------------------------------------------------------------------------------------------------
-// Pair geometry from quantised coordinates.  Positions are stored as 32-bit fractions of the box edge,
-// so the wrapped integer difference IS the minimum image (exact, branch-free); the result is converted
-// to Angstrom in fp32.  d = r_j - r_i.  dx(i,j) = -dx(j,i) bit for bit, so r2 is the same
+// Pair geometry from quantised coordinates.  Positions are stored as 32-bit fractions along the lattice
+// vectors a, b, c, so the wrapped integer difference IS the minimum image (exact, branch-free; reading A8t:
+// valid for cutoffs up to half the smallest perpendicular width); it is converted to Angstrom in fp32,
+// d = fa a + fb b + fc c -- one multiplication per component in an orthorhombic cell.  d = r_j - r_i.  dx(i,j) = -dx(j,i) bit for bit, so r2 is the same
 // for both orderings of a pair and both atoms take the same in-cutoff decision.
 __device__ __forceinline__ void pair_vec(const int4& pi, const int4& pj, const NepDims& D,
                                          float& dx, float& dy, float& dz, float& r2)
 {
-    dx = (float)(int)((unsigned)pj.x - (unsigned)pi.x) * D.sx;
-    dy = (float)(int)((unsigned)pj.y - (unsigned)pi.y) * D.sy;
-    dz = (float)(int)((unsigned)pj.z - (unsigned)pi.z) * D.sz;
+    const float fa = (float)(int)((unsigned)pj.x - (unsigned)pi.x);
+    const float fb = (float)(int)((unsigned)pj.y - (unsigned)pi.y);
+    const float fc = (float)(int)((unsigned)pj.z - (unsigned)pi.z);
+    if (!D.tri) { dx = fa * D.h[0]; dy = fb * D.h[4]; dz = fc * D.h[8]; }
+    else {
+        dx = fmaf(fc, D.h[6], fmaf(fb, D.h[3], fa * D.h[0]));
+        dy = fmaf(fc, D.h[7], fmaf(fb, D.h[4], fa * D.h[1]));
+        dz = fmaf(fc, D.h[8], fmaf(fb, D.h[5], fa * D.h[2]));
+    }
     r2 = dx * dx + dy * dy + dz * dz;
 }
 

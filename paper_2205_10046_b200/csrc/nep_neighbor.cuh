@@ -22,18 +22,21 @@ struct BuildParams {
     int ncx, ncy, ncz;
     int ntx, nty;            // tiles (4 cells) per axis x, y: cell rank = tile * 64 + Morton(cell & 3)
     int hx, hy, hz;          // stencil half widths (2) -- or "all cells" when 2h+1 >= nc
-    double Lx, Ly, Lz;
-    double inv_Lx, inv_Ly, inv_Lz;
-    float sx, sy, sz;
+    double H[9], Hinv[9];    // cell rows a, b, c and the inverse
+    float h[9];              // H * 2^-32 (fp32 candidate test)
+    int tri;                 // off-diagonal elements present
     float cutA2, cutR2;      // (rcA+skin)^2, (rcR+skin)^2 in fp32 (fast test)
     float guardA, guardR;    // half width of the fp64-resolve band around each
     double cutA2_d, cutR2_d; // exact fp64 thresholds rc*rc
     int capA, capS;
 };
 
-__device__ __forceinline__ unsigned quantize_frac(double x, double inv_L)
+struct CellInv { double m[9]; };     // Hinv, passed by value
+
+// fractional coordinate k of a position, wrapped into [0,1), as a 32-bit fraction
+__device__ __forceinline__ unsigned quantize_frac(const double* __restrict__ p, const double* inv, int k)
 {
-    double f = x * inv_L;
+    double f = (p[0] * inv[k] + p[1] * inv[3 + k]) + p[2] * inv[6 + k];
     f -= floor(f);
     return (unsigned)(unsigned long long)(f * 4294967296.0);
 }
@@ -54,9 +57,9 @@ __global__ void k_cell_hist(BuildParams P, const double* __restrict__ pos, unsig
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    unsigned qx = quantize_frac(pos[3 * (size_t)i + 0], P.inv_Lx);
-    unsigned qy = quantize_frac(pos[3 * (size_t)i + 1], P.inv_Ly);
-    unsigned qz = quantize_frac(pos[3 * (size_t)i + 2], P.inv_Lz);
+    unsigned qx = quantize_frac(pos + 3 * (size_t)i, P.Hinv, 0);
+    unsigned qy = quantize_frac(pos + 3 * (size_t)i, P.Hinv, 1);
+    unsigned qz = quantize_frac(pos + 3 * (size_t)i, P.Hinv, 2);
     unsigned c = cell_rank(cell_coord(qx, P.ncx), cell_coord(qy, P.ncy), cell_coord(qz, P.ncz), P.ntx, P.nty);
     cell_of[i] = c;
     rank_in_cell[i] = atomicAdd(&cell_count[c], 1u);
@@ -148,31 +151,45 @@ __global__ void k_sort_cells(int64_t n_cells, const unsigned* __restrict__ cell_
 
 // sorted quantised positions from the caller's fp64 positions (also used every step)
 __global__ void k_quantize(int n, const double* __restrict__ pos, const int* __restrict__ type_orig,
-                           const int* __restrict__ perm, double inv_Lx, double inv_Ly, double inv_Lz,
+                           const int* __restrict__ perm, CellInv inv,
                            int4* __restrict__ posq)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     int i = perm[s];
     int4 q;
-    q.x = (int)quantize_frac(pos[3 * (size_t)i + 0], inv_Lx);
-    q.y = (int)quantize_frac(pos[3 * (size_t)i + 1], inv_Ly);
-    q.z = (int)quantize_frac(pos[3 * (size_t)i + 2], inv_Lz);
+    q.x = (int)quantize_frac(pos + 3 * (size_t)i, inv.m, 0);
+    q.y = (int)quantize_frac(pos + 3 * (size_t)i, inv.m, 1);
+    q.z = (int)quantize_frac(pos + 3 * (size_t)i, inv.m, 2);
     q.w = type_orig[i];
     posq[s] = q;
 }
 
 // ---- 4. list build -----------------------------------------------------------------------------------
-// exact predicate of reading A8, literally: d = (rj - ri) - L*rint((rj - ri)/L);
+// exact predicate of reading A8 (orthorhombic cell), literally: d = (rj - ri) - L*rint((rj - ri)/L);
+// of reading A8t for a general cell;
 // d2 = (dx*dx + dy*dy) + dz*dz; all IEEE fp64 round-to-nearest, no FMA contraction.
 __device__ __forceinline__ double exact_d2(const double* __restrict__ pos, int i, int j, const BuildParams& P)
 {
     double tx = __dsub_rn(pos[3 * (size_t)j + 0], pos[3 * (size_t)i + 0]);
     double ty = __dsub_rn(pos[3 * (size_t)j + 1], pos[3 * (size_t)i + 1]);
     double tz = __dsub_rn(pos[3 * (size_t)j + 2], pos[3 * (size_t)i + 2]);
-    tx = __dsub_rn(tx, __dmul_rn(P.Lx, rint(__ddiv_rn(tx, P.Lx))));
-    ty = __dsub_rn(ty, __dmul_rn(P.Ly, rint(__ddiv_rn(ty, P.Ly))));
-    tz = __dsub_rn(tz, __dmul_rn(P.Lz, rint(__ddiv_rn(tz, P.Lz))));
+    if (!P.tri) {
+        tx = __dsub_rn(tx, __dmul_rn(P.H[0], rint(__ddiv_rn(tx, P.H[0]))));
+        ty = __dsub_rn(ty, __dmul_rn(P.H[4], rint(__ddiv_rn(ty, P.H[4]))));
+        tz = __dsub_rn(tz, __dmul_rn(P.H[8], rint(__ddiv_rn(tz, P.H[8]))));
+    } else {   // reading A8t: n_k = rint(t . Hinv[:,k]); d = ((t - n_a a) - n_b b) - n_c c
+        double nk[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            nk[k] = rint(__dadd_rn(__dadd_rn(__dmul_rn(tx, P.Hinv[k]), __dmul_rn(ty, P.Hinv[3 + k])), __dmul_rn(tz, P.Hinv[6 + k])));
+        const double t[3] = {tx, ty, tz};
+        double d[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            d[a] = __dsub_rn(__dsub_rn(__dsub_rn(t[a], __dmul_rn(nk[0], P.H[a])), __dmul_rn(nk[1], P.H[3 + a])), __dmul_rn(nk[2], P.H[6 + a]));
+        tx = d[0]; ty = d[1]; tz = d[2];
+    }
     return __dadd_rn(__dadd_rn(__dmul_rn(tx, tx), __dmul_rn(ty, ty)), __dmul_rn(tz, tz));
 }
 
@@ -207,9 +224,16 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
                 for (int t = t0; t < t1; ++t) {
                     if (t == s) continue;
                     const int4 pj = posq[t];
-                    float dx = (float)(int)((unsigned)pj.x - (unsigned)pi.x) * P.sx;
-                    float dy = (float)(int)((unsigned)pj.y - (unsigned)pi.y) * P.sy;
-                    float dz = (float)(int)((unsigned)pj.z - (unsigned)pi.z) * P.sz;
+                    const float fa = (float)(int)((unsigned)pj.x - (unsigned)pi.x);
+                    const float fb = (float)(int)((unsigned)pj.y - (unsigned)pi.y);
+                    const float fc = (float)(int)((unsigned)pj.z - (unsigned)pi.z);
+                    float dx, dy, dz;
+                    if (!P.tri) { dx = fa * P.h[0]; dy = fb * P.h[4]; dz = fc * P.h[8]; }
+                    else {
+                        dx = fmaf(fc, P.h[6], fmaf(fb, P.h[3], fa * P.h[0]));
+                        dy = fmaf(fc, P.h[7], fmaf(fb, P.h[4], fa * P.h[1]));
+                        dz = fmaf(fc, P.h[8], fmaf(fb, P.h[5], fa * P.h[2]));
+                    }
                     float r2 = dx * dx + dy * dy + dz * dz;
                     if (r2 >= P.cutR2 + P.guardR) continue;
                     bool inR = r2 < P.cutR2 - P.guardR;

@@ -159,3 +159,84 @@ def test_berendsen_nvt_reaches_target_and_rejects_bad_arguments(pkg, oracle_mod)
     assert abs(oracle_mod.kinetic_temperature(vel.cpu().numpy(), m) - 600.0) < 60.0
     assert nep.nep_max_displacement() < 0.5
     nep.close()
+
+
+# ------------------------------------------------------------------ triclinic cells
+TRI_CASES = [
+    (1, (5, 5, 4), 1.0, (0.21, -0.13, 0.17), "baseline"),      # diamond, 1 species
+    (2, (4, 4, 4), 0.5, (-0.18, 0.11, 0.09), "stress"),        # rock salt, 2 species, rc 6/4
+    (3, (8, 7, 7), 1.0, (0.25, 0.2, -0.22), "stress"),         # fcc alloy, 5 species
+    (4, (10, 9, 9), 0.5, (0.15, -0.1, 0.12), "stress"),        # bcc, rc 6/5, two angular passes
+]
+
+
+def _tri_system(idx, cells, tilt):
+    cfg = W.get_config(idx, cells)
+    s = W.make_system(cfg)
+    pos, H = W.sheared(s, *tilt)
+    return cfg, s, pos, H
+
+
+@pytest.mark.parametrize("idx,cells,skin,tilt,kind", TRI_CASES)
+def test_triclinic_neighbours_and_efw(pkg, oracle_mod, idx, cells, skin, tilt, kind):
+    """Sheared replicas of the configurations: neighbour sets bit-exact against the oracle's reading A8t,
+    E / F / W within north_star's tolerances."""
+    cfg, s, pos, H = _tri_system(idx, cells, tilt)
+    assert W.perpendicular_widths(H).min() >= 2 * (cfg.hyper.rc_radial + skin)
+    p = W.make_params(cfg, kind)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    dpos = torch.tensor(pos, device="cuda:0")
+    nep.nep_neighbors(dpos, torch.tensor(s.types, device="cuda:0"), H, skin)
+    for which, rc in ((0, cfg.hyper.rc_radial), (1, cfg.hyper.rc_angular)):
+        cnt, lst = nep.nep_get_neighbors(which)
+        ocnt, olst = oracle_mod.neighbors(pos, H, rc + skin)
+        cnt, lst = cnt.cpu().numpy(), lst.cpu().numpy()
+        assert np.array_equal(cnt, ocnt)
+        for i in range(len(pos)):
+            assert set(lst[i, :cnt[i]].tolist()) == set(olst[i, :ocnt[i]].tolist())
+    e, f, w = nep.nep_compute(dpos)
+    eo, fo, wo = oracle_mod.compute(cfg.hyper, p, pos, s.types, H)
+    e, f, w = e.cpu().numpy(), f.cpu().numpy(), w.cpu().numpy()
+    assert np.abs(e - eo).max() <= 1e-5
+    fn = np.linalg.norm(fo, axis=1, keepdims=True)
+    assert (np.abs(f - fo) <= np.maximum(1e-4, 1e-4 * fn)).all()
+    assert np.abs(f - fo).max() <= 1e-4 * max(np.abs(fo).max(), 1e-6)
+    wn = np.linalg.norm(wo, axis=1)
+    assert (np.linalg.norm(w - wo, axis=1) <= 1e-4 * np.maximum(wn, np.median(wn))).all()
+    assert np.linalg.norm(w.sum(axis=0) - wo.sum(axis=0)) <= 1e-4 * np.linalg.norm(wo.sum(axis=0))
+    nep.close()
+
+
+def test_triclinic_md_and_equivalent_cell(pkg, oracle_mod):
+    """10 NVE steps in a sheared cell with list rebuilds follow the oracle; and the skewed description
+    (a, b + a, c) of an orthorhombic crystal gives the orthorhombic forces (positions far outside [0,1)^3 in
+    fractional coordinates included)."""
+    cfg, s, pos, H = _tri_system(3, (8, 7, 7), (0.25, 0.2, -0.22))
+    p = W.make_params(cfg, "stress")
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    dpos, dvel = torch.tensor(pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(dpos, torch.tensor(s.types, device="cuda:0"), H, 1.0)
+    nep.md_step(dpos, dvel, 1.0, 10, 3, 1.0)
+    po, vo, ep, ek = oracle_mod.md(cfg.hyper, p, pos, s.vel, s.types, s.masses, H, 1.0, 10)
+    assert np.abs(dpos.cpu().numpy() - po).max() < 3e-6
+    assert np.abs(dvel.cpu().numpy() - vo).max() < 3e-8
+    nep.close()
+
+    cfg = W.get_config(3, (8, 8, 8))
+    s = W.make_system(cfg)
+    H0 = np.diag(s.box)
+    H1 = np.array([H0[0], H0[1] + H0[0], H0[2]])
+    assert W.perpendicular_widths(H1).min() >= 2 * (cfg.hyper.rc_radial + 0.5)
+    rng = np.random.default_rng(11)
+    pos1 = s.pos + rng.integers(-2, 3, size=s.pos.shape).astype(np.float64) @ H0      # any lattice shifts
+    out = []
+    for pp, HH in ((s.pos, s.box), (pos1, H1)):
+        nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+        dp = torch.tensor(pp, device="cuda:0")
+        nep.nep_neighbors(dp, torch.tensor(s.types, device="cuda:0"), HH, 0.5)
+        e, f, w = nep.nep_compute(dp)
+        out.append((e.cpu().numpy(), f.cpu().numpy(), w.cpu().numpy()))
+        nep.close()
+    assert np.abs(out[0][0] - out[1][0]).max() <= 2e-6
+    assert np.abs(out[0][1] - out[1][1]).max() <= 2e-5 * np.abs(out[0][1]).max()
+    assert np.abs(out[0][2] - out[1][2]).max() <= 2e-5 * np.abs(out[0][2]).max()

@@ -169,8 +169,13 @@ def test_errors(pkg):
     with pytest.raises(pkg.NepError) as ei:
         nep.nep_neighbors(pos, types, s.box, 1.0)             # 10.86 < 2 (5 + 1)
     assert ei.value.status == -2
-    box = np.diag(s.box).copy(); box[0, 1] = 0.5
+    box = np.diag(s.box).copy(); box[[0, 1]] = box[[1, 0]]              # left-handed cell: det < 0
     with pytest.raises(pkg.NepError) as ei:
         nep.nep_neighbors(pos, types, box, 0.0)
     assert ei.value.status == -3
+    box = np.diag(s.box).copy(); box[1, 0] = 0.8 * box[0, 0]            # tilt that narrows a perpendicular width below 2 rc
+    box[2, 1] = 2.0 * box[1, 1]
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_neighbors(pos, types, box, 0.0)
+    assert ei.value.status == -2
     nep.close()
