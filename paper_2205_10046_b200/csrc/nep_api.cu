@@ -210,8 +210,13 @@ int build_lists(nep_t* nep, const double* pos_dev)
     for (int attempt = 0; attempt < 4; ++attempt) {
         P.capA = nep->capA; P.capS = nep->capS;
         NEP_CUDA(cudaMemsetAsync(nep->flags, 0, sizeof(int) * 8, st));
-        NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
-                                                    nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
+        if (P.tri) {
+            NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<true><<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
+                                                              nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
+        } else {
+            NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<false><<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
+                                                               nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
+        }
         int fl[8];
         NEP_CUDA(cudaMemcpyAsync(fl, nep->flags, sizeof(fl), cudaMemcpyDeviceToHost, st));
         NEP_CUDA(cudaStreamSynchronize(st));

@@ -169,12 +169,13 @@ __global__ void k_quantize(int n, const double* __restrict__ pos, const int* __r
 // exact predicate of reading A8 (orthorhombic cell), literally: d = (rj - ri) - L*rint((rj - ri)/L);
 // of reading A8t for a general cell;
 // d2 = (dx*dx + dy*dy) + dz*dz; all IEEE fp64 round-to-nearest, no FMA contraction.
+template <bool TRI>
 __device__ __forceinline__ double exact_d2(const double* __restrict__ pos, int i, int j, const BuildParams& P)
 {
     double tx = __dsub_rn(pos[3 * (size_t)j + 0], pos[3 * (size_t)i + 0]);
     double ty = __dsub_rn(pos[3 * (size_t)j + 1], pos[3 * (size_t)i + 1]);
     double tz = __dsub_rn(pos[3 * (size_t)j + 2], pos[3 * (size_t)i + 2]);
-    if (!P.tri) {
+    if (!TRI) {
         tx = __dsub_rn(tx, __dmul_rn(P.H[0], rint(__ddiv_rn(tx, P.H[0]))));
         ty = __dsub_rn(ty, __dmul_rn(P.H[4], rint(__ddiv_rn(ty, P.H[4]))));
         tz = __dsub_rn(tz, __dmul_rn(P.H[8], rint(__ddiv_rn(tz, P.H[8]))));
@@ -193,6 +194,7 @@ __device__ __forceinline__ double exact_d2(const double* __restrict__ pos, int i
     return __dadd_rn(__dadd_rn(__dmul_rn(tx, tx), __dmul_rn(ty, ty)), __dmul_rn(tz, tz));
 }
 
+template <bool TRI>
 __global__ void __launch_bounds__(128)
 k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restrict__ perm,
               const int4* __restrict__ posq, const unsigned* __restrict__ cell_start,
@@ -228,7 +230,7 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
                     const float fb = (float)(int)((unsigned)pj.y - (unsigned)pi.y);
                     const float fc = (float)(int)((unsigned)pj.z - (unsigned)pi.z);
                     float dx, dy, dz;
-                    if (!P.tri) { dx = fa * P.h[0]; dy = fb * P.h[4]; dz = fc * P.h[8]; }
+                    if (!TRI) { dx = fa * P.h[0]; dy = fb * P.h[4]; dz = fc * P.h[8]; }
                     else {
                         dx = fmaf(fc, P.h[6], fmaf(fb, P.h[3], fa * P.h[0]));
                         dy = fmaf(fc, P.h[7], fmaf(fb, P.h[4], fa * P.h[1]));
@@ -241,7 +243,7 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
                     const bool nearR = !inR;                                    // within the R guard band
                     const bool nearA = !inA && r2 < P.cutA2 + P.guardA;
                     if (nearR || nearA) {
-                        double d2 = exact_d2(pos, perm[s], perm[t], P);
+                        double d2 = exact_d2<TRI>(pos, perm[s], perm[t], P);
                         inR = d2 < P.cutR2_d;
                         inA = d2 < P.cutA2_d;
                     }
