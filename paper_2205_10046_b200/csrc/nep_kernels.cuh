@@ -132,63 +132,76 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
         pair_vec(posq_build[s], pi, D, dx, dy, dz, r2);
         if (r2 > 0.0f) atomicMax(disp_max, __float_as_uint(r2));
     }
-    int na = 0, nb = 0;
+    // Branch-free inner loops: the write pointers of the two compact columns advance by n under a predicate,
+    // the mask bit of the current slot is shifted along, list / rev pointers step by 4 n per batch.
     ulonglong2* rec = reinterpret_cast<ulonglong2*>(mask) + (size_t)s * (2 * D.maskW);
-    const int ca = cntA[s];
-    for (int w = 0; w < D.maskW; ++w) {
-        unsigned long long wa = 0ull, wb = 0ull;
-        const int mend = min(ca, 64 * (w + 1));
-        for (int m0 = 64 * w; m0 < mend; m0 += 4) {          // 4 independent gathers in flight
-            int j[4], rs[4]; int4 pj[4];
+    int* pa = cA + s;
+    int* pb = cB + s;
+    int na = 0, nb = 0;
+    const size_t n4 = 4 * n;
+    {
+        const int ca = cntA[s];
+        const int* lp = listA + s;
+        const unsigned char* rp = rev + s;
+        for (int w = 0; w < D.maskW; ++w) {
+            unsigned long long wa = 0ull, wb = 0ull, bit = 1ull;
+            const int mend = min(ca, 64 * (w + 1));
+            for (int m0 = 64 * w; m0 < mend; m0 += 4) {          // 4 independent gathers in flight
+                int j[4], rs[4]; int4 pj[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const bool ok = m0 + u < mend;
-                j[u] = ok ? listA[(size_t)(m0 + u) * n + s] : s;
-                rs[u] = ok ? rev[(size_t)(m0 + u) * n + s] : 0;
-            }
+                for (int u = 0; u < 4; ++u) {
+                    const bool ok = m0 + u < mend;
+                    j[u] = ok ? lp[u * n] : s;
+                    rs[u] = ok ? rp[u * n] : 0;
+                }
+                lp += n4; rp += n4;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+                for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (m0 + u < mend) {
+                for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
                     pair_vec(pi, pj[u], D, dx, dy, dz, r2);
                     const int e = (j[u] << NEP_SLOT_BITS) | rs[u];
-                    if (r2 < D.rcA2) { cA[(size_t)na * n + s] = e; ++na; wa |= 1ull << ((m0 + u) & 63); }
-                    else if (r2 < D.rcR2) { cB[(size_t)nb * n + s] = e; ++nb; wb |= 1ull << ((m0 + u) & 63); }
+                    const bool ok = m0 + u < mend;
+                    const bool inA = ok && r2 < D.rcA2;
+                    const bool inB = ok && !inA && r2 < D.rcR2;
+                    if (inA) { *pa = e; pa += n; ++na; wa |= bit; }
+                    if (inB) { *pb = e; pb += n; ++nb; wb |= bit; }
+                    bit <<= 1;
                 }
             }
+            rec[w] = make_ulonglong2(wa, wb);
         }
-        rec[w] = make_ulonglong2(wa, wb);
     }
     const unsigned long long nouter = (unsigned long long)nb;
-    const int cs = cntS[s];
-    for (int w = 0; w < D.maskW; ++w) {
-        unsigned long long ws = 0ull;
-        const int mend = min(cs, 64 * (w + 1));
-        for (int m0 = 64 * w; m0 < mend; m0 += 4) {
-            int j[4], rs[4]; int4 pj[4];
+    {
+        const int cs = cntS[s];
+        const int* lp = listS + s;
+        const unsigned char* rp = revS + s;
+        for (int w = 0; w < D.maskW; ++w) {
+            unsigned long long ws = 0ull, bit = 1ull;
+            const int mend = min(cs, 64 * (w + 1));
+            for (int m0 = 64 * w; m0 < mend; m0 += 4) {
+                int j[4], rs[4]; int4 pj[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const bool ok = m0 + u < mend;
-                j[u] = ok ? listS[(size_t)(m0 + u) * n + s] : s;
-                rs[u] = ok ? revS[(size_t)(m0 + u) * n + s] : 0;
-            }
+                for (int u = 0; u < 4; ++u) {
+                    const bool ok = m0 + u < mend;
+                    j[u] = ok ? lp[u * n] : s;
+                    rs[u] = ok ? rp[u * n] : 0;
+                }
+                lp += n4; rp += n4;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+                for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (m0 + u < mend) {
+                for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
                     pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                    if (r2 < D.rcR2) {
-                        cB[(size_t)nb * n + s] = (j[u] << NEP_SLOT_BITS) | rs[u]; ++nb;
-                        ws |= 1ull << ((m0 + u) & 63);
-                    }
+                    if (m0 + u < mend && r2 < D.rcR2) { *pb = (j[u] << NEP_SLOT_BITS) | rs[u]; pb += n; ++nb; ws |= bit; }
+                    bit <<= 1;
                 }
             }
+            rec[D.maskW + w] = make_ulonglong2(ws, nouter);
         }
-        rec[D.maskW + w] = make_ulonglong2(ws, nouter);
     }
     ncA[s] = na;
     ncB[s] = nb;
