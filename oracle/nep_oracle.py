@@ -291,3 +291,57 @@ def md_berendsen(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_st
         t_before[s - 1] = T
         t_after[s - 1] = kinetic_temperature(vel, m_atom)
     return pos, vel, t_before, t_after
+
+
+# ---- Langevin thermostat (reading A16) ---------------------------------------------------------
+_M64 = (1 << 64) - 1
+
+
+def counter_normal(seed: int, counter: int) -> float:
+    """Standard normal deviate number `counter` of stream `seed` -- the counter-based generator both sides
+    implement (reading A16): two SplitMix64 outputs x = mix(seed + (2 counter + h) * 0x9E3779B97F4A7C15),
+    h = 0, 1 (mix = the SplitMix64 finaliser of Steele, Lea & Flood), uniforms u = ((x >> 11) + 0.5) 2^-53 in
+    (0, 1), Box-Muller z = sqrt(-2 ln u_0) cos(2 pi u_1)."""
+    u = []
+    for h in (0, 1):
+        z = (seed + (2 * counter + h) * 0x9E3779B97F4A7C15) & _M64
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & _M64
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & _M64
+        z = z ^ (z >> 31)
+        u.append(((z >> 11) + 0.5) * (1.0 / 9007199254740992.0))
+    return float(np.sqrt(-2.0 * np.log(u[0])) * np.cos(2.0 * np.pi * u[1]))
+
+
+def langevin_half_step(vel, masses_per_atom, t_target: float, c1: float, seed: int, draw: int):
+    """v <- c1 v + sqrt(1 - c1^2) sqrt(k_B T / m) R for every component; R = counter_normal(seed,
+    (draw * n + i) * 3 + a) for atom i (caller's order), component a, and `draw` the running number of
+    the thermostat application (two per MD step)."""
+    v, m = _d(vel).copy(), _d(masses_per_atom)
+    n = len(m)
+    c2 = np.sqrt(1.0 - c1 * c1)
+    for i in range(n):
+        sig = np.sqrt(KB_EV_PER_K * t_target / m[i] * ACC_CONV)
+        for a in range(3):
+            v[i, a] = c1 * v[i, a] + c2 * sig * counter_normal(seed, (draw * n + i) * 3 + a)
+    return v
+
+
+def md_langevin(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int,
+                t_start: float, t_stop: float, tau_fs: float, seed: int, first_step: int = 0, pbc=(1, 1, 1)):
+    """NVT with the Langevin thermostat (named PAPER.md:318, `nvt_lan` PAPER.md:574-590; the paper cites
+    Bussi & Parrinello, ref. 80 PAPER.md:1227, and prints no equation: DESIGN.md reading A16).  Step s =
+    first_step .. first_step + n_steps - 1: thermostat half step (draw 2 s), one velocity-Verlet step of md(),
+    thermostat half step (draw 2 s + 1); c1 = exp(-dt / (2 tau)); the target temperature of the (s - first_step
+    + 1)-th step of the call ramps linearly like md_berendsen's.  Returns (pos, vel, T[n_steps]) with T after each step."""
+    pos, vel = _d(pos).copy(), _d(vel).copy()
+    m_atom = _d(masses)[np.ascontiguousarray(types, dtype=np.int32)]
+    c1 = float(np.exp(-dt_fs / (2.0 * tau_fs)))
+    temps = np.zeros(n_steps)
+    for k in range(n_steps):
+        s = first_step + k
+        t_target = t_start + (t_stop - t_start) * (k + 1) / n_steps
+        vel = langevin_half_step(vel, m_atom, t_target, c1, seed, 2 * s)
+        pos, vel, _, _ = md(hyper, params, pos, vel, types, masses, box, dt_fs, 1, pbc=pbc)
+        vel = langevin_half_step(vel, m_atom, t_target, c1, seed, 2 * s + 1)
+        temps[k] = kinetic_temperature(vel, m_atom)
+    return pos, vel, temps

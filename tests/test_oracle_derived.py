@@ -231,3 +231,51 @@ def test_triclinic_forces_and_shear_virial_by_finite_differences(oracle_mod):
         Fp, Fm = (np.eye(3) + eps).T, (np.eye(3) - eps).T
         dE = (E(pos @ Fp, H @ Fp) - E(pos @ Fm, H @ Fm)) / (2 * h)
         assert wtot[a, b] == pytest.approx(-dE, rel=5e-6, abs=1e-8)
+
+
+# ------------------------------------------------------------------ Langevin NVT (reading A16)
+def test_counter_normal_statistics_and_independence(oracle_mod):
+    z = np.array([oracle_mod.counter_normal(20220510, c) for c in range(200000)])
+    n = len(z)
+    assert abs(z.mean()) < 4.0 / np.sqrt(n)
+    assert abs(z.var() - 1.0) < 4.0 * np.sqrt(2.0 / n)
+    assert abs((z ** 3).mean()) < 4.0 * np.sqrt(15.0 / n)
+    assert abs((z ** 4).mean() - 3.0) < 4.0 * np.sqrt(96.0 / n)
+    assert abs(np.mean(z[:-1] * z[1:])) < 4.0 / np.sqrt(n)                 # neighbouring counters uncorrelated
+    assert abs(np.mean(z[:-3] * z[3:])) < 4.0 / np.sqrt(n)                 # ... and the 3 components of an atom
+    # the Kolmogorov distance to the normal distribution
+    from scipy import stats
+    assert stats.kstest(z, "norm").statistic < 1.63 / np.sqrt(n) * 1.5
+    z2 = np.array([oracle_mod.counter_normal(20220511, c) for c in range(50000)])
+    assert abs(np.mean(z[:50000] * z2)) < 4.0 / np.sqrt(50000)             # another seed: another stream
+    assert oracle_mod.counter_normal(7, 12345) == oracle_mod.counter_normal(7, 12345)
+
+
+def test_langevin_limits_and_free_particle_relaxation(oracle_mod):
+    cfg = W.get_config(3, cells=(3, 3, 3))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    args = (cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box)
+    m_atom = s.masses[s.types]
+    # tau -> infinity: c1 = 1, c2 = 0: the pinned NVE trajectory
+    pos_n, vel_n, _, _ = oracle_mod.md(*args, 1.0, 4)
+    pos_l, vel_l, _ = oracle_mod.md_langevin(*args, 1.0, 4, 900.0, 900.0, 1e30, seed=5)
+    np.testing.assert_allclose(pos_l, pos_n, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(vel_l, vel_n, rtol=0, atol=1e-14)
+    # one half step: exactly c1 v + c2 sigma R with the documented counters
+    c1 = 0.8
+    v1 = oracle_mod.langevin_half_step(s.vel, m_atom, 500.0, c1, seed=9, draw=3)
+    n = len(m_atom)
+    for i, a in ((0, 0), (5, 2), (n - 1, 1)):
+        sig = np.sqrt(oracle_mod.KB_EV_PER_K * 500.0 / m_atom[i] * oracle_mod.ACC_CONV)
+        want = c1 * s.vel[i, a] + np.sqrt(1 - c1 * c1) * sig * oracle_mod.counter_normal(9, (3 * n + i) * 3 + a)
+        assert v1[i, a] == pytest.approx(want, rel=1e-14)
+    # free particles (zero model): E[T_{k+1}] = c1^4 T_k + (1 - c1^4) T0 per full step (two half steps);
+    # the kinetic temperature of 3N independent components fluctuates by T sqrt(2 / 3N)
+    cfg0 = W.get_config(1, cells=(5, 5, 5))
+    s0, p0 = W.make_system(cfg0), _zero_model(cfg0)
+    dt, tau, T0, nst = 2.0, 8.0, 900.0, 10
+    _, _, temps = oracle_mod.md_langevin(cfg0.hyper, p0, s0.pos, s0.vel, s0.types, s0.masses, s0.box, dt, nst, T0, T0, tau, seed=1)
+    c4 = np.exp(-dt / (2 * tau)) ** 4
+    want = T0 + (cfg0.temperature - T0) * c4 ** np.arange(1, nst + 1)
+    assert (np.abs(temps - want) < 5.0 * want * np.sqrt(2.0 / (3 * len(s0.pos)))).all()
+    assert temps[-1] > 2.5 * cfg0.temperature
