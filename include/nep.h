@@ -136,6 +136,18 @@ int md_step_nvt_berendsen(nep_t* nep, double* pos_dev, double* vel_dev, double d
                           int32_t rebuild_every, double skin, double t_start_K, double t_stop_K, double tau_fs);
 int nep_last_temperature(nep_t* nep, double* t_before_host, double* lambda_host);
 
+/* ---- NVT: velocity-Verlet + Langevin thermostat (named PAPER.md:318, `nvt_lan` PAPER.md:574-590, refs.
+ * 80-81; equations per DESIGN.md reading A16).  Every MD step s = first_step .. first_step + n_steps - 1 is:
+ * thermostat half step, the velocity-Verlet step of md_step, thermostat half step; a half step replaces every
+ * velocity component by c1 v + sqrt(1 - c1^2) sqrt(k_B T_target / m) R with c1 = exp(-dt_fs / (2 tau_fs)) and R
+ * the counter-based standard normal deviate of reading A16 (seed; counter from the step number, the atom's
+ * index in the caller's order and the component), so a trajectory is reproducible and independent of how the
+ * steps are split over calls (pass first_step = steps done so far).  T_target ramps as in
+ * md_step_nvt_berendsen.  NEP_ERR_INVALID_ARG if tau_fs <= 0, a temperature < 0 or first_step < 0.        */
+int md_step_nvt_langevin(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps,
+                         int32_t rebuild_every, double skin, double t_start_K, double t_stop_K, double tau_fs,
+                         uint64_t seed, int64_t first_step);
+
 /* Results of the most recent internal evaluation (the one md_step ended with, or nep_compute):
  * same layouts as nep_compute; any pointer may be NULL.  Does not synchronise.                        */
 int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* virial_dev);

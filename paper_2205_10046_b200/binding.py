@@ -20,7 +20,7 @@ exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
-    "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature",
+    "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
@@ -93,6 +93,8 @@ def load_library():
     L.nep_get_angular_sums.argtypes = [vp, vp]
     L.md_step_nvt_berendsen.restype = C.c_int
     L.md_step_nvt_berendsen.argtypes = [vp, vp, vp, dbl, i32, i32, dbl, dbl, dbl, dbl]
+    L.md_step_nvt_langevin.restype = C.c_int
+    L.md_step_nvt_langevin.argtypes = [vp, vp, vp, dbl, i32, i32, dbl, dbl, dbl, dbl, C.c_uint64, i64]
     L.nep_last_temperature.restype = C.c_int
     L.nep_last_temperature.argtypes = [vp, dp, dp]
     L.nep_get_latent.restype = C.c_int
@@ -246,6 +248,15 @@ class NEP:
                                                   self._dev(vel, torch.float64, 3 * n), float(dt_fs), int(n_steps),
                                                   int(rebuild_every), float(skin), float(t_start), float(t_stop),
                                                   float(tau_fs)))
+
+    def md_step_nvt_langevin(self, pos, vel, dt_fs: float, n_steps: int, rebuild_every: int, skin: float,
+                             t_start: float, t_stop: float, tau_fs: float, seed: int, first_step: int = 0):
+        torch = self._torch
+        n = self.n
+        self._check(self._L.md_step_nvt_langevin(self._h_ptr, self._dev(pos, torch.float64, 3 * n),
+                                                 self._dev(vel, torch.float64, 3 * n), float(dt_fs), int(n_steps),
+                                                 int(rebuild_every), float(skin), float(t_start), float(t_stop),
+                                                 float(tau_fs), int(seed), int(first_step)))
 
     def nep_last_temperature(self):
         """(T before the rescale, lambda) of the last thermostatted step."""

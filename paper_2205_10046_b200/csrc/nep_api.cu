@@ -822,10 +822,12 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
     return nep_get_last(nep, energy_dev, force_dev, virial_dev);
 }
 
-// thermostat of md_loop: none (NVE) or Berendsen (reading A15)
+// thermostat of md_loop: none (NVE), Berendsen (reading A15) or Langevin (reading A16)
 struct Thermostat {
-    bool on;
+    int kind;                 // 0 none, 1 Berendsen, 2 Langevin
     double t_start, t_stop, tau_fs;
+    unsigned long long seed;
+    int64_t first_step;
 };
 
 static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
@@ -834,7 +836,7 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
     if (!nep) return NEP_ERR_INVALID_ARG;
     if (!pos_dev || !vel_dev || n_steps < 0 || rebuild_every < 1 || !(skin >= 0.0) || !(dt_fs == dt_fs))
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad md_step argument");
-    if (th.on && (!(th.tau_fs > 0.0) || !(th.t_start >= 0.0) || !(th.t_stop >= 0.0)))
+    if (th.kind && (!(th.tau_fs > 0.0) || !(th.t_start >= 0.0) || !(th.t_stop >= 0.0)))
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad thermostat argument");
     if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
     NEP_CUDA(cudaSetDevice(nep->device));
@@ -852,19 +854,26 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
     const double hdt = 0.5 * dt_fs * kAccConv;
     const int TB = 256;
     const int nb = div_up(n, 256);
-    if (th.on && nb + 2 > nep->thermo_cap) {
+    if (th.kind == 1 && nb + 2 > nep->thermo_cap) {
         nep->thermo_cap = 0;
         NEP_TRY(dev_alloc(nep, &nep->thermo, (size_t)nb + 2));
         nep->thermo_cap = nb + 2;
     }
+    const double lc1 = th.kind == 2 ? exp(-dt_fs / (2.0 * th.tau_fs)) : 1.0, lc2 = sqrt(1.0 - lc1 * lc1);
     for (int s = 0; s < n_steps; ++s) {
+        const double t_target = th.kind ? th.t_start + (th.t_stop - th.t_start) * (double)(s + 1) / (double)n_steps : 0.0;
+        if (th.kind == 2)
+            NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
+                                                      2ull * (unsigned long long)(th.first_step + s), nep->type_orig, nep->mass_dev, vel_dev));
         NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
         NEP_TRY(evaluate(nep, pos_dev));
         NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
-        if (th.on) {
-            const double t_target = th.t_start + (th.t_stop - th.t_start) * (double)(s + 1) / (double)n_steps;
+        if (th.kind == 2)
+            NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
+                                                      2ull * (unsigned long long)(th.first_step + s) + 1ull, nep->type_orig, nep->mass_dev, vel_dev));
+        if (th.kind == 1) {
             double* lam = nep->thermo + (nep->thermo_cap - 2);
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_mv2_partial<<<nb, 256, 0, st>>>(n, nep->type_orig, nep->mass_dev, vel_dev, nep->thermo));
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_berendsen_lambda<<<1, 256, 0, st>>>(nb, nep->thermo, 1.0 / (kAccConv * 3.0 * (double)n * kBoltzmann),
@@ -879,14 +888,22 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
 
 int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every, double skin)
 {
-    const Thermostat none = {false, 0.0, 0.0, 0.0};
+    const Thermostat none = {0, 0.0, 0.0, 0.0, 0ull, 0};
     return md_loop(nep, pos_dev, vel_dev, dt_fs, n_steps, rebuild_every, skin, none);
 }
 
 int md_step_nvt_berendsen(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
                           double skin, double t_start_K, double t_stop_K, double tau_fs)
 {
-    const Thermostat th = {true, t_start_K, t_stop_K, tau_fs};
+    const Thermostat th = {1, t_start_K, t_stop_K, tau_fs, 0ull, 0};
+    return md_loop(nep, pos_dev, vel_dev, dt_fs, n_steps, rebuild_every, skin, th);
+}
+
+int md_step_nvt_langevin(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
+                         double skin, double t_start_K, double t_stop_K, double tau_fs, uint64_t seed, int64_t first_step)
+{
+    if (first_step < 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad thermostat argument");
+    const Thermostat th = {2, t_start_K, t_stop_K, tau_fs, (unsigned long long)seed, first_step};
     return md_loop(nep, pos_dev, vel_dev, dt_fs, n_steps, rebuild_every, skin, th);
 }
 

@@ -1397,6 +1397,35 @@ k_berendsen_lambda(int nblocks, const double* __restrict__ partial, double inv_c
     }
 }
 
+// Langevin thermostat half step (reading A16): v <- c1 v + c2 sqrt(k_B T / m) R per component,
+// R a counter-based standard normal deviate: SplitMix64 finaliser of seed + (2 c + h) * 0x9E3779B97F4A7C15,
+// h = 0, 1 -> u = ((x >> 11) + 1/2) 2^-53 -> Box-Muller; counter c = (draw * n + i) * 3 + a.
+__device__ __forceinline__ unsigned long long splitmix_mix(unsigned long long z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+__device__ __forceinline__ double counter_normal(unsigned long long seed, unsigned long long c)
+{
+    const unsigned long long x0 = splitmix_mix(seed + (2ull * c) * 0x9E3779B97F4A7C15ull);
+    const unsigned long long x1 = splitmix_mix(seed + (2ull * c + 1ull) * 0x9E3779B97F4A7C15ull);
+    const double u0 = ((double)(x0 >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+    const double u1 = ((double)(x1 >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+    return sqrt(-2.0 * log(u0)) * cos(2.0 * 3.14159265358979323846 * u1);
+}
+
+__global__ void k_langevin_half(int n, double c1, double c2, double kt_conv, unsigned long long seed, unsigned long long draw,
+                                const int* __restrict__ type, const double* __restrict__ mass, double* __restrict__ vel)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 3 * n) return;
+    const int i = t / 3;
+    const double sig = sqrt(kt_conv / mass[type[i]]);             // sqrt(k_B T conv / m), Angstrom / fs
+    vel[t] = c1 * vel[t] + c2 * sig * counter_normal(seed, draw * (unsigned long long)n * 3ull + (unsigned long long)t);
+}
+
 __global__ void k_scale_velocities(int n3, const double* __restrict__ lambda, double* __restrict__ vel)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;

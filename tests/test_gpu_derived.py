@@ -240,3 +240,60 @@ def test_triclinic_md_and_equivalent_cell(pkg, oracle_mod):
     assert np.abs(out[0][0] - out[1][0]).max() <= 2e-6
     assert np.abs(out[0][1] - out[1][1]).max() <= 2e-5 * np.abs(out[0][1]).max()
     assert np.abs(out[0][2] - out[1][2]).max() <= 2e-5 * np.abs(out[0][2]).max()
+
+
+# ------------------------------------------------------------------ Langevin NVT (reading A16)
+@pytest.mark.parametrize("idx,cells,skin,kind", [(0, None, 0.0, "baseline"), (3, (7, 6, 5), 1.0, "stress")])
+def test_langevin_nvt_trajectory(pkg, oracle_mod, idx, cells, skin, kind):
+    """Same seed and counters on both sides: the thermostatted trajectories agree like the NVE ones (the
+    normal deviates differ by fp64 round-off of log / cos only).  Splitting the run over two calls with
+    first_step continues the same random stream."""
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s, p = W.make_system(cfg), W.make_params(cfg, kind)
+    n_steps, t0, t1, tau, seed = 8, 400.0, 700.0, 40.0, 20220510
+    po, vo, temps = oracle_mod.md_langevin(cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box, cfg.dt_fs, n_steps, t0, t1, tau, seed)
+    tol = 1.0 if kind == "baseline" else 30.0
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    nep.md_step_nvt_langevin(pos, vel, cfg.dt_fs, n_steps, cfg.rebuild_every, skin, t0, t1, tau, seed)
+    assert np.abs(pos.cpu().numpy() - po).max() < 1e-7 * tol
+    assert np.abs(vel.cpu().numpy() - vo).max() < 1e-9 * tol
+    m = s.masses[s.types]
+    assert oracle_mod.kinetic_temperature(vel.cpu().numpy(), m) == pytest.approx(temps[-1], rel=1e-6)
+    nep.close()
+    # two calls of 4 steps with a constant target == one call of 8 (first_step continues the counters)
+    ref = oracle_mod.md_langevin(cfg.hyper, p, s.pos, s.vel, s.types, s.masses, s.box, cfg.dt_fs, 8, 500.0, 500.0, tau, seed)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    nep.md_step_nvt_langevin(pos, vel, cfg.dt_fs, 4, cfg.rebuild_every, skin, 500.0, 500.0, tau, seed, 0)
+    nep.md_step_nvt_langevin(pos, vel, cfg.dt_fs, 4, cfg.rebuild_every, skin, 500.0, 500.0, tau, seed, 4)
+    assert np.abs(pos.cpu().numpy() - ref[0]).max() < 1e-7 * tol
+    assert np.abs(vel.cpu().numpy() - ref[1]).max() < 1e-9 * tol
+    nep.close()
+
+
+def test_langevin_normal_deviates_and_equilibrium(pkg, oracle_mod):
+    """tau << dt resamples every velocity: v = sqrt(k_B T / m) R exactly, which exposes the device generator
+    deviate by deviate against the oracle's; and a long run samples the target temperature."""
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.vel, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 1.0)
+    n, m = len(s.pos), s.masses[s.types]
+    nep.md_step_nvt_langevin(pos, vel, 1.0, 1, 10, 1.0, 650.0, 650.0, 1e-3, 77, 5)     # c1 = exp(-500) = 0
+    sig = np.sqrt(oracle_mod.KB_EV_PER_K * 650.0 / m * oracle_mod.ACC_CONV)
+    z = vel.cpu().numpy() / sig[:, None]
+    for i, a in ((0, 0), (1, 2), (417, 1), (n - 1, 2)):
+        assert z[i, a] == pytest.approx(oracle_mod.counter_normal(77, ((2 * 5 + 1) * n + i) * 3 + a), rel=1e-12, abs=1e-14)
+    assert abs(z.mean()) < 4.0 / np.sqrt(3 * n) and abs(z.var() - 1.0) < 4.0 * np.sqrt(2.0 / (3 * n))
+    for bad in ((300.0, 300.0, 0.0, 1, 0), (-1.0, 300.0, 10.0, 1, 0), (300.0, 300.0, 10.0, 1, -1)):
+        with pytest.raises(pkg.NepError) as ei:
+            nep.md_step_nvt_langevin(pos, vel, 1.0, 1, 10, 1.0, *bad)
+        assert ei.value.status == -1
+    nep.md_step_nvt_langevin(pos, vel, 1.0, 200, 10, 1.0, 650.0, 650.0, 25.0, 78, 6)
+    t_end = oracle_mod.kinetic_temperature(vel.cpu().numpy(), m)
+    assert abs(t_end - 650.0) < 6.0 * 650.0 * np.sqrt(2.0 / (3 * n)) + 30.0
+    nep.close()
