@@ -682,7 +682,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
             if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); delete nep; return NEP_ERR_CUDA; }
             nep->num_sms = prop.multiProcessorCount;
         }
-        auto stride_of = [&](int nch) { return 4 * (((d.KAR * round_up4(nch)) / 4) | 1); };
+        auto stride_of = [&](int nch) { return (d.KAR * round_up4(nch)) | 1; };
         const int npass = (d.NA + nep->nch_max - 1) / nep->nch_max;
         const int base = d.NA / npass, rem = d.NA % npass;
         nep->angular_tab_smem = sizeof(float) * (size_t)TT * stride_of(base + (rem ? 1 : 0)) <= kSmemTableMax;

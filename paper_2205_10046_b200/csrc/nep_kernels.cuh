@@ -437,16 +437,16 @@ __device__ __forceinline__ void q_from_S(const float* S, const NepCoef& C, float
 // KAR rows of NCHP = round_up4(NCH) floats.  Row 0 holds csum'_n = 2 c_{n0} + sum_{k>=1} c_{nk}, row k
 // (1 <= k < KA) holds c_{nk}, rows KA..KAR-1 are zero (KAR - 1 is a multiple of 4 so that the k loop
 // unrolls by 4).  Then   g_n(r) = (f_c/2) [ csum'_n + sum_{k>=1} c_nk T_k(x) ]            (Eqs. 3-4)
-// The type-pair stride is an odd number of float4, so rows are 16-byte aligned (128-bit loads) and the
-// lanes of a warp -- which differ in tp -- fall into different bank groups.
+// The type-pair stride is an odd number of floats and a row is read with NCH scalar loads: lanes that differ
+// in tp hit different banks, lanes with the same tp the same word (broadcast), so every load is one
+// wavefront.  (128-bit row loads need fewer instructions but 7 wavefronts per load here -- the 8 lanes of a
+// quarter warp share 8 bank groups among up to 25 type pairs -- and this kernel is bound by that pipe.)
 // SM = true: the table is staged in shared memory; false: read from global memory (huge tables).
 template <bool SM>
 __device__ __forceinline__ const float* stage_table(const float* __restrict__ tab_g, int count, float* sc)
 {
     if (SM) {
-        const float4* g4 = reinterpret_cast<const float4*>(tab_g);
-        float4* s4 = reinterpret_cast<float4*>(sc);
-        for (int t = threadIdx.x; t < count / 4; t += blockDim.x) s4[t] = g4[t];
+        for (int t = threadIdx.x; t < count; t += blockDim.x) sc[t] = tab_g[t];
         __syncthreads();
         return sc;
     }
@@ -454,13 +454,10 @@ __device__ __forceinline__ const float* stage_table(const float* __restrict__ ta
 }
 
 template <int NCH>
-__device__ __forceinline__ void load_row(const float4* __restrict__ row, float* c)
+__device__ __forceinline__ void load_row(const float* __restrict__ row, float* c)
 {
 #pragma unroll
-    for (int q4 = 0; q4 < (NCH + 3) / 4; ++q4) {
-        const float4 v = row[q4];
-        c[4 * q4 + 0] = v.x; c[4 * q4 + 1] = v.y; c[4 * q4 + 2] = v.z; c[4 * q4 + 3] = v.w;
-    }
+    for (int a = 0; a < NCH; ++a) c[a] = row[a];
 }
 
 // Warps take 32-atom tiles from a global counter (dynamic, in spatial order): the coefficient table is
@@ -494,7 +491,7 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<false>(r, D.rcA_inv);
-        const float4* c4 = reinterpret_cast<const float4*>(tab_i + w.pj.w * tab_stride);
+        const float* c4 = tab_i + w.pj.w * tab_stride;
         float g[4 * N4];
         load_row<NCH>(c4, g);                              // csum'
         float Tkm1 = 1.0f, Tk = h.x;
@@ -502,7 +499,7 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 float c[4 * N4];
-                load_row<NCH>(c4 + (r0 + u) * N4, c);
+                load_row<NCH>(c4 + (r0 + u) * (4 * N4), c);
 #pragma unroll
                 for (int a = 0; a < NCH; ++a) g[a] = fmaf(c[a], Tk, g[a]);
                 const float Tn = fmaf(h.two_x, Tk, -Tkm1);
@@ -840,7 +837,7 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         pair_vec(pi, w.pj, D, dx, dy, dz, r2);
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<true>(r, D.rcA_inv);
-        const float4* c4 = reinterpret_cast<const float4*>(tab_i + w.pj.w * tab_stride);
+        const float* c4 = tab_i + w.pj.w * tab_stride;
         float g[4 * N4], dg[NCH];
         load_row<NCH>(c4, g);                              // csum'
 #pragma unroll
@@ -851,7 +848,7 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     float c[4 * N4];
-                    load_row<NCH>(c4 + (r0 + u) * N4, c);
+                    load_row<NCH>(c4 + (r0 + u) * (4 * N4), c);
 #pragma unroll
                     for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
                     const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
