@@ -146,6 +146,18 @@ def measured_peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def measured_tf32_peak():
+    """Dense TF32 tensor peak in TFLOP/s for the network kernel (k_ann_tc): the measured bf16 figure of
+    MEASURED_PEAKS.json times the nominal TF32 : bf16 ratio 1/2 (B200_PROFILING.md), else half the guide's
+    fallback (the kernel is timed inside a long step: the sustained figure)."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return 0.5 * float(json.load(f)["bf16_tflops_sustained"]), "of measured: sustained bf16 x 1/2 (MEASURED_PEAKS.json)"
+    except (OSError, KeyError, ValueError):
+        return 0.5 * 1400.0, "of fallback: sustained bf16 1.4 PFLOP/s x 1/2 (B200_PROFILING.md)"
+
+
 def ncu_traffic(workload: str):
     """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this workload:
     profiles/traffic_<workload>.csv with lines `kernel,dram_bytes_per_launch`."""
@@ -353,6 +365,12 @@ def run_ours(args):
             entry.update({"tflops": fl / avg_s / 1e12, "alu_frac": fl / avg_s / 1e12 / alu_peak,
                           "gbs": by / avg_s / 1e9, "hbm_frac": by / avg_s / 1e9 / hbm_peak,
                           "flops_per_launch": fl, "bytes_per_launch": by})
+        if name == "ann" and "tflops" in entry:
+            # the network runs on the tensor cores (3xTF32 mma.sync): its contraction peak is the TF32 one;
+            # algorithmic flops are counted once (the split issues three MMAs per product)
+            tf32_peak, tf32_src = measured_tf32_peak()
+            entry.update({"tensor_frac": entry["tflops"] / tf32_peak, "tensor_peak_tflops": tf32_peak,
+                          "tensor_peak_source": tf32_src})
         kernels.append(entry)
     top = next((k for k in kernels if "tflops" in k), None)
     roofline = None
