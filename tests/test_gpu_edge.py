@@ -196,6 +196,44 @@ def test_more_species_than_the_register_kernels_take(pkg, oracle_mod):
     run_both(pkg, oracle_mod, hy, p, s.masses, s.pos, s.types, s.box, skin=0.5)
 
 
+def test_tables_too_large_for_shared_memory(pkg, oracle_mod):
+    """Twelve species with 32 basis functions: the type-pair coefficient tables (148 / 152 KB) stay in global
+    memory (k_angular / k_force_angular <4, false> in passes of four channels, the radial kernels' TAB_SM =
+    false) and the per-thread radial tables force 32-thread blocks."""
+    base = W.get_config(2, (3, 3, 3))
+    hy = W.Hyper(n_types=12, rc_radial=6.0, rc_angular=4.0, n_max_radial=7, n_max_angular=5, basis_radial=31,
+                 basis_angular=31, n_neurons=16)
+    cfg = replace(base, hyper=hy, masses=tuple(20.0 + 3.0 * t for t in range(12)), species_rule="random")
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    run_both(pkg, oracle_mod, hy, p, s.masses, s.pos, s.types, s.box, skin=0.5)
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_models_and_cells(pkg, oracle_mod, seed):
+    """Seeded fuzz over the template space: species, channel and basis counts, neurons, many-body blocks,
+    orthorhombic or sheared cell, skin."""
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 904, seed]))
+    T = int(rng.integers(1, 7))
+    hy = W.Hyper(n_types=T, rc_radial=float(rng.uniform(4.5, 6.0)), rc_angular=float(rng.uniform(3.0, 4.5)),
+                 n_max_radial=int(rng.integers(0, 13)), n_max_angular=int(rng.integers(0, 11)),
+                 basis_radial=int(rng.integers(0, 17)), basis_angular=int(rng.integers(0, 17)),
+                 n_neurons=int(rng.integers(1, 70)), l_max_4b=int(rng.choice([0, 2])), l_max_5b=int(rng.choice([0, 1])))
+    base = W.get_config(int(rng.choice([1, 2, 3])), tuple(int(c) for c in rng.integers(4, 6, size=3)))
+    cfg = replace(base, hyper=hy, masses=tuple(float(m) for m in rng.uniform(10.0, 200.0, size=T)),
+                  species_rule="random" if T > 1 else "single")
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    skin = float(rng.choice([0.0, 0.4, 1.0]))
+    if rng.random() < 0.5:
+        pos, box = W.sheared(s, *rng.uniform(-0.25, 0.25, size=3))
+    else:
+        pos, box = s.pos, np.diag(s.box)
+    if W.perpendicular_widths(box).min() < 2 * (hy.rc_radial + skin):
+        skin = 0.0
+    if W.perpendicular_widths(box).min() < 2 * hy.rc_radial:
+        pytest.skip("cell too small for this draw")
+    run_both(pkg, oracle_mod, hy, p, s.masses, pos, s.types, box, skin=skin)
+
+
 @pytest.mark.parametrize("idx,cells", [(0, None), (2, (3, 3, 3)), (3, (4, 4, 3))])
 def test_shared_memory_radial_variants(pkg, oracle_mod, idx, cells):
     """The configurations' species counts have register variants of the radial kernels; NEP_RADIAL_SMEM
