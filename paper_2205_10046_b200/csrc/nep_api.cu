@@ -287,9 +287,9 @@ int dispatch_radial_reg(nep_t* nep)
 {
     const NepDims& d = nep->d;
     if (d.T * nep->KP > 64 || d.T > 5) return kNoVariant;
-    // the force kernel evaluates all T dot products per pair and selects one: beyond three species the
-    // shared-memory variant (one row of E per pair) is faster (measured at T = 5: 486 vs 523 us)
-    if (FORCE && d.T > 3) return kNoVariant;
+    // the register variants spend T x KR select-FMAs per pair: beyond three species the shared-memory
+    // variants (one row per pair) are faster (measured at T = 5: force 486 vs 523 us, descriptor 346 vs 355)
+    if (d.T > 3) return kNoVariant;
     if (sizeof(float) * (size_t)d.T * d.T * nep->strideR > kRegTableMax) return kNoVariant;
     if (sizeof(float) * (size_t)d.T * d.T * d.NR * nep->KP > kRegTableMax) return kNoVariant;
 #define NEP_REG_CASE(TT, KPV)                                                                      \
@@ -312,7 +312,8 @@ int launch_radial_multi2(nep_t* nep, size_t sm)
 {
     const NepDims& d = nep->d;
     NEP_TRY(allow_smem(nep, k_radial_multi<KP, TAB_SM, BS>, sm));
-    NEP_TRY(cap_smem(nep, k_radial_multi<KP, TAB_SM, BS>, sm, nep->smem_budget));
+    // one gather per pair and a read-modify-write of shared memory: occupancy matters more than L1 here
+    NEP_TRY(cap_smem(nep, k_radial_multi<KP, TAB_SM, BS>, sm, (size_t)227 * 1024));
     NEP_LAUNCH(NEP_K_RADIAL, (k_radial_multi<KP, TAB_SM, BS><<<div_up(d.n, BS), BS, sm, nep->stream>>>(d, nep->strideR, nep->posq, nep->cA, nep->ncA,
                                                                                           nep->cB, nep->ncB, nep->cR_t, nep->q)));
     return NEP_OK;
