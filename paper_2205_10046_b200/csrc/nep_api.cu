@@ -360,24 +360,33 @@ int persistent_grid(nep_t* nep, K kernel, size_t smem, int* grid)
 }
 
 template <int NCH, bool SM>
-int launch_angular(nep_t* nep, const NepCoef& C, int p, bool force_pass)
+int launch_angular(nep_t* nep, const NepCoef& C, int p)
 {
     const NepDims& d = nep->d;
     const int stride = nep->pass_stride[p], n0 = nep->pass_n0[p];
     const float* tab = nep->cA_t + nep->pass_off[p];
     const size_t sm = SM ? sizeof(float) * (size_t)d.T * d.T * stride : 0;
     int grid = 0;
-    if (!force_pass) {
-        NEP_TRY(allow_smem(nep, k_angular<NCH, SM>, sm));
-        NEP_TRY(persistent_grid(nep, k_angular<NCH, SM>, sm, &grid));
-        NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, stride, nep->posq, nep->cA, nep->ncA, tab, nep->S, nep->q,
-                                                                                     nep->tile_ctr + p)));
-    } else {
-        NEP_TRY(allow_smem(nep, k_force_angular<NCH, SM>, sm));
-        NEP_TRY(persistent_grid(nep, k_force_angular<NCH, SM>, sm, &grid));
-        NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, p > 0, stride, nep->posq, nep->cA, nep->ncA, nep->mask, tab,
-                                                                                                 nep->S, nep->fp, nep->pf, nep->fa, nep->tile_ctr + 16 + p)));
-    }
+    NEP_TRY(allow_smem(nep, k_angular<NCH, SM>, sm));
+    NEP_TRY(persistent_grid(nep, k_angular<NCH, SM>, sm, &grid));
+    NEP_LAUNCH(NEP_K_ANGULAR, (k_angular<NCH, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, stride, nep->posq, nep->cA, nep->ncA, tab, nep->S, nep->q,
+                                                                                 nep->tile_ctr + p)));
+    return NEP_OK;
+}
+
+// NCH channels with G in registers + NSM channels with G in shared memory (passes of 6 or 7 channels)
+template <int NCH, int NSM, bool SM>
+int launch_force_angular(nep_t* nep, const NepCoef& C, int p)
+{
+    const NepDims& d = nep->d;
+    const int stride = nep->pass_stride[p], n0 = nep->pass_n0[p];
+    const float* tab = nep->cA_t + nep->pass_off[p];
+    const size_t sm = (SM ? sizeof(float) * (size_t)d.T * d.T * stride : 0) + sizeof(float) * (size_t)NSM * NEP_NUM_S * 128;
+    int grid = 0;
+    NEP_TRY(allow_smem(nep, k_force_angular<NCH, NSM, SM>, sm));
+    NEP_TRY(persistent_grid(nep, k_force_angular<NCH, NSM, SM>, sm, &grid));
+    NEP_LAUNCH(NEP_K_FORCE_ANGULAR, (k_force_angular<NCH, NSM, SM><<<grid, 128, sm, nep->stream>>>(d, C, n0, p > 0, stride, nep->posq, nep->cA, nep->ncA, nep->mask, tab,
+                                                                                                  nep->S, nep->fp, nep->pf, nep->fa, nep->tile_ctr + 16 + p)));
     return NEP_OK;
 }
 
@@ -385,14 +394,24 @@ int dispatch_angular(nep_t* nep, const NepCoef& C, bool force_pass)
 {
     for (int p = 0; p < nep->n_pass; ++p) {
         int rc;
-        if (!nep->angular_tab_smem) { rc = launch_angular<4, false>(nep, C, p, force_pass); }
+        if (!nep->angular_tab_smem) rc = force_pass ? launch_force_angular<4, 0, false>(nep, C, p) : launch_angular<4, false>(nep, C, p);
+        else if (!force_pass) switch (nep->pass_nch[p]) {
+            case 1: rc = launch_angular<1, true>(nep, C, p); break;
+            case 2: rc = launch_angular<2, true>(nep, C, p); break;
+            case 3: rc = launch_angular<3, true>(nep, C, p); break;
+            case 4: rc = launch_angular<4, true>(nep, C, p); break;
+            case 5: rc = launch_angular<5, true>(nep, C, p); break;
+            case 6: rc = launch_angular<6, true>(nep, C, p); break;
+            default: rc = launch_angular<7, true>(nep, C, p); break;
+        }
         else switch (nep->pass_nch[p]) {
-            case 1: rc = launch_angular<1, true>(nep, C, p, force_pass); break;
-            case 2: rc = launch_angular<2, true>(nep, C, p, force_pass); break;
-            case 3: rc = launch_angular<3, true>(nep, C, p, force_pass); break;
-            case 4: rc = launch_angular<4, true>(nep, C, p, force_pass); break;
-            case 5: rc = launch_angular<5, true>(nep, C, p, force_pass); break;
-            default: rc = launch_angular<6, true>(nep, C, p, force_pass); break;
+            case 1: rc = launch_force_angular<1, 0, true>(nep, C, p); break;
+            case 2: rc = launch_force_angular<2, 0, true>(nep, C, p); break;
+            case 3: rc = launch_force_angular<3, 0, true>(nep, C, p); break;
+            case 4: rc = launch_force_angular<4, 0, true>(nep, C, p); break;
+            case 5: rc = launch_force_angular<5, 0, true>(nep, C, p); break;
+            case 6: rc = launch_force_angular<5, 1, true>(nep, C, p); break;
+            default: rc = launch_force_angular<5, 2, true>(nep, C, p); break;
         }
         if (rc != NEP_OK) return rc;
     }
@@ -671,11 +690,12 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     nep->KP = round_up4(d.KR);
     nep->strideR = (d.KR * d.NRP) | 1;
     nep->nch_max = 5;
+    bool nch_forced = false;
     nep->smem_budget = 180 * 1024;
     nep->ann_fp32 = getenv("NEP_ANN_FP32") != nullptr;                // tests / comparison: the fp32-FMA network kernel
     nep->force_smem_radial = getenv("NEP_RADIAL_SMEM") != nullptr;    // tests: exercise the shared-memory variants
     if (const char* e = getenv("NEP_SMEM_KB")) { const int v = atoi(e); if (v >= 8 && v <= 227) nep->smem_budget = (size_t)v * 1024; }
-    if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) nep->nch_max = v; }
+    if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) { nep->nch_max = v; nch_forced = true; } }
     {   // angular passes: at most nch_max channels each, tables staged in shared memory; if a table would
         // not fit there, passes of 4 channels read it from global memory (zero-padded surplus channels)
         {
@@ -684,6 +704,9 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
             nep->num_sms = prop.multiProcessorCount;
         }
         auto stride_of = [&](int nch) { return (d.KAR * round_up4(nch)) | 1; };
+        // six or seven channels go in ONE pass (the descriptor kernel holds 24 x 7 sums in registers, the force
+        // kernel keeps the G of channels 6-7 in shared memory); more channels in passes of at most nch_max
+        if (!nch_forced && (d.NA == 6 || d.NA == 7)) nep->nch_max = d.NA;
         const int npass = (d.NA + nep->nch_max - 1) / nep->nch_max;
         const int base = d.NA / npass, rem = d.NA % npass;
         nep->angular_tab_smem = sizeof(float) * (size_t)TT * stride_of(base + (rem ? 1 : 0)) <= kSmemTableMax;

@@ -11,7 +11,7 @@
 
 #define NEP_MAX_TYPES 16
 #define NEP_NUM_S 24            // sums S_{n,k}, k = 0..23 (Eq. 12)
-#define NEP_NCH_MAX 6           // most angular n-values handled per pass (24*NCH accumulators in registers)
+#define NEP_NCH_MAX 7           // most angular n-values handled per pass (24*NCH accumulators in registers)
 #define NEP_SLOT_BITS 8         // packed angular entry: (j << 8) | skin slot
 #define NEP_MAX_ATOMS (1 << 24)
 

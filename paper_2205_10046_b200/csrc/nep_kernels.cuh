@@ -794,15 +794,20 @@ __device__ __forceinline__ void G_from_S(const float* S, const float* f3, float 
 // g_n and g_n' from the table of k_angular:  with G0_n = sum_{k>=1} c_nk T_k + csum'_n and
 // G1_n = sum_{k>=1} c_nk T_k'(x):  g_n = (f_c/2) G0_n,  g_n' = (f_c'/2) G0_n + (f_c/2) x'(r) G1_n;
 // T_{k+1}' = 2 T_k + 2 x T_k' - T_{k-1}'.
-template <int NCH>
+// NCH channels keep their G_nk in registers; NSM further channels (a pass of 6 or 7) keep them in this thread's
+// column of shared memory, [channel * 24 + k][128]: one pass with 48 extra shared loads per pair instead of a
+// second pass that would repeat the pair geometry, b_k, grad P_k and the assembly.
+template <int NCH, int NSM>
 __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCoef& C, int n0, int accumulate, int tab_stride,
                                                    const float* tab, const int4* __restrict__ posq,
                                                    const int* __restrict__ cA, const int* __restrict__ ncA,
                                                    const unsigned long long* __restrict__ mask,
                                                    const float* __restrict__ S_in, const float* __restrict__ fp,
-                                                   float4* __restrict__ pf, float4* __restrict__ fa, int s)
+                                                   float4* __restrict__ pf, float4* __restrict__ fa, int s,
+                                                   float* __restrict__ myG)
 {
-    constexpr int N4 = (NCH + 3) / 4;
+    constexpr int NT = NCH + NSM;
+    constexpr int N4 = (NT + 3) / 4;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
     float G[NCH][NEP_NUM_S];
@@ -810,7 +815,7 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         const float* fpa = fp + (size_t)D.NR * n + s;          // angular blocks: fpa[(blk * NA + nn) * n]
         const size_t blk = (size_t)D.NA * n;
 #pragma unroll
-        for (int a = 0; a < NCH; ++a) {
+        for (int a = 0; a < NT; ++a) {
             const int nn = min(n0 + a, D.NA - 1);
             float Sv[NEP_NUM_S], f3[4];
             const float* Sp = S_in + (size_t)(nn * NEP_NUM_S) * n + s;
@@ -822,10 +827,16 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
             float f4 = 0.0f, f5 = 0.0f;
             if (D.has4) { f4 = *fq; fq += blk; }
             if (D.has5) f5 = *fq;
-            G_from_S(Sv, f3, f4, f5, C, G[a]);
+            float Gt[NEP_NUM_S];
+            G_from_S(Sv, f3, f4, f5, C, Gt);
             if (n0 + a >= D.NA) {                              // padded channel of the global-table fallback
 #pragma unroll
-                for (int k = 0; k < NEP_NUM_S; ++k) G[a][k] = 0.0f;
+                for (int k = 0; k < NEP_NUM_S; ++k) Gt[k] = 0.0f;
+            }
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S; ++k) {
+                if (a < NCH) G[a < NCH ? a : 0][k] = Gt[k];
+                else myG[((a - NCH) * NEP_NUM_S + k) * 128] = Gt[k];
             }
         }
     }
@@ -838,26 +849,26 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         const float rinv = rsqrtf(r2), r = r2 * rinv;
         const BasisHead h = basis_head<true>(r, D.rcA_inv);
         const float* c4 = tab_i + w.pj.w * tab_stride;
-        float g[4 * N4], dg[NCH];
-        load_row<NCH>(c4, g);                              // csum'
+        float g[4 * N4], dg[NT];
+        load_row<NT>(c4, g);                              // csum'
 #pragma unroll
-        for (int a = 0; a < NCH; ++a) dg[a] = 0.0f;
+        for (int a = 0; a < NT; ++a) dg[a] = 0.0f;
         {
             float Tkm1 = 1.0f, Tk = h.x, Dkm1 = 0.0f, Dk = 1.0f;      // T_0,T_1 ; T_0',T_1'
             for (int r0 = 1; r0 < D.KAR; r0 += 4) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     float c[4 * N4];
-                    load_row<NCH>(c4 + (r0 + u) * (4 * N4), c);
+                    load_row<NT>(c4 + (r0 + u) * (4 * N4), c);
 #pragma unroll
-                    for (int a = 0; a < NCH; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
+                    for (int a = 0; a < NT; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
                     const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
                     const float Tn = fmaf(h.two_x, Tk, -Tkm1);
                     Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
                 }
             }
 #pragma unroll
-            for (int a = 0; a < NCH; ++a) {
+            for (int a = 0; a < NT; ++a) {
                 const float G0 = g[a];
                 g[a] = G0 * h.hfc;
                 dg[a] = fmaf(G0, h.hdfc, dg[a] * h.hfc_dx);
@@ -873,6 +884,9 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         {                                                                                           \
             float A = 0.0f, B = 0.0f;                                                               \
             _Pragma("unroll") for (int a = 0; a < NCH; ++a) { A = fmaf(G[a][k], g[a], A); B = fmaf(G[a][k], dg[a], B); } \
+            _Pragma("unroll") for (int a = 0; a < NSM; ++a) {                                      \
+                const float Gs = myG[(a * NEP_NUM_S + (k)) * 128];                                  \
+                A = fmaf(Gs, g[NCH + a], A); B = fmaf(Gs, dg[NCH + a], B); }                        \
             cu = fmaf(fmaf(-(float)(l) * rinv, A, B), b[k], cu);                                    \
             vx = fmaf(A, (gx), vx); vy = fmaf(A, (gy), vy); vz = fmaf(A, (gz), vz);                 \
         }
@@ -913,19 +927,20 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
     fa[s] = make_float4(sx, sy, sz, 0.0f);
 }
 
-template <int NCH, bool SM>
+template <int NCH, int NSM, bool SM>
 __global__ void __launch_bounds__(128)
 k_force_angular(NepDims D, NepCoef C, int n0, int accumulate, int tab_stride, const int4* __restrict__ posq,
                 const int* __restrict__ cA, const int* __restrict__ ncA, const unsigned long long* __restrict__ mask,
                 const float* __restrict__ cA_t, const float* __restrict__ S_in, const float* __restrict__ fp,
                 float4* __restrict__ pf, float4* __restrict__ fa, int* __restrict__ tile_ctr)
 {
-    extern __shared__ __align__(16) float sc[];
+    extern __shared__ __align__(16) float sc[];         // [coefficient table (SM)] [G of the NSM channels: NSM * 24 rows of 128]
     const float* tab = stage_table<SM>(cA_t, D.T * D.T * tab_stride, sc);
+    float* myG = sc + (SM ? D.T * D.T * tab_stride : 0) + threadIdx.x;
     const int ntile = (D.n + 31) >> 5;
     for (int tile = next_tile(tile_ctr); tile < ntile; tile = next_tile(tile_ctr)) {
         const int s = tile * 32 + (threadIdx.x & 31);
-        if (s < D.n) force_angular_atom<NCH>(D, C, n0, accumulate, tab_stride, tab, posq, cA, ncA, mask, S_in, fp, pf, fa, s);
+        if (s < D.n) force_angular_atom<NCH, NSM>(D, C, n0, accumulate, tab_stride, tab, posq, cA, ncA, mask, S_in, fp, pf, fa, s, myG);
     }
 }
 
