@@ -187,6 +187,32 @@ int nep_get_descriptors(nep_t* nep, float* q_dev, float* fp_dev);
 int nep_get_angular_sums(nep_t* nep, float* S_dev);
 int nep_get_latent(nep_t* nep, float* latent_dev);
 
+/* ---- parameter sets: SNES training evaluates a POPULATION of parameter vectors z on the same structures
+ * (Eqs. (31)-(33)); the neighbour lists and the per-step in-cutoff lists depend on the
+ * geometry only (single-structure slice).
+ * nep_set_parameters: replaces the model parameters (same hyper-parameters, same layouts as nep_create);
+ *   lists stay valid; the next nep_compute / md_step uses the new model.  Synchronises the stream.
+ * nep_compute_population: n_pop parameter sets, stacked member-major in HOST arrays (c_radial
+ *   [n_pop][T][T][NR][KR], c_angular [n_pop][T][T][NA][KA], w0 [n_pop][H][D], b0, w1 [n_pop][H], b1 [n_pop]),
+ *   evaluated at the same positions: energy_dev [n_pop][n], force_dev [n_pop][n][3], virial_dev
+ *   [n_pop][n][9] (any may be NULL).  Positions are quantised and the skin lists filtered once; every
+ *   member runs the descriptor, network and force kernels.  Leaves the LAST member's parameters in the
+ *   handle.  NEP_ERR_STATE before nep_neighbors.  Synchronises once per member (parameter upload).         */
+int nep_set_parameters(nep_t* nep, const float* c_radial, const float* c_angular,
+                       const float* w0, const float* b0, const float* w1, const float* b1);
+int nep_compute_population(nep_t* nep, const double* pos_dev, int32_t n_pop,
+                           const float* c_radial, const float* c_angular,
+                           const float* w0, const float* b0, const float* w1, const float* b1,
+                           double* energy_dev, double* force_dev, double* virial_dev);
+
+/* Data terms of the loss function, Eq. (33) (reading A17), of the LAST evaluation
+ * for one structure of n atoms: terms_host[0] = |sum_i U_i / n - u_target_per_atom|, [1] = sqrt(sum_i |F_i -
+ * F_i^tar|^2 / (3 n)), [2] = sqrt(sum over {xx,yy,zz,xy,yz,zx} of (sum_i W_i / n - w_target_per_atom)^2 / 6).
+ * f_target_dev [n][3] device, w_target_per_atom[6] and terms_host[3] host.  Reduced on the device in a fixed
+ * order; synchronises.  The weights lambda and the regularisation terms of Eq. (33) are the caller's.      */
+int nep_loss_terms(nep_t* nep, double u_target_per_atom, const double* f_target_dev,
+                   const double w_target_per_atom[6], double terms_host[3]);
+
 /* ---- heat current, Eqs. (25)-(26) ------------------------------------------------
  * J_i = W_i . v_i with the per-atom virial W_i of the last evaluation (Eq. (24), layout W[3a+b]):
  * j_atom_dev [n][3] gets J_i^a = sum_b W_i^{ab} v_i^b, j_total_dev [3] gets J = sum_i J_i (reduced in a

@@ -345,3 +345,28 @@ def md_langevin(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_ste
         vel = langevin_half_step(vel, m_atom, t_target, c1, seed, 2 * s + 1)
         temps[k] = kinetic_temperature(vel, m_atom)
     return pos, vel, temps
+
+
+# ---- loss of one structure under one parameter set: the data terms of Eq. (33), PAPER.md:266-283 ---------
+def loss_terms(energy, force, virial, u_target: float, f_target, w_target6):
+    """The three RMSE terms of Eq. (33) for N_str = 1 (reading A17): with N atoms,
+      L_e = |sum_i U_i / N - u_target|                           (per-atom energy of the structure)
+      L_f = sqrt( sum_i |F_i - F_i^tar|^2 / (3 N) )
+      L_v = sqrt( sum_{mu nu in xx,yy,zz,xy,yz,zx} (sum_i W_i^{mu nu} / N - w_target[mu nu])^2 / 6 )
+    Returns (L_e, L_f, L_v); the weighted sum and the regularisation terms of Eq. (33) are the caller's."""
+    e, f, w = _d(energy), _d(force), _d(virial)
+    ft, wt = _d(f_target), _d(w_target6)
+    n = len(e)
+    le = abs(e.sum() / n - u_target)
+    lf = float(np.sqrt(((f - ft) ** 2).sum() / (3.0 * n)))
+    wtot = w.sum(axis=0) / n
+    six = np.array([wtot[0], wtot[4], wtot[8], wtot[1], wtot[5], wtot[6]])
+    lv = float(np.sqrt(((six - wt) ** 2).sum() / 6.0))
+    return float(le), lf, lv
+
+
+def regularisation_terms(params):
+    """The last two terms of Eq. (33) without their weights: (sum |z_n| / N_par, sqrt(sum z_n^2 / N_par)) over
+    all trainable parameters z (Eq. (30): c_radial, c_angular, w0, b0, w1, b1)."""
+    z = np.concatenate([_d(a).reshape(-1) for a in (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1)])
+    return float(np.abs(z).sum() / len(z)), float(np.sqrt((z * z).sum() / len(z)))

@@ -20,7 +20,8 @@ exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
-    "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin",
+    "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
+    "nep_compute_population", "nep_loss_terms",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
@@ -97,6 +98,12 @@ def load_library():
     L.md_step_nvt_langevin.argtypes = [vp, vp, vp, dbl, i32, i32, dbl, dbl, dbl, dbl, C.c_uint64, i64]
     L.nep_last_temperature.restype = C.c_int
     L.nep_last_temperature.argtypes = [vp, dp, dp]
+    L.nep_set_parameters.restype = C.c_int
+    L.nep_set_parameters.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.nep_compute_population.restype = C.c_int
+    L.nep_compute_population.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.nep_loss_terms.restype = C.c_int
+    L.nep_loss_terms.argtypes = [vp, dbl, vp, dp, dp]
     L.nep_get_latent.restype = C.c_int
     L.nep_get_latent.argtypes = [vp, vp]
     L.nep_heat_current.restype = C.c_int
@@ -292,6 +299,32 @@ class NEP:
         S = torch.empty((self.n, self.hyper.n_max_angular + 1, 24), dtype=torch.float32, device=f"cuda:{self.device}")
         self._check(self._L.nep_get_angular_sums(self._h_ptr, C.c_void_p(S.data_ptr())))
         return S
+
+    def nep_set_parameters(self, params):
+        arrs = [_f32(a) for a in (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1)]
+        self._check(self._L.nep_set_parameters(self._h_ptr, *[C.c_void_p(a.ctypes.data) for a in arrs]))
+
+    def nep_compute_population(self, pos, members):
+        """E [n_pop][n], F [n_pop][n][3], W [n_pop][n][9] of a list of parameter sets at the same positions."""
+        torch = self._torch
+        n, dev, P = self.n, f"cuda:{self.device}", len(members)
+        stack = [np.ascontiguousarray(np.stack([_f32(getattr(m, k)).reshape(-1) for m in members]))
+                 for k in ("c_radial", "c_angular", "w0", "b0", "w1", "b1")]
+        e = torch.empty((P, n), dtype=torch.float64, device=dev)
+        f = torch.empty((P, n, 3), dtype=torch.float64, device=dev)
+        w = torch.empty((P, n, 9), dtype=torch.float64, device=dev)
+        self._check(self._L.nep_compute_population(self._h_ptr, self._dev(pos, torch.float64, 3 * n), P,
+                                                   *[C.c_void_p(a.ctypes.data) for a in stack],
+                                                   C.c_void_p(e.data_ptr()), C.c_void_p(f.data_ptr()), C.c_void_p(w.data_ptr())))
+        return e, f, w
+
+    def nep_loss_terms(self, u_target: float, f_target, w_target6):
+        """(L_e, L_f, L_v) of Eq. (33) for the last evaluation."""
+        torch = self._torch
+        wt = (C.c_double * 6)(*[float(x) for x in w_target6])
+        out = (C.c_double * 3)()
+        self._check(self._L.nep_loss_terms(self._h_ptr, float(u_target), self._dev(f_target, torch.float64, 3 * self.n), wt, out))
+        return out[0], out[1], out[2]
 
     def nep_get_latent(self):
         """[n][H] latent-space vectors of the last evaluation."""

@@ -528,7 +528,7 @@ int dispatch_final(nep_t* nep)
     return NEP_OK;
 }
 
-int evaluate(nep_t* nep, const double* pos_dev)
+int evaluate(nep_t* nep, const double* pos_dev, bool reuse_geometry = false)
 {
     static const NepCoef C = make_coef();
     const NepDims& d = nep->d;
@@ -536,11 +536,13 @@ int evaluate(nep_t* nep, const double* pos_dev)
     cudaStream_t st = nep->stream;
     CellInv inv;
     for (int a = 0; a < 9; ++a) inv.m[a] = nep->Hinv[a];
-    NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
-    NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
     NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
-    NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
-                                             nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
+    if (!reuse_geometry) {   // else: same positions as the previous evaluation (another member of a population)
+        NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
+        NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
+        NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
+                                                 nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
+    }
     NEP_TRY(dispatch_radial(nep));
     NEP_TRY(dispatch_angular(nep, C, false));
     NEP_TRY(dispatch_ann(nep));
@@ -616,6 +618,58 @@ int launch_latent(nep_t* nep, float* latent_dev)
     const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H);
     NEP_TRY(allow_smem(nep, k_latent<DP>, sm));
     NEP_LAUNCH(NEP_K_EXPORT, k_latent<DP><<<div_up(d.n, 128), 128, sm, nep->stream>>>(d, nep->perm, nep->q, nep->w0p, nep->b0, nep->w1, latent_dev));
+    return NEP_OK;
+}
+
+// Re-laid-out parameter tables (layouts documented at the kernels that read them) from the caller's host
+// arrays; device arrays are allocated on first use.  Copies are enqueued on the handle's stream and the
+// stream is synchronised (the host vectors are temporaries), so a later evaluation sees the new model.
+int upload_parameters(nep_t* nep, const float* c_radial, const float* c_angular, const float* w0, const float* b0,
+                      const float* w1, const float* b1)
+{
+    const NepDims& d = nep->d;
+    const int TT = d.T * d.T;
+    std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f);
+    std::vector<float> cAt((size_t)nep->pass_off[nep->n_pass - 1] + (size_t)TT * nep->pass_stride[nep->n_pass - 1], 0.0f);
+    std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
+    for (int tt = 0; tt < TT; ++tt) {
+        for (int nn = 0; nn < d.NR; ++nn)
+            for (int k = 0; k < d.KR; ++k) {
+                const float v = c_radial[((size_t)tt * d.NR + nn) * d.KR + k];
+                cRt[(size_t)tt * nep->strideR + (size_t)k * d.NRP + nn] = v;
+                cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
+            }
+        for (int p = 0; p < nep->n_pass; ++p) {
+            const int NCHP = round_up4(nep->pass_nch[p]);
+            float* tab = cAt.data() + nep->pass_off[p] + (size_t)tt * nep->pass_stride[p];
+            for (int a = 0; a < nep->pass_nch[p] && nep->pass_n0[p] + a < d.NA; ++a) {
+                const float* c = c_angular + ((size_t)tt * d.NA + nep->pass_n0[p] + a) * d.KA;
+                double csum = 2.0 * (double)c[0];                  // csum'_n = 2 c_n0 + sum_{k>=1} c_nk
+                for (int k = 1; k < d.KA; ++k) {
+                    tab[(size_t)k * NCHP + a] = c[k];
+                    csum += (double)c[k];
+                }
+                tab[a] = (float)csum;
+            }
+        }
+    }
+    for (int m = 0; m < d.H; ++m)
+        for (int v = 0; v < d.D; ++v) w0p[(size_t)m * nep->DP + v] = w0[(size_t)m * d.D + v];
+    nep->b1 = b1[0];
+    std::vector<float> vb0(b0, b0 + d.H), vw1(w1, w1 + d.H);
+#define UPLOAD(dst, vec)                                                                          \
+    do {                                                                                          \
+        if (!nep->dst) NEP_TRY(dev_alloc(nep, &nep->dst, (vec).size()));                          \
+        NEP_CUDA(cudaMemcpyAsync(nep->dst, (vec).data(), (vec).size() * sizeof((vec)[0]), cudaMemcpyHostToDevice, nep->stream)); \
+    } while (0)
+    UPLOAD(cR_t, cRt);
+    UPLOAD(cA_t, cAt);
+    UPLOAD(cR_e, cRe);
+    UPLOAD(w0p, w0p);
+    UPLOAD(b0, vb0);
+    UPLOAD(w1, vw1);
+#undef UPLOAD
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
     return NEP_OK;
 }
 
@@ -720,51 +774,14 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
             n0 += nch;
         }
     }
-    std::vector<float> cRt((size_t)TT * nep->strideR, 0.0f);
-    std::vector<float> cAt((size_t)nep->pass_off[nep->n_pass - 1] + (size_t)TT * nep->pass_stride[nep->n_pass - 1], 0.0f);
-    std::vector<float> cRe((size_t)TT * d.NR * d.KRP, 0.0f), w0p((size_t)d.H * nep->DP, 0.0f);
-    for (int tt = 0; tt < TT; ++tt) {
-        for (int nn = 0; nn < d.NR; ++nn)
-            for (int k = 0; k < d.KR; ++k) {
-                const float v = c_radial[((size_t)tt * d.NR + nn) * d.KR + k];
-                cRt[(size_t)tt * nep->strideR + (size_t)k * d.NRP + nn] = v;
-                cRe[((size_t)tt * d.NR + nn) * d.KRP + k] = v;
-            }
-        for (int p = 0; p < nep->n_pass; ++p) {
-            const int NCHP = round_up4(nep->pass_nch[p]);
-            float* tab = cAt.data() + nep->pass_off[p] + (size_t)tt * nep->pass_stride[p];
-            for (int a = 0; a < nep->pass_nch[p] && nep->pass_n0[p] + a < d.NA; ++a) {
-                const float* c = c_angular + ((size_t)tt * d.NA + nep->pass_n0[p] + a) * d.KA;
-                double csum = 2.0 * (double)c[0];                  // csum'_n = 2 c_n0 + sum_{k>=1} c_nk
-                for (int k = 1; k < d.KA; ++k) {
-                    tab[(size_t)k * NCHP + a] = c[k];
-                    csum += (double)c[k];
-                }
-                tab[a] = (float)csum;
-            }
-        }
+    rc = upload_parameters(nep, c_radial, c_angular, w0, b0, w1, b1);
+    if (rc != NEP_OK) { nep_destroy(nep); return rc; }
+    {
+        std::vector<double> vm(nep->mass, nep->mass + d.T);
+        rc = dev_alloc(nep, &nep->mass_dev, vm.size());
+        if (rc == NEP_OK && cudaMemcpy(nep->mass_dev, vm.data(), vm.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) rc = NEP_ERR_CUDA;
+        if (rc != NEP_OK) { nep_destroy(nep); return rc; }
     }
-    for (int m = 0; m < d.H; ++m)
-        for (int v = 0; v < d.D; ++v) w0p[(size_t)m * nep->DP + v] = w0[(size_t)m * d.D + v];
-    nep->b1 = b1[0];
-
-#define UPLOAD(dst, vec)                                                                          \
-    do {                                                                                          \
-        rc = dev_alloc(nep, &nep->dst, (vec).size());                                             \
-        if (rc == NEP_OK && cudaMemcpy(nep->dst, (vec).data(), (vec).size() * sizeof((vec)[0]),   \
-                                       cudaMemcpyHostToDevice) != cudaSuccess) rc = NEP_ERR_CUDA; \
-        if (rc != NEP_OK) { nep_destroy(nep); return rc; }                                        \
-    } while (0)
-    UPLOAD(cR_t, cRt);
-    UPLOAD(cA_t, cAt);
-    UPLOAD(cR_e, cRe);
-    UPLOAD(w0p, w0p);
-    std::vector<float> vb0(b0, b0 + d.H), vw1(w1, w1 + d.H);
-    UPLOAD(b0, vb0);
-    UPLOAD(w1, vw1);
-    std::vector<double> vm(nep->mass, nep->mass + d.T);
-    UPLOAD(mass_dev, vm);
-#undef UPLOAD
     rc = dev_alloc(nep, &nep->flags, 8);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->tile_ctr, 64);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 1);
@@ -980,6 +997,69 @@ int nep_get_angular_sums(nep_t* nep, float* S_dev)
 }
 
 // ---- derived outputs ----------------------------------------------------
+int nep_set_parameters(nep_t* nep, const float* c_radial, const float* c_angular, const float* w0, const float* b0,
+                       const float* w1, const float* b1)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!c_radial || !c_angular || !w0 || !b0 || !w1 || !b1) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    NEP_TRY(upload_parameters(nep, c_radial, c_angular, w0, b0, w1, b1));
+    nep->have_eval = nep->force_current = false;         // E/F/W of the old model no longer apply
+    return NEP_OK;
+}
+
+int nep_compute_population(nep_t* nep, const double* pos_dev, int32_t n_pop, const float* c_radial, const float* c_angular,
+                           const float* w0, const float* b0, const float* w1, const float* b1,
+                           double* energy_dev, double* force_dev, double* virial_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!pos_dev || n_pop < 1 || !c_radial || !c_angular || !w0 || !b0 || !w1 || !b1) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n_pop < 1");
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const NepDims& d = nep->d;
+    const size_t n = (size_t)nep->n;
+    const size_t sR = (size_t)d.T * d.T * d.NR * d.KR, sA = (size_t)d.T * d.T * d.NA * d.KA, sW = (size_t)d.H * d.D;
+    for (int32_t m = 0; m < n_pop; ++m) {
+        NEP_TRY(upload_parameters(nep, c_radial + m * sR, c_angular + m * sA, w0 + m * sW, b0 + (size_t)m * d.H, w1 + (size_t)m * d.H, b1 + m));
+        // the geometry is the population's: positions are quantised and the lists filtered once
+        NEP_TRY(evaluate(nep, pos_dev, m > 0));
+        NEP_TRY(nep_get_last(nep, energy_dev ? energy_dev + m * n : nullptr, force_dev ? force_dev + 3 * m * n : nullptr,
+                             virial_dev ? virial_dev + 9 * m * n : nullptr));
+    }
+    nep->force_current = false;                          // the handle now holds the LAST member's model and forces
+    return NEP_OK;
+}
+
+int nep_loss_terms(nep_t* nep, double u_target_per_atom, const double* f_target_dev, const double w_target_per_atom[6],
+                   double terms_host[3])
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!f_target_dev || !w_target_per_atom || !terms_host) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int n = (int)nep->n;
+    const int nb = div_up(n, 256);
+    if (11 * nb + 11 > nep->loss_cap) {
+        nep->loss_cap = 0;
+        NEP_TRY(dev_alloc(nep, &nep->loss_partial, 11 * (size_t)nb + 11));
+        nep->loss_cap = 11 * nb + 11;
+    }
+    double* tot_dev = nep->loss_partial + 11 * (size_t)nb;
+    NEP_LAUNCH(NEP_K_EXPORT, k_loss_partial<<<nb, 256, 0, nep->stream>>>(n, nep->e_out, nep->f_out, nep->w_out, f_target_dev, nep->loss_partial));
+    NEP_LAUNCH(NEP_K_EXPORT, k_loss_total<<<1, 256, 0, nep->stream>>>(nb, nep->loss_partial, tot_dev));
+    double t[11];
+    NEP_CUDA(cudaMemcpyAsync(t, tot_dev, sizeof(t), cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    const double N = (double)n;
+    terms_host[0] = fabs(t[0] / N - u_target_per_atom);
+    terms_host[1] = sqrt(t[1] / (3.0 * N));
+    const int six[6] = {0, 4, 8, 1, 5, 6};               // xx, yy, zz, xy, yz, zx of W[3a+b]
+    double sv = 0.0;
+    for (int c = 0; c < 6; ++c) { const double dv = t[2 + six[c]] / N - w_target_per_atom[c]; sv += dv * dv; }
+    terms_host[2] = sqrt(sv / 6.0);
+    return NEP_OK;
+}
+
 int nep_get_latent(nep_t* nep, float* latent_dev)
 {
     if (!nep) return NEP_ERR_INVALID_ARG;

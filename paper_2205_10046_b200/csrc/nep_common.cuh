@@ -135,6 +135,8 @@ struct nep_ctx {
 
     double* thermo;          // [blocks] partials of sum m v^2, then {lambda, T before the rescale} of the last step
     int thermo_cap;
+    double* loss_partial;    // [11 * blocks + 11] block partials and totals of nep_loss_terms
+    int loss_cap;
     double* heat_partial;    // [3 * blocks + 3] block partials of the total heat current (nep_heat_current)
     int heat_cap;
 

@@ -1443,3 +1443,60 @@ __global__ void k_scale_velocities(int n3, const double* __restrict__ lambda, do
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t < n3) vel[t] *= lambda[0];
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Data terms of the loss, Eq. (33) (reading A17), of the last evaluation: block
+// partials of {sum U_i, sum |F_i - F_i^tar|^2, sum W_i[0..8]} (11 numbers), then one block adds them in a
+// fixed order.
+__global__ void __launch_bounds__(256)
+k_loss_partial(int n, const double* __restrict__ e, const double* __restrict__ f, const double* __restrict__ w,
+               const double* __restrict__ f_target, double* __restrict__ partial)
+{
+    __shared__ double sh[11][256];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double v[11];
+#pragma unroll
+    for (int a = 0; a < 11; ++a) v[a] = 0.0;
+    if (i < n) {
+        v[0] = e[i];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { const double d = f[3 * (size_t)i + a] - f_target[3 * (size_t)i + a]; v[1] += d * d; }
+#pragma unroll
+        for (int a = 0; a < 9; ++a) v[2 + a] = w[9 * (size_t)i + a];
+    }
+#pragma unroll
+    for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] = v[a];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x < 11) partial[11 * (size_t)blockIdx.x + threadIdx.x] = sh[threadIdx.x][0];
+}
+
+__global__ void __launch_bounds__(256)
+k_loss_total(int nblocks, const double* __restrict__ partial, double* __restrict__ total)
+{
+    __shared__ double sh[11][256];
+    double v[11];
+#pragma unroll
+    for (int a = 0; a < 11; ++a) v[a] = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 256) {
+#pragma unroll
+        for (int a = 0; a < 11; ++a) v[a] += partial[11 * (size_t)b + a];
+    }
+#pragma unroll
+    for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] = v[a];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x < 11) total[threadIdx.x] = sh[threadIdx.x][0];
+}

@@ -297,3 +297,69 @@ def test_langevin_normal_deviates_and_equilibrium(pkg, oracle_mod):
     t_end = oracle_mod.kinetic_temperature(vel.cpu().numpy(), m)
     assert abs(t_end - 650.0) < 6.0 * 650.0 * np.sqrt(2.0 / (3 * n)) + 30.0
     nep.close()
+
+
+# ------------------------------------------------------------------ parameter populations (one-structure slice)
+@pytest.mark.parametrize("idx,cells,skin", [(0, None, 0.0), (3, (7, 6, 5), 1.0), (4, (9, 8, 7), 0.5)])
+def test_population_of_parameter_sets(pkg, oracle_mod, idx, cells, skin):
+    """Six parameter sets (an evolution-strategy population, one of them the NEP2 pattern c_nk = delta_nk c_n)
+    evaluated at the same positions with one list filter: each member against the oracle; then
+    nep_set_parameters + nep_compute reproduces a member bit for bit."""
+    cfg = W.get_config(idx, cells) if cells else W.get_config(idx)
+    s = W.make_system(cfg)
+    members = W.make_population(cfg, 5, 0.15)
+    members.append(W.nep2_pattern(members[0]))
+    nep = pkg.NEP(cfg.hyper, members[3], s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, skin)
+    e, f, w = nep.nep_compute_population(pos, members)
+    e, f, w = e.cpu().numpy(), f.cpu().numpy(), w.cpu().numpy()
+    assert np.abs(e[0] - e[1]).max() > 1e-4                      # the members do differ
+    for m, p in enumerate(members):
+        eo, fo, wo = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box)
+        assert np.abs(e[m] - eo).max() <= 1e-5
+        fn = np.linalg.norm(fo, axis=1, keepdims=True)
+        assert (np.abs(f[m] - fo) <= np.maximum(1e-4, 1e-4 * fn)).all()
+        wn = np.linalg.norm(wo, axis=1)
+        assert (np.linalg.norm(w[m] - wo, axis=1) <= 1e-4 * np.maximum(wn, np.median(wn))).all()
+    nep.nep_set_parameters(members[2])
+    e2, f2, w2 = nep.nep_compute(pos)
+    assert np.array_equal(e2.cpu().numpy(), e[2]) and np.array_equal(f2.cpu().numpy(), f[2]) and np.array_equal(w2.cpu().numpy(), w[2])
+    # and MD continues with the new model
+    vel = torch.tensor(s.vel, device="cuda:0")
+    nep.md_step(pos, vel, cfg.dt_fs, 2, cfg.rebuild_every, skin)
+    po, vo, _, _ = oracle_mod.md(cfg.hyper, members[2], s.pos, s.vel, s.types, s.masses, s.box, cfg.dt_fs, 2)
+    assert np.abs(pos.cpu().numpy() - po).max() < 3e-6
+    nep.close()
+
+
+def test_loss_terms_of_a_population(pkg, oracle_mod):
+    """Eq. (33)'s data terms per member against synthetic targets (the oracle's E/F/W of the population mean
+    plus noise): device reduction vs the oracle's loss_terms on the oracle's own E/F/W."""
+    cfg = W.get_config(3, (7, 6, 5))
+    s = W.make_system(cfg)
+    members = W.make_population(cfg, 4, 0.15)
+    rng = np.random.default_rng(5)
+    e0, f0, w0 = oracle_mod.compute(cfg.hyper, members[0], s.pos, s.types, s.box)
+    n = len(s.pos)
+    u_t = e0.sum() / n + 0.003
+    f_t = f0 + 0.05 * rng.normal(size=f0.shape)
+    wt9 = w0.sum(axis=0) / n
+    w_t = np.array([wt9[0], wt9[4], wt9[8], wt9[1], wt9[5], wt9[6]]) * 1.02 + 0.001
+    nep = pkg.NEP(cfg.hyper, members[0], s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    f_t_dev = torch.tensor(f_t, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 1.0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.nep_loss_terms(u_t, f_t_dev, w_t)
+    assert ei.value.status == -5
+    for p in members:
+        nep.nep_set_parameters(p)
+        nep.nep_compute(pos)
+        le, lf, lv = nep.nep_loss_terms(u_t, f_t_dev, w_t)
+        eo, fo, wo = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box)
+        oe, of, ov = oracle_mod.loss_terms(eo, fo, wo, u_t, f_t, w_t)
+        assert le == pytest.approx(oe, abs=1e-6)          # per-atom energy: 1e-5 eV per atom at worst, averaged
+        assert lf == pytest.approx(of, rel=1e-4)
+        assert lv == pytest.approx(ov, rel=2e-3, abs=1e-6)
+    nep.close()

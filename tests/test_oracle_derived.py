@@ -279,3 +279,27 @@ def test_langevin_limits_and_free_particle_relaxation(oracle_mod):
     want = T0 + (cfg0.temperature - T0) * c4 ** np.arange(1, nst + 1)
     assert (np.abs(temps - want) < 5.0 * want * np.sqrt(2.0 / (3 * len(s0.pos)))).all()
     assert temps[-1] > 2.5 * cfg0.temperature
+
+
+# ------------------------------------------------------------------ loss terms of Eq. (33) (reading A17)
+def test_loss_terms_hand_case_and_zero(oracle_mod):
+    e = np.array([1.0, 3.0]); f = np.array([[1.0, 0.0, 0.0], [0.0, 2.0, 0.0]])
+    w = np.zeros((2, 9)); w[0, 0] = 2.0; w[1, 0] = 4.0; w[0, 1] = 1.0; w[1, 5] = -2.0; w[0, 6] = 6.0
+    ft = np.zeros((2, 3)); wt = np.zeros(6)
+    le, lf, lv = oracle_mod.loss_terms(e, f, w, 1.5, ft, wt)
+    assert le == pytest.approx(0.5)                                     # |4/2 - 1.5|
+    assert lf == pytest.approx(np.sqrt(5.0 / 6.0))                      # (1 + 4) / (3 * 2)
+    # per-atom totals: xx 3, xy 0.5, yz -1, zx 3; yy = zz = 0
+    assert lv == pytest.approx(np.sqrt((9.0 + 0.25 + 1.0 + 9.0) / 6.0))
+    le, lf, lv = oracle_mod.loss_terms(e, f, w, 2.0, f, np.array([3.0, 0.0, 0.0, 0.5, -1.0, 3.0]))
+    assert (le, lf, lv) == (0.0, 0.0, 0.0)
+    # Eq. (30) parameter count and the two norms
+    cfg = W.get_config(2)
+    p = W.make_params(cfg)
+    h = cfg.hyper
+    npar = (h.n_des + 2) * h.n_neurons + 1 + h.n_types ** 2 * (h.NR * h.KR + h.NA * h.KA)
+    z = np.concatenate([np.asarray(a, np.float64).ravel() for a in (p.c_radial, p.c_angular, p.w0, p.b0, p.w1, p.b1)])
+    assert len(z) == npar
+    l1, l2 = oracle_mod.regularisation_terms(p)
+    assert l1 == pytest.approx(np.abs(z).mean()) and l2 == pytest.approx(np.sqrt((z ** 2).mean()))
+    assert l1 <= l2 + 1e-15                                              # mean |z| <= rms z

@@ -231,3 +231,28 @@ def perpendicular_widths(box33) -> np.ndarray:
     a, b, c = H
     return np.array([vol / np.linalg.norm(np.cross(b, c)), vol / np.linalg.norm(np.cross(c, a)),
                      vol / np.linalg.norm(np.cross(a, b))])
+
+
+def make_population(cfg: Config, n_pop: int, sigma: float = 0.1, kind: str = "stress"):
+    """A seeded population of parameter sets around make_params(cfg, kind), as an evolution strategy draws
+    them: member m = mean + sigma * N(0, 1) per parameter, rounded to fp32.  Member 0 is the
+    mean itself.  With nep2=True-like patterns see nep2_pattern()."""
+    mean = make_params(cfg, kind)
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 905, cfg.index, n_pop]))
+    members = [mean]
+    for _ in range(1, n_pop):
+        members.append(Params(*[np.ascontiguousarray((a.astype(np.float64) + sigma * rng.normal(size=a.shape) * np.abs(a).mean()).astype(np.float32))
+                                for a in (mean.c_radial, mean.c_angular, mean.w0, mean.b0, mean.w1, mean.b1)]))
+    return members
+
+
+def nep2_pattern(params: Params) -> Params:
+    """The NEP2 special case of the NEP3 radial functions: c_nk^{ij} = delta_nk c_n^{ij}, i.e.
+    g_n = c_n^{ij} f_n -- every coefficient with k != n set to zero (needs N_bas >= n_max)."""
+    out = []
+    for c in (params.c_radial, params.c_angular):
+        z = np.zeros_like(c)
+        for n_ in range(min(c.shape[2], c.shape[3])):
+            z[:, :, n_, n_] = c[:, :, n_, n_]
+        out.append(z)
+    return Params(out[0], out[1], params.w0, params.b0, params.w1, params.b1)
