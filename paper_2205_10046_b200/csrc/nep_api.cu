@@ -234,8 +234,8 @@ int build_lists(nep_t* nep, const double* pos_dev)
     }
     {
         const int row = nep->capA + nep->capS;
-        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capA, 32)), 256, 0, st>>>(n, nep->capA, row, 0, nep->listA, nep->listT));
-        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capS, 32)), 256, 0, st>>>(n, nep->capS, row, nep->capA, nep->listS, nep->listT));
+        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capA, 64)), 256, 0, st>>>(n, nep->capA, row, 0, nep->listA, nep->listT));
+        NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capS, 64)), 256, 0, st>>>(n, nep->capS, row, nep->capA, nep->listS, nep->listT));
     }
     NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA + nep->capS, 0, nep->listA, nep->cntA, nep->listT, nep->rev));
     NEP_LAUNCH(NEP_K_BUILD_REV, k_build_rev<<<div_up(n, 128), 128, 0, st>>>(n, nep->capA + nep->capS, nep->capA, nep->listS, nep->cntS, nep->listT, nep->revS));

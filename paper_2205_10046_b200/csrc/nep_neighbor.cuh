@@ -271,17 +271,22 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
 __global__ void __launch_bounds__(256)
 k_transpose_list(int n, int cap, int cap_row, int base, const int* __restrict__ in, int* __restrict__ out)
 {
-    __shared__ int tile[32][33];
-    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    __shared__ int tile[64][33];                                         // 64 slots x 32 atoms
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 64;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;             // 32 x 8 threads
-    for (int r = ty; r < 32; r += 8) {
+#pragma unroll
+    for (int r = ty; r < 64; r += 8) {                                  // 8 coalesced 128-byte row reads in flight
         const int m = m0 + r, a = a0 + tx;
         tile[r][tx] = (m < cap && a < n) ? in[(size_t)m * n + a] : 0;
     }
     __syncthreads();
-    for (int r = ty; r < 32; r += 8) {
-        const int a = a0 + r, m = m0 + tx;
-        if (a < n && m < cap) out[(size_t)a * cap_row + base + m] = tile[tx][r];
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {                                  // an atom's 64 slots: two 128-byte writes
+        const int a = a0 + r;
+        if (a < n) {
+            if (m0 + tx < cap) out[(size_t)a * cap_row + base + m0 + tx] = tile[tx][r];
+            if (m0 + 32 + tx < cap) out[(size_t)a * cap_row + base + m0 + 32 + tx] = tile[32 + tx][r];
+        }
     }
 }
 
