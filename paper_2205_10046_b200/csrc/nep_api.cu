@@ -798,6 +798,7 @@ int nep_destroy(nep_t* nep)
     cudaSetDevice(nep->device);
     cudaStreamSynchronize(nep->stream);
     for (int a = 0; a < nep->n_owned; ++a) cudaFree(nep->owned[a].p);
+    if (nep->copy_stream) { cudaStreamDestroy(nep->copy_stream); cudaEventDestroy(nep->ev_pos); }
     if (nep->prof_ev) {
         for (int a = 0; a < 2 * NEP_PROF_PAIRS; ++a) cudaEventDestroy(nep->prof_ev[a]);
         free(nep->prof_ev);
@@ -871,8 +872,10 @@ struct Thermostat {
     int64_t first_step;
 };
 
+// pos_ready (optional): recorded on the stream as soon as the positions have their final values (after the
+// drift of the last step), so that a copy on another stream can overlap the last force evaluation
 static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
-                   double skin, const Thermostat& th)
+                   double skin, const Thermostat& th, cudaEvent_t pos_ready = nullptr)
 {
     if (!nep) return NEP_ERR_INVALID_ARG;
     if (!pos_dev || !vel_dev || n_steps < 0 || rebuild_every < 1 || !(skin >= 0.0) || !(dt_fs == dt_fs))
@@ -900,6 +903,7 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
         NEP_TRY(dev_alloc(nep, &nep->thermo, (size_t)nb + 2));
         nep->thermo_cap = nb + 2;
     }
+    if (pos_ready && n_steps == 0) NEP_CUDA(cudaEventRecord(pos_ready, st));
     const double lc1 = th.kind == 2 ? exp(-dt_fs / (2.0 * th.tau_fs)) : 1.0, lc2 = sqrt(1.0 - lc1 * lc1);
     for (int s = 0; s < n_steps; ++s) {
         const double t_target = th.kind ? th.t_start + (th.t_stop - th.t_start) * (double)(s + 1) / (double)n_steps : 0.0;
@@ -907,6 +911,7 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
                                                       2ull * (unsigned long long)(th.first_step + s), nep->type_orig, nep->mass_dev, vel_dev));
         NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
+        if (pos_ready && s == n_steps - 1) NEP_CUDA(cudaEventRecord(pos_ready, st));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
         NEP_TRY(evaluate(nep, pos_dev));
@@ -1155,11 +1160,20 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
         NEP_CUDA(cudaMemcpyAsync(nep->h_type, type_host, sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, nep->stream));
         NEP_TRY(nep_neighbors(nep, n, nep->h_pos, nep->h_type, box, skin));
     }
-    NEP_TRY(md_step(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin));
-    NEP_CUDA(cudaMemcpyAsync(pos_host, nep->h_pos, b3, cudaMemcpyDeviceToHost, nep->stream));
+    if (!nep->copy_stream) {
+        NEP_CUDA(cudaStreamCreateWithFlags(&nep->copy_stream, cudaStreamNonBlocking));
+        NEP_CUDA(cudaEventCreateWithFlags(&nep->ev_pos, cudaEventDisableTiming));
+    }
+    // the positions are final after the last drift: their download (on a second stream) overlaps the last
+    // force evaluation; velocities, energies and forces follow on the compute stream
+    const Thermostat none = {0, 0.0, 0.0, 0.0, 0ull, 0};
+    NEP_TRY(md_loop(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin, none, nep->ev_pos));
+    NEP_CUDA(cudaStreamWaitEvent(nep->copy_stream, nep->ev_pos, 0));
+    NEP_CUDA(cudaMemcpyAsync(pos_host, nep->h_pos, b3, cudaMemcpyDeviceToHost, nep->copy_stream));
     NEP_CUDA(cudaMemcpyAsync(vel_host, nep->h_vel, b3, cudaMemcpyDeviceToHost, nep->stream));
     NEP_TRY(download_results(nep, energy_host, force_host, virial_host));
     NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->copy_stream));
     nep->h_run = true;
     return NEP_OK;
 }

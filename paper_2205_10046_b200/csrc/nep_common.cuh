@@ -144,6 +144,8 @@ struct nep_ctx {
     double* h_pos; double* h_vel; int* h_type;
     int64_t h_cap;
     bool h_run;              // an md_run_host trajectory is in progress (continuation allowed)
+    cudaStream_t copy_stream;   // md_run_host: second stream for the position download (created on first use)
+    cudaEvent_t ev_pos;         // ... recorded when the positions of the last step are final
 
     // bookkeeping of owned device memory (nep_device_bytes)
     struct { void* p; size_t bytes; } owned[96];
