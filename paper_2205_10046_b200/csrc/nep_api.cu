@@ -910,12 +910,18 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
         if (th.kind == 2)
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
                                                       2ull * (unsigned long long)(th.first_step + s), nep->type_orig, nep->mass_dev, vel_dev));
-        NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
+        // NVE: the closing half kick of step s - 1 is fused with the opening half kick + drift of step s
+        const bool fuse_kicks = th.kind == 0;
+        if (fuse_kicks && s > 0)
+            NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
+        else
+            NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         if (pos_ready && s == n_steps - 1) NEP_CUDA(cudaEventRecord(pos_ready, st));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
         NEP_TRY(evaluate(nep, pos_dev));
-        NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
+        if (!fuse_kicks || s == n_steps - 1)
+            NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
         if (th.kind == 2)
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
                                                       2ull * (unsigned long long)(th.first_step + s) + 1ull, nep->type_orig, nep->mass_dev, vel_dev));

@@ -1355,6 +1355,21 @@ __global__ void k_kick_drift(int n, double half_dt_conv, double dt, const int* _
     pos[t] += dt * v;
 }
 
+// second half kick of one step fused with the first half kick + drift of the next (NVE, same forces): the
+// two kicks are applied one after the other, exactly as the separate kernels would
+__global__ void k_kick_kick_drift(int n, double half_dt_conv, double dt, const int* __restrict__ type,
+                                  const double* __restrict__ mass, const double* __restrict__ f,
+                                  double* __restrict__ vel, double* __restrict__ pos)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 3 * n) return;
+    const double a = f[t] / mass[type[t / 3]];
+    double v = vel[t] + half_dt_conv * a;
+    v = v + half_dt_conv * a;
+    vel[t] = v;
+    pos[t] += dt * v;
+}
+
 __global__ void k_kick(int n, double half_dt_conv, const int* __restrict__ type, const double* __restrict__ mass,
                        const double* __restrict__ f, double* __restrict__ vel)
 {
