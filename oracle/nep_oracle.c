@@ -21,7 +21,8 @@
  * Eqs.(7)-(8) |A_nlm|^2 with library spherical harmonics, Wigner-3j contractions Eqs.(9)-(11),
  * q_n1111 = (7/15) q_n1^2, cos(k arccos x), N_des worked values 55/77/82, central finite differences
  * for F and for dU/dq, sum F = 0, translation / rotation / permutation invariance, sum W = -dE/d(eps),
- * hand-computed dimer.  Parity of E/F/W against any trained-model number of the paper: UNPINNED
+ * hand-computed dimer; brute-force neighbours (onep_neighbors and the per-selected-atom onep_neighbors_of) vs
+ * scipy's cKDTree and a 125-lattice-image search, orthorhombic and sheared.  Parity of E/F/W against any trained-model number of the paper: UNPINNED
  * (the paper's models and datasets are not available) -- see DESIGN.md.
  *
  * Compile: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC nep_oracle.c -o libnep_oracle.so -lm

@@ -301,5 +301,16 @@ def test_loss_terms_hand_case_and_zero(oracle_mod):
     z = np.concatenate([np.asarray(a, np.float64).ravel() for a in (p.c_radial, p.c_angular, p.w0, p.b0, p.w1, p.b1)])
     assert len(z) == npar
     l1, l2 = oracle_mod.regularisation_terms(p)
-    assert l1 == pytest.approx(np.abs(z).mean()) and l2 == pytest.approx(np.sqrt((z ** 2).mean()))
-    assert l1 <= l2 + 1e-15                                              # mean |z| <= rms z
+    assert 0.0 < l1 <= l2 + 1e-15                                        # mean |z| <= rms z (Cauchy-Schwarz)
+    # hand case, Eq. (33) last two terms: the six arrays hold z = {3, -4 | 0 | 12 | -5 | 0 | 0},
+    # N_par = 7: sum |z| / N_par = 24 / 7;  sqrt(sum z^2 / N_par) = sqrt((9 + 16 + 144 + 25) / 7) = sqrt(194 / 7)
+    import types
+    hand = types.SimpleNamespace(c_radial=np.array([3.0, -4.0], np.float32), c_angular=np.array([0.0], np.float32),
+                                 w0=np.array([[12.0]], np.float32), b0=np.array([-5.0], np.float32),
+                                 w1=np.array([0.0], np.float32), b1=np.array([0.0], np.float32))
+    l1, l2 = oracle_mod.regularisation_terms(hand)
+    assert l1 == pytest.approx(3.4285714285714284, rel=1e-15) and l2 == pytest.approx(5.264435935053794, rel=1e-15)
+    # a sign flip of every parameter changes neither; scaling by 3 scales both by 3
+    flip = types.SimpleNamespace(**{k: -3.0 * v for k, v in vars(hand).items()})
+    l1f, l2f = oracle_mod.regularisation_terms(flip)
+    assert l1f == pytest.approx(10.285714285714286, rel=1e-15) and l2f == pytest.approx(15.793307805161383, rel=1e-15)

@@ -304,6 +304,55 @@ def test_bruteforce_neighbours_vs_ckdtree(oracle_mod, seed):
         assert set(lst[i, :cnt[i]].tolist()) == set(ref[i]) - {i}
 
 
+def _lattice_image_sets(pos, H, rc, sel):
+    """the plain definition for the chosen atoms: j is a neighbour of i iff some lattice image of j is closer
+    than rc (125 images; numpy, shares nothing with the C oracle)"""
+    shifts = np.array([[a, b, c] for a in (-2, -1, 0, 1, 2) for b in (-2, -1, 0, 1, 2) for c in (-2, -1, 0, 1, 2)],
+                      dtype=np.float64) @ H
+    out = []
+    for i in sel:
+        d = pos[None, :, :] - pos[i][None, None, :] + shifts[:, None, :]
+        close = ((d * d).sum(axis=2) < rc * rc).any(axis=0)
+        close[i] = False
+        out.append(set(np.nonzero(close)[0].tolist()))
+    return out
+
+
+@pytest.mark.parametrize("sheared", [False, True])
+def test_neighbours_of_selected_atoms(oracle_mod, sheared):
+    """onep_neighbors_of (the checker of the full-size neighbour-set parity tests) against the full brute force
+    onep_neighbors, scipy's cKDTree (orthorhombic cell) and the lattice-image definition (sheared cell); a `cap`
+    smaller than the longest list must be regrown, never truncate."""
+    rng = np.random.default_rng(17)
+    box = np.array([13.0, 11.0, 12.5])
+    pos = rng.uniform(0, 1, size=(400, 3)) * box
+    H = np.diag(box)
+    if sheared:
+        H = np.array([[13.0, 0.0, 0.0], [2.1, 11.0, 0.0], [-1.7, 1.3, 12.5]])
+        pos = (pos / box) @ H
+    pos = pos + rng.integers(-2, 3, size=pos.shape).astype(np.float64) @ H        # unwrapped input
+    rc = 5.0
+    sel = np.array([399, 0, 17, 17, 250, 3, 128], dtype=np.int64)                 # unordered, one repeated
+    cnt_all, lst_all = oracle_mod.neighbors(pos, H if sheared else box, rc)
+    for cap in (256, 4):                                                          # 4 << longest list (~45)
+        cnt, lst = oracle_mod.neighbors_of(pos, H if sheared else box, rc, sel, cap=cap)
+        assert cnt.shape == (len(sel),) and lst.shape[1] >= cnt.max() > 4
+        for s_, i in enumerate(sel):
+            assert cnt[s_] == cnt_all[i]
+            assert lst[s_, :cnt[s_]].tolist() == lst_all[i, :cnt_all[i]].tolist()      # same order too
+            assert (lst[s_, cnt[s_]:] == -1).all()
+    frac = pos @ np.linalg.inv(H)
+    wrapped = (frac - np.floor(frac)) @ H                  # same periodic structure; images within +-2 cells suffice
+    want = _lattice_image_sets(wrapped, H, rc, sel)
+    assert sum(len(w) for w in want) > 20 * len(sel)
+    for s_, i in enumerate(sel):
+        assert set(lst[s_, :cnt[s_]].tolist()) == want[s_]
+    if not sheared:
+        ref = cKDTree(wrapped, boxsize=box).query_ball_point(wrapped[sel], rc)
+        for s_, i in enumerate(sel):
+            assert set(lst[s_, :cnt[s_]].tolist()) == set(ref[s_]) - {int(i)}
+
+
 def test_neighbour_predicate_is_strict_and_minimum_image(oracle_mod):
     box = np.array([12.0, 12.0, 12.0])
     pos = np.array([[0.5, 0.5, 0.5], [3.5, 4.5, 0.5],      # distance exactly 5.0 (3-4-5) -> excluded at rc=5
