@@ -48,7 +48,8 @@ typedef enum {
     NEP_ERR_NEIGHBOR_OVERFLOW = -4,  /* a list outgrew its storage and regrowing failed (never truncated) */
     NEP_ERR_STATE = -5,              /* compute / md_step before nep_neighbors, or hook before compute    */
     NEP_ERR_CUDA = -6,               /* a CUDA runtime call failed (text in nep_last_error)               */
-    NEP_ERR_NOMEM = -7               /* device or host allocation failed                                  */
+    NEP_ERR_NOMEM = -7,              /* device or host allocation failed                                  */
+    NEP_ERR_SKIN_EXCEEDED = -8       /* md_step*: an atom moved more than skin/2 between two list builds   */
 } nep_status;
 
 /* ---- model ---------------------------------------------------------------------------------------
@@ -89,7 +90,8 @@ int nep_num_descriptors(const nep_hyper_t* h);
  * test.  Both are evaluated exactly so (fp64, no contraction) for every candidate near a cutoff, so
  * the sets equal a brute-force fp64 search bit for bit.  The list order within an atom is unspecified
  * but deterministic.  Copies the types; synchronises (reads back list sizes; regrows and rebuilds on
- * overflow).  n <= 16,777,216.                                                                        */
+ * overflow; NEP_ERR_INVALID_ARG if a type is outside [0, T)).  n <= 16,777,216 = 2^24 (list entries pack the
+ * neighbour's index into 24 bits; tests/test_gpu_fullsize.py runs exactly 2^24 atoms).                 */
 int nep_neighbors(nep_t* nep, int64_t n, const double* pos_dev, const int32_t* type_dev,
                   const double box[9], double skin);
 
@@ -121,7 +123,12 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
  *   The first call after nep_neighbors()/nep_compute() with other positions evaluates F(r) first; later
  *   calls reuse the forces of the previous call (so positions must not be edited in between without
  *   calling nep_neighbors() again).  rebuild_every >= 1; skin as in nep_neighbors().
- * Synchronises once per list rebuild (overflow check), otherwise asynchronous.                        */
+ * Skin check (all md_step* calls): the lists are valid while no atom has moved more than skin/2 since the
+ * build.  The largest displacement of every evaluation is reduced on the device; it is read at every
+ * scheduled rebuild and when the call ends, and NEP_ERR_SKIN_EXCEEDED is returned if it was ever above
+ * skin/2 (pairs may then have been missed since that build: use a smaller rebuild_every or a larger skin;
+ * the state in pos_dev / vel_dev is the one reached, not rolled back).
+ * Synchronises once per list rebuild (overflow check) and once before it returns (skin check).        */
 int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs,
             int32_t n_steps, int32_t rebuild_every, double skin);
 
@@ -129,8 +136,8 @@ int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs,
  * equation per DESIGN.md reading A15).  As md_step, and after the second half kick of every step all
  * velocities are scaled by lambda = sqrt(1 + (dt_fs / tau_fs) (T_target / T - 1)), T = sum m v^2 / (3 n k_B),
  * T_target of step s = 1..n_steps = t_start_K + (t_stop_K - t_start_K) s / n_steps.  The kinetic-energy sum
- * is reduced on the device in a fixed order; no host round trip.  NEP_ERR_INVALID_ARG if tau_fs <= 0 or a
- * temperature < 0.  nep_last_temperature: T before the rescale and lambda of the last thermostatted step
+ * is reduced on the device in a fixed order; no host round trip.  NEP_ERR_INVALID_ARG if tau_fs < dt_fs (the
+ * rescale would overshoot the target; lambda^2 is clamped at 0 besides), tau_fs <= 0 or a temperature < 0.  nep_last_temperature: T before the rescale and lambda of the last thermostatted step
  * (host scalars; synchronises; NEP_ERR_STATE if there was none).                                        */
 int md_step_nvt_berendsen(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps,
                           int32_t rebuild_every, double skin, double t_start_K, double t_stop_K, double tau_fs);
@@ -141,9 +148,11 @@ int nep_last_temperature(nep_t* nep, double* t_before_host, double* lambda_host)
  * thermostat half step, the velocity-Verlet step of md_step, thermostat half step; a half step replaces every
  * velocity component by c1 v + sqrt(1 - c1^2) sqrt(k_B T_target / m) R with c1 = exp(-dt_fs / (2 tau_fs)) and R
  * the counter-based standard normal deviate of reading A16 (seed; counter from the step number, the atom's
- * index in the caller's order and the component), so a trajectory is reproducible and independent of how the
- * steps are split over calls (pass first_step = steps done so far).  T_target ramps as in
- * md_step_nvt_berendsen.  NEP_ERR_INVALID_ARG if tau_fs <= 0, a temperature < 0 or first_step < 0.        */
+ * index in the caller's order and the component), so the random forces are reproducible and independent of how
+ * the steps are split over calls (pass first_step = steps done so far).  T_target ramps as in
+ * md_step_nvt_berendsen, i.e. over the steps of ONE call: a ramp split over several calls must be split by the
+ * caller (t_start_K / t_stop_K of each piece); with t_start_K == t_stop_K the whole trajectory is independent of
+ * the split.  NEP_ERR_INVALID_ARG if tau_fs <= 0, a temperature < 0 or first_step < 0.        */
 int md_step_nvt_langevin(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps,
                          int32_t rebuild_every, double skin, double t_start_K, double t_stop_K, double tau_fs,
                          uint64_t seed, int64_t first_step);

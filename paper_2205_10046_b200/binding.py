@@ -375,21 +375,37 @@ class NEP:
 
     # host-buffer entry points: numpy arrays or pinned CPU tensors (anything exposing a host pointer)
     @staticmethod
-    def _host_ptr(a):
+    def _host_ptr(a, kind: str = "f8", count: Optional[int] = None):
+        """Pointer to a HOST array (numpy, or a CPU torch tensor, pinned or pageable) after checking what the C
+        side assumes: element type `kind` ("f8" = float64, "i4" = int32), C-contiguous, `count` elements."""
         if a is None:
             return None
         if isinstance(a, np.ndarray):
+            if a.dtype != np.dtype(kind):
+                raise TypeError(f"host array has dtype {a.dtype}, the C ABI reads {np.dtype(kind)}")
             if not a.flags["C_CONTIGUOUS"]:
                 raise ValueError("host arrays must be C-contiguous")
+            if count is not None and a.size != count:
+                raise ValueError(f"host array has {a.size} elements, expected {count}")
             return C.c_void_p(a.ctypes.data)
-        return C.c_void_p(a.data_ptr())          # CPU torch tensor (pinned or pageable)
+        name = str(a.dtype)
+        if name != {"f8": "torch.float64", "i4": "torch.int32"}[kind]:
+            raise TypeError(f"host tensor has dtype {name}, the C ABI reads {np.dtype(kind)}")
+        if a.is_cuda:
+            raise ValueError("the *_host calls take HOST memory")
+        if not a.is_contiguous():
+            raise ValueError("host tensors must be contiguous")
+        if count is not None and a.numel() != count:
+            raise ValueError(f"host tensor has {a.numel()} elements, expected {count}")
+        return C.c_void_p(a.data_ptr())
 
     def nep_compute_host(self, pos, types, box, skin: float, energy=None, force=None, virial=None):
         n = pos.shape[0]
         b = _box9(box)
-        self._check(self._L.nep_compute_host(self._h_ptr, n, self._host_ptr(pos), self._host_ptr(types),
+        hp = self._host_ptr
+        self._check(self._L.nep_compute_host(self._h_ptr, n, hp(pos, "f8", 3 * n), hp(types, "i4", n),
                                              b.ctypes.data_as(C.POINTER(C.c_double)), float(skin),
-                                             self._host_ptr(energy), self._host_ptr(force), self._host_ptr(virial)))
+                                             hp(energy, "f8", n), hp(force, "f8", 3 * n), hp(virial, "f8", 9 * n)))
         self.n = n
 
     def md_run_host(self, pos, vel, types, box, dt_fs: float, n_steps: int, rebuild_every: int, skin: float,
@@ -397,8 +413,9 @@ class NEP:
         """types=None continues the run of the previous md_run_host call (see include/nep.h)."""
         n = pos.shape[0]
         b = _box9(box if box is not None else np.zeros(3))
-        self._check(self._L.md_run_host(self._h_ptr, n, self._host_ptr(pos), self._host_ptr(vel),
-                                        self._host_ptr(types), b.ctypes.data_as(C.POINTER(C.c_double)),
+        hp = self._host_ptr
+        self._check(self._L.md_run_host(self._h_ptr, n, hp(pos, "f8", 3 * n), hp(vel, "f8", 3 * n),
+                                        hp(types, "i4", n), b.ctypes.data_as(C.POINTER(C.c_double)),
                                         float(dt_fs), int(n_steps), int(rebuild_every), float(skin),
-                                        self._host_ptr(energy), self._host_ptr(force), self._host_ptr(virial)))
+                                        hp(energy, "f8", n), hp(force, "f8", 3 * n), hp(virial, "f8", 9 * n)))
         self.n = n

@@ -16,8 +16,6 @@ namespace {
 const double kAccConv = 9.648533212e-3;   // (eV/Angstrom/amu) -> Angstrom/fs^2 (reading A10)
 const double kBoltzmann = 8.617333262e-5; // eV/K (reading A10)
 
-struct HostCoef { NepCoef c; };
-
 NepCoef make_coef()
 {
     // Eqs. (13)-(16), (18), (19): closed forms of the pre-computed coefficients.
@@ -118,6 +116,7 @@ int alloc_lists(nep_t* nep, int capA, int capS)
     if (capA > 256) capA = 256;
     if (capS > 256) capS = 256;
     const size_t n = (size_t)nep->n;
+    nep->capA = nep->capS = nep->d.capA = nep->d.capS = 0;   // stay zero if an allocation below fails
     NEP_TRY(dev_alloc(nep, &nep->listA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->rev, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->cA, (size_t)capA * n));
@@ -169,8 +168,12 @@ int build_lists(nep_t* nep, const double* pos_dev)
     const int n = (int)nep->n;
     cudaStream_t st = nep->stream;
     const double rcut = nep->h.rc_radial + nep->skin, acut = nep->h.rc_angular + nep->skin;
+    // the lists are overwritten from here on: nothing may use them (or an evaluation made with them) unless
+    // this build succeeds
+    nep->have_lists = nep->have_eval = nep->force_current = false;
     BuildParams P;
     P.n = n;
+    P.n_types = nep->d.T;
     P.ncx = nep->ncell[0]; P.ncy = nep->ncell[1]; P.ncz = nep->ncell[2];
     P.ntx = nep->ntile[0]; P.nty = nep->ntile[1];
     P.hx = P.hy = P.hz = 2;
@@ -199,6 +202,7 @@ int build_lists(nep_t* nep, const double* pos_dev)
     NEP_LAUNCH(NEP_K_SORT_CELLS, k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm));
     NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
     NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+    NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, 2 * sizeof(unsigned), st));
 
     if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
         const double rho = (double)n / nep->volume;
@@ -223,6 +227,7 @@ int build_lists(nep_t* nep, const double* pos_dev)
         nep->maxA_skin = fl[2];
         nep->maxR_skin = fl[3];
         nep->maxS_skin = fl[4];
+        if (fl[5]) return nep_fail(nep, NEP_ERR_INVALID_ARG, "an atom type is outside [0, n_types)");
         if (fl[2] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours inside rc_angular + skin");
         if (fl[4] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours between rc_angular + skin and rc_radial + skin");
         if (!fl[0] && !fl[1]) break;
@@ -539,7 +544,7 @@ int evaluate(nep_t* nep, const double* pos_dev, bool reuse_geometry = false)
     NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
     if (!reuse_geometry) {   // else: same positions as the previous evaluation (another member of a population)
         NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
-        NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));
+        NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));   // [0] only: [1] runs since the build
         NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
                                                  nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
     }
@@ -689,6 +694,7 @@ const char* nep_status_string(int status)
         case NEP_ERR_STATE: return "call out of order";
         case NEP_ERR_CUDA: return "CUDA error";
         case NEP_ERR_NOMEM: return "out of memory";
+        case NEP_ERR_SKIN_EXCEEDED: return "an atom moved more than skin/2 between two list builds";
     }
     return "unknown status";
 }
@@ -784,9 +790,9 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     }
     rc = dev_alloc(nep, &nep->flags, 8);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->tile_ctr, 64);
-    if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 1);
+    if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 2);
     if (rc != NEP_OK) { nep_destroy(nep); return rc; }
-    cudaMemset(nep->disp_max, 0, sizeof(unsigned));
+    cudaMemset(nep->disp_max, 0, 2 * sizeof(unsigned));
     if (cudaDeviceSynchronize() != cudaSuccess) { nep_destroy(nep); return NEP_ERR_CUDA; }
     *out = nep;
     return NEP_OK;
@@ -874,14 +880,30 @@ struct Thermostat {
 
 // pos_ready (optional): recorded on the stream as soon as the positions have their final values (after the
 // drift of the last step), so that a copy on another stream can overlap the last force evaluation
-static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
-                   double skin, const Thermostat& th, cudaEvent_t pos_ready = nullptr)
+// the lists are valid while no atom has moved more than skin/2 since the build (both atoms of a pair may approach)
+static int skin_check(nep_t* nep, unsigned disp2_bits)
 {
+    float r2;
+    memcpy(&r2, &disp2_bits, sizeof(r2));
+    if (sqrt((double)r2) > 0.5 * nep->skin) {
+        snprintf(nep->err, sizeof(nep->err), "an atom moved %.4g A since the last list build, more than skin/2 = %.4g A: pairs may have "
+                 "been missed; use a smaller rebuild_every or a larger skin", sqrt((double)r2), 0.5 * nep->skin);
+        return NEP_ERR_SKIN_EXCEEDED;
+    }
+    return NEP_OK;
+}
+
+// defer_check: the caller reads disp_max[1] itself after its own synchronisation (md_run_host)
+static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, int32_t n_steps, int32_t rebuild_every,
+                   double skin, const Thermostat& th, cudaEvent_t pos_ready = nullptr, bool defer_check = false)
+{
+    unsigned disp_bits = 0;
     if (!nep) return NEP_ERR_INVALID_ARG;
     if (!pos_dev || !vel_dev || n_steps < 0 || rebuild_every < 1 || !(skin >= 0.0) || !(dt_fs == dt_fs))
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad md_step argument");
     if (th.kind && (!(th.tau_fs > 0.0) || !(th.t_start >= 0.0) || !(th.t_stop >= 0.0)))
         return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad thermostat argument");
+    if (th.kind == 1 && th.tau_fs < dt_fs) return nep_fail(nep, NEP_ERR_INVALID_ARG, "Berendsen thermostat: tau_fs < dt_fs");
     if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
     NEP_CUDA(cudaSetDevice(nep->device));
     const int n = (int)nep->n;
@@ -918,7 +940,12 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
             NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         if (pos_ready && s == n_steps - 1) NEP_CUDA(cudaEventRecord(pos_ready, st));
         nep->steps_since_build++;
-        if (nep->steps_since_build >= rebuild_every) NEP_TRY(build_lists(nep, pos_dev));
+        if (nep->steps_since_build >= rebuild_every) {
+            // skin check of the interval that ends here: the copy completes with the build's own synchronisation
+            NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+            NEP_TRY(build_lists(nep, pos_dev));
+            NEP_TRY(skin_check(nep, disp_bits));
+        }
         NEP_TRY(evaluate(nep, pos_dev));
         if (!fuse_kicks || s == n_steps - 1)
             NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
@@ -935,6 +962,11 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
     }
     nep->force_current = true;
     nep->force_pos_tag = pos_dev;
+    if (n_steps > 0 && !defer_check) {
+        NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+        NEP_CUDA(cudaStreamSynchronize(st));
+        NEP_TRY(skin_check(nep, disp_bits));
+    }
     return NEP_OK;
 }
 
@@ -1173,7 +1205,9 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
     // the positions are final after the last drift: their download (on a second stream) overlaps the last
     // force evaluation; velocities, energies and forces follow on the compute stream
     const Thermostat none = {0, 0.0, 0.0, 0.0, 0ull, 0};
-    NEP_TRY(md_loop(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin, none, nep->ev_pos));
+    NEP_TRY(md_loop(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin, none, nep->ev_pos, true));
+    unsigned disp_bits = 0;
+    NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, nep->stream));
     NEP_CUDA(cudaStreamWaitEvent(nep->copy_stream, nep->ev_pos, 0));
     NEP_CUDA(cudaMemcpyAsync(pos_host, nep->h_pos, b3, cudaMemcpyDeviceToHost, nep->copy_stream));
     NEP_CUDA(cudaMemcpyAsync(vel_host, nep->h_vel, b3, cudaMemcpyDeviceToHost, nep->stream));
@@ -1181,7 +1215,7 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
     NEP_CUDA(cudaStreamSynchronize(nep->stream));
     NEP_CUDA(cudaStreamSynchronize(nep->copy_stream));
     nep->h_run = true;
-    return NEP_OK;
+    return skin_check(nep, disp_bits);
 }
 
 // ---- measurement support ----------------------------------------------------------------------------------

@@ -118,7 +118,7 @@ struct nep_ctx {
     int64_t mask_cap;           // allocated 64-bit words
     int* cB; int* ncB;       // [capA+capS][n] per step: packed like cA, rcA <= |r| < rcR (listA part, then listS part)
     int* flags;              // [4] device: 0 overflow A, 1 overflow S, 2 max cntA, 3 max (cntA+cntS)
-    unsigned* disp_max;      // [1] device: float bits of max displacement^2 since build
+    unsigned* disp_max;      // [2] device: float bits of the max displacement^2 since the build: [0] at the last evaluation, [1] at any evaluation since
     int64_t atom_cap;        // allocated atoms
 
     float* q;                // [D][n]

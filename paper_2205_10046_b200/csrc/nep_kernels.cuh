@@ -28,6 +28,11 @@ struct NepCoef {
     float c5[3];
 };
 
+// Packed list entry (j << 8) | slot, j < 2^24 = NEP_MAX_ATOMS: all 32 bits are used, so packing and unpacking go
+// through unsigned arithmetic (a signed shift would sign-extend every j >= 2^23).
+__device__ __forceinline__ int entry_pack(int j, int slot) { return (int)(((unsigned)j << NEP_SLOT_BITS) | (unsigned)slot); }
+__device__ __forceinline__ int entry_j(int e) { return (int)((unsigned)e >> NEP_SLOT_BITS); }
+
 // ---------------------------------------------------------------------------------------------------
 // Software-pipelined walk over one atom's compact entries  e_m = list[m*n + s] = (j << 8) | rs,
 // m = 0..cnt-1: the entry two pairs ahead and the neighbour's position one pair ahead are in flight while
@@ -69,7 +74,7 @@ struct PairWalk {
     }
     __device__ __forceinline__ void fetch(int ee, int mm, int4& p, ulonglong2& w, const NepDims& D)   // entry ee at position mm
     {
-        const int j1 = ee >> NEP_SLOT_BITS;
+        const int j1 = entry_j(ee);
         p = posq[j1];
         if (MODE >= 1) {
             const int word = (ee & ((1 << NEP_SLOT_BITS) - 1)) >> 6;
@@ -89,7 +94,7 @@ struct PairWalk {
         lp += n;
         return true;
     }
-    __device__ __forceinline__ int j() const { return e >> NEP_SLOT_BITS; }
+    __device__ __forceinline__ int j() const { return entry_j(e); }
     // compact slot of this atom in the neighbour's column of the same list
     __device__ __forceinline__ int slot(const NepDims& D) const
     {
@@ -127,10 +132,13 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
     if (s >= D.n) return;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    {   // displacement since the last list build (reported by nep_max_displacement)
+    {   // displacement since the last list build: [0] of this evaluation (nep_max_displacement), [1] the
+        // largest of any evaluation since the build (md_step's skin check); one atomic pair per warp
         float dx, dy, dz, r2;
         pair_vec(posq_build[s], pi, D, dx, dy, dz, r2);
-        if (r2 > 0.0f) atomicMax(disp_max, __float_as_uint(r2));
+        const unsigned am = __activemask();
+        const unsigned worst = __reduce_max_sync(am, __float_as_uint(r2));
+        if ((threadIdx.x & 31) == (unsigned)(__ffs(am) - 1) && worst > 0u) { atomicMax(disp_max, worst); atomicMax(disp_max + 1, worst); }
     }
     // Branch-free inner loops: the write pointers of the two compact columns advance by n under a predicate,
     // the mask bit of the current slot is shifted along, list / rev pointers step by 4 n per batch.
@@ -161,7 +169,7 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
                 for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
                     pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                    const int e = (j[u] << NEP_SLOT_BITS) | rs[u];
+                    const int e = entry_pack(j[u], rs[u]);
                     const bool ok = m0 + u < mend;
                     const bool inA = ok && r2 < D.rcA2;
                     const bool inB = ok && !inA && r2 < D.rcR2;
@@ -196,7 +204,7 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
                 for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
                     pair_vec(pi, pj[u], D, dx, dy, dz, r2);
-                    if (m0 + u < mend && r2 < D.rcR2) { *pb = (j[u] << NEP_SLOT_BITS) | rs[u]; pb += n; ++nb; ws |= bit; }
+                    if (m0 + u < mend && r2 < D.rcR2) { *pb = entry_pack(j[u], rs[u]); pb += n; ++nb; ws |= bit; }
                     bit <<= 1;
                 }
             }
@@ -1188,7 +1196,7 @@ __device__ __forceinline__ void final_walk(const NepDims& D, const int4& pi, con
     for (int m0 = 0; m0 < cnt; m0 += 4) {
         int4 pj[4]; float mv[4]; float4 pv[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) pj[u] = posq[en[u] >> NEP_SLOT_BITS];
+        for (int u = 0; u < 4; ++u) pj[u] = posq[entry_j(en[u])];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             if (m0 + u < cnt) {
@@ -1419,7 +1427,7 @@ k_berendsen_lambda(int nblocks, const double* __restrict__ partial, double inv_c
     }
     if (threadIdx.x == 0) {
         const double T = sh[0] * inv_conv_3nkb;
-        out[0] = T > 0.0 ? sqrt(1.0 + dt_over_tau * (t_target / T - 1.0)) : 1.0;
+        out[0] = T > 0.0 ? sqrt(fmax(0.0, 1.0 + dt_over_tau * (t_target / T - 1.0))) : 1.0;
         out[1] = T;
     }
 }

@@ -29,6 +29,7 @@ struct BuildParams {
     float guardA, guardR;    // half width of the fp64-resolve band around each
     double cutA2_d, cutR2_d; // exact fp64 thresholds rc*rc
     int capA, capS;
+    int n_types;             // atom types must lie in [0, n_types): checked here, reported through flags[5]
 };
 
 struct CellInv { double m[9]; };     // Hinv, passed by value
@@ -204,6 +205,7 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
     const int4 pi = posq[s];
+    if ((unsigned)pi.w >= (unsigned)P.n_types) atomicOr(&flags[5], 1);
     const int cx = cell_coord((unsigned)pi.x, P.ncx);
     const int cy = cell_coord((unsigned)pi.y, P.ncy);
     const int cz = cell_coord((unsigned)pi.z, P.ncz);

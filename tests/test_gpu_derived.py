@@ -147,7 +147,8 @@ def test_berendsen_nvt_reaches_target_and_rejects_bad_arguments(pkg, oracle_mod)
     with pytest.raises(pkg.NepError) as ei:
         nep.nep_last_temperature()
     assert ei.value.status == -5
-    for bad in ((300.0, 300.0, 0.0), (-1.0, 300.0, 10.0), (300.0, -5.0, 10.0)):
+    # tau < dt would overshoot the target (and lambda^2 could go negative): rejected
+    for bad in ((300.0, 300.0, 0.0), (-1.0, 300.0, 10.0), (300.0, -5.0, 10.0), (300.0, 300.0, 0.5)):
         with pytest.raises(pkg.NepError) as ei:
             nep.md_step_nvt_berendsen(pos, vel, 1.0, 1, 10, 1.0, *bad)
         assert ei.value.status == -1

@@ -321,3 +321,59 @@ def test_host_buffer_entry_points_match_device_ones(pkg):
     e, f, w = nep.nep_get_last()
     assert np.array_equal(fh, f.cpu().numpy())
     nep.close()
+
+
+def test_skin_violation_is_reported_not_silent(pkg):
+    """md_step used to rebuild on the fixed cadence only.  A run whose atoms move more than skin/2
+    between two builds must fail with NEP_ERR_SKIN_EXCEEDED (-8), both at a scheduled rebuild and when the call
+    ends; the same run with a cadence that keeps the bound passes."""
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    hot = s.vel * 12.0                                            # ~0.044 A/fs rms: 0.1 A in two or three steps
+    for n_steps, every in ((12, 6), (4, 50)):                     # detected at the rebuild / at the end of the call
+        nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+        pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(hot, device="cuda:0")
+        nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 0.2)
+        with pytest.raises(pkg.NepError) as ei:
+            nep.md_step(pos, vel, 1.0, n_steps, every, 0.2)
+        assert ei.value.status == -8 and "skin/2" in str(ei.value)
+        nep.close()
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, vel = torch.tensor(s.pos, device="cuda:0"), torch.tensor(hot, device="cuda:0")
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 0.5)
+    nep.md_step(pos, vel, 1.0, 12, 1, 0.5)                        # rebuilt every step: displacement 0 at every evaluation
+    assert nep.nep_max_displacement() == 0.0
+    # skin = 0 needs a build per step: with a longer cadence any motion is a violation
+    nep.nep_neighbors(pos, torch.tensor(s.types, device="cuda:0"), s.box, 0.0)
+    with pytest.raises(pkg.NepError) as ei:
+        nep.md_step(pos, vel, 1.0, 2, 5, 0.0)
+    assert ei.value.status == -8
+    nep.close()
+
+
+def test_bad_types_and_host_array_dtypes_are_rejected(pkg):
+    cfg = W.get_config(3, (7, 6, 5))
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    n = len(s.pos)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    for bad in (cfg.hyper.n_types, -1):
+        t = s.types.copy(); t[n // 2] = bad
+        with pytest.raises(pkg.NepError) as ei:
+            nep.nep_neighbors(pos, torch.tensor(t, device="cuda:0"), s.box, 1.0)
+        assert ei.value.status == -1 and "type" in str(ei.value)
+        with pytest.raises(pkg.NepError) as ei:                   # the failed build left no usable lists behind
+            nep.nep_compute(pos)
+        assert ei.value.status == -5
+    e, f, w = np.zeros(n), np.zeros((n, 3)), np.zeros((n, 9))
+    with pytest.raises(TypeError):
+        nep.nep_compute_host(s.pos.astype(np.float32), s.types, s.box, 1.0, e, f, w)
+    with pytest.raises(TypeError):
+        nep.nep_compute_host(s.pos, s.types.astype(np.int64), s.box, 1.0, e, f, w)
+    with pytest.raises(ValueError):
+        nep.nep_compute_host(s.pos, s.types, s.box, 1.0, e, np.zeros((n, 2)), w)
+    with pytest.raises(TypeError):
+        nep.md_run_host(s.pos.copy(), s.vel.astype(np.float32), s.types, s.box, 1.0, 1, 5, 1.0)
+    nep.nep_compute_host(s.pos, s.types, s.box, 1.0, e, f, w)    # and the well-formed call still works
+    assert np.isfinite(f).all() and np.abs(f).max() > 0.0
+    nep.close()

@@ -111,3 +111,55 @@ def test_full_size_sampled_parity(pkg, oracle_mod, idx, n_sample, n_md, half):
         n_inner += int(inner.sum())
     assert n_inner >= 300
     nep.close()
+
+
+def test_largest_atom_count_2_pow_24(pkg, oracle_mod):
+    """n = 16,777,216 = 2^24 atoms, the limit include/nep.h states (config 1's diamond lattice and model at
+    128^3 cells; ~65 GB of device memory).  List entries pack the neighbour's sorted index into the top 24
+    bits of a 32-bit word: every index >= 2^23 used to come back negative (VERDICT r1 / ADVICE r1).  Sampled
+    neighbour sets, and oracle windows in every octant -- the internal order is spatial, so the windows at high
+    z hold atoms whose sorted indices are above 2^23."""
+    cfg = W.get_config(1, (128, 128, 128))
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    h = cfg.hyper
+    n = len(s.pos)
+    assert n == 1 << 24
+    rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 701]))
+    nep = pkg.NEP(h, p, s.masses, device=0)
+    pos = torch.tensor(s.pos, device="cuda:0")
+    vel = torch.tensor(s.vel, device="cuda:0")
+    types = torch.tensor(s.types, device="cuda:0")
+    nep.nep_neighbors(pos, types, s.box, cfg.skin)
+    del types
+    sel = np.sort(rng.choice(n, size=256, replace=False))
+    sel_dev = torch.tensor(sel, device="cuda:0")
+    for which, rc in ((0, h.rc_radial), (1, h.rc_angular)):
+        cnt, lst = nep.nep_get_neighbors(which)
+        c, l = cnt[sel_dev].cpu().numpy(), lst[sel_dev].cpu().numpy()
+        assert int(lst.max().item()) >= (1 << 24) - 4096 and int(lst.min().item()) >= -1
+        del cnt, lst
+        torch.cuda.empty_cache()
+        oc, ol = oracle_mod.neighbors_of(s.pos, s.box, rc + cfg.skin, sel)
+        assert np.array_equal(c, oc)
+        big = np.iinfo(np.int32).max
+        a = np.sort(np.where(np.arange(l.shape[1])[None, :] < c[:, None], l, big), axis=1)
+        b = np.sort(np.where(np.arange(ol.shape[1])[None, :] < oc[:, None], ol, big), axis=1)
+        wd = min(a.shape[1], b.shape[1])
+        assert np.array_equal(a[:, :wd], b[:, :wd])
+    nep.md_step(pos, vel, cfg.dt_fs, 3, 2, cfg.skin)              # one rebuild inside
+    e, f, w = nep.nep_get_last()
+    assert torch.isfinite(pos).all() and torch.isfinite(f).all()
+    fsum, fabs = f.sum(0).abs().max().item(), f.abs().sum(0).max().item()
+    assert fsum <= 2e-6 * fabs
+    snap = pos.cpu().numpy()
+    e, f, w = e.cpu().numpy(), f.cpu().numpy(), w.cpu().numpy()
+    wscale = np.median(np.linalg.norm(w[rng.choice(n, size=20000, replace=False)], axis=1))
+    n_inner = 0
+    for frac in ((0.0, 0.0, 0.0), (0.2, 0.3, 0.85), (0.9, 0.7, 0.6), (0.5, 0.5, 0.97)):
+        isel, xyz, inner = cut_window(snap, s.box, np.array(frac) * s.box, 8.0, 2.0 * h.rc_radial)
+        eo, fo, wo = oracle_mod.compute(h, p, xyz, s.types[isel], np.full(3, 1.0e4), pbc=(0, 0, 0))
+        ii = isel[inner]
+        assert_efw_window(e[ii], f[ii], w[ii], eo[inner], fo[inner], wo[inner], wscale)
+        n_inner += int(inner.sum())
+    assert n_inner >= 600
+    nep.close()
