@@ -12,7 +12,7 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
+_LIB_PATH = os.environ.get("NEP_B200_LIB") or os.path.join(_HERE, "libnep_b200.so")   # NEP_B200_LIB: another build of the same library (kernel experiments)
 _lib = None
 
 # every symbol include/nep.h declares

@@ -363,6 +363,7 @@ def test_bad_types_and_host_array_dtypes_are_rejected(pkg):
             nep.nep_neighbors(pos, torch.tensor(t, device="cuda:0"), s.box, 1.0)
         assert ei.value.status == -1 and "type" in str(ei.value)
         with pytest.raises(pkg.NepError) as ei:                   # the failed build left no usable lists behind
+            nep.n = n
             nep.nep_compute(pos)
         assert ei.value.status == -5
     e, f, w = np.zeros(n), np.zeros((n, 3)), np.zeros((n, 9))
