@@ -21,6 +21,7 @@
 #pragma once
 #include "nep_common.cuh"
 
+
 // Pre-computed coefficients of Eqs. (13)-(19), filled on the host at nep_create.
 struct NepCoef {
     float c3[NEP_NUM_S];
@@ -487,11 +488,13 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
     constexpr int N4 = (NCH + 3) / 4;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    float S[NCH][NEP_NUM_S];
+    // S_nk accumulators as 12 packed pairs per channel: S += g_n * (b_k, b_k+1) is one FFMA2 (sm_100 packed fp32,
+    // scalar g broadcast) instead of two FFMA -- the kernel is bound by issue slots, not by the FMA pipe
+    float2 S2[NCH][NEP_NUM_S / 2];
 #pragma unroll
     for (int a = 0; a < NCH; ++a)
 #pragma unroll
-        for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = 0.0f;
+        for (int k = 0; k < NEP_NUM_S / 2; ++k) S2[a][k] = make_float2(0.0f, 0.0f);
     const float* tab_i = tab + (size_t)(pi.w * D.T) * tab_stride;
     PairWalk<0> w(cA, n, s, ncA[s], posq, D);
     while (w.next(D)) {
@@ -519,9 +522,11 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
         float b[NEP_NUM_S];
         angular_b(dx * rinv, dy * rinv, dz * rinv, b);
 #pragma unroll
-        for (int a = 0; a < NCH; ++a)
+        for (int a = 0; a < NCH; ++a) {
+            const float2 ga = make_float2(g[a], g[a]);
 #pragma unroll
-            for (int k = 0; k < NEP_NUM_S; ++k) S[a][k] = fmaf(g[a], b[k], S[a][k]);
+            for (int k = 0; k < NEP_NUM_S / 2; ++k) S2[a][k] = __ffma2_rn(ga, make_float2(b[2 * k], b[2 * k + 1]), S2[a][k]);
+        }
     }
     float* qa = q + (size_t)D.NR * n + s;                  // angular blocks: qa[(blk * NA + nn) * n]
     float* Sp = S_out + (size_t)(n0 * NEP_NUM_S) * n + s;
@@ -529,8 +534,11 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
     for (int a = 0; a < NCH; ++a) {
         const int nn = n0 + a;
         if (nn < D.NA) {
+            float Sa[NEP_NUM_S];
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S / 2; ++k) { Sa[2 * k] = S2[a][k].x; Sa[2 * k + 1] = S2[a][k].y; }
             float out[6];
-            q_from_S(S[a], C, out);
+            q_from_S(Sa, C, out);
             float* qp = qa + (size_t)nn * n;
             const size_t blk = (size_t)D.NA * n;
 #pragma unroll
@@ -538,7 +546,7 @@ __device__ __forceinline__ void angular_atom(const NepDims& D, const NepCoef& C,
             if (D.has4) { *qp = out[4]; qp += blk; }
             if (D.has5) *qp = out[5];
 #pragma unroll
-            for (int k = 0; k < NEP_NUM_S; ++k) { *Sp = S[a][k]; Sp += n; }
+            for (int k = 0; k < NEP_NUM_S; ++k) { *Sp = Sa[k]; Sp += n; }
         }
     }
 }
@@ -630,6 +638,16 @@ k_ann(NepDims D, const float* __restrict__ q, const float* __restrict__ w0p, con
 // per block into shared memory, in two layouts whose row strides make the B-fragment reads of the forward
 // (stride = 12 mod 32) and of the backward pass (stride = 8 mod 32) bank-conflict-free; cf passes through
 // a per-warp shared tile (C-fragment layout -> A-fragment layout).  Fragment layouts: PTX ISA, mma.m16n8k8.
+// tanh(x) = 1 - 2 / (exp(2x) + 1) with the hardware exp2 and reciprocal (MUFU.EX2, MUFU.RCP): absolute error
+// ~1e-7 over the whole range (exact limits +-1), 6 instructions instead of tanhf's ~20; the network's energy bar is
+// 1e-5 eV absolute and |w1| < 1.
+__device__ __forceinline__ float tanh_fast(float x)
+{
+    float e;                                               // exp(2x) = 2^(2x log2 e)
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.885390081777927f));
+    return 1.0f - __fdividef(2.0f, e + 1.0f);
+}
+
 __device__ __forceinline__ void tf32_split(float x, unsigned& hi, unsigned& lo)
 {
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
@@ -711,7 +729,7 @@ k_ann_tc(NepDims D, int HP, const float* __restrict__ q, const float* __restrict
             const float w1a = sw1[nt * 8 + 2 * t4], w1b = sw1[nt * 8 + 2 * t4 + 1];
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                const float x0 = tanhf(c[mt][0]), x1 = tanhf(c[mt][1]), x2 = tanhf(c[mt][2]), x3 = tanhf(c[mt][3]);
+                const float x0 = tanh_fast(c[mt][0]), x1 = tanh_fast(c[mt][1]), x2 = tanh_fast(c[mt][2]), x3 = tanh_fast(c[mt][3]);
                 e[mt][0] = fmaf(w1a, x0, fmaf(w1b, x1, e[mt][0]));
                 e[mt][1] = fmaf(w1a, x2, fmaf(w1b, x3, e[mt][1]));
                 float* r0 = scf + (mt * 16 + g) * SC + nt * 8 + 2 * t4;
@@ -816,9 +834,10 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
 {
     constexpr int NT = NCH + NSM;
     constexpr int N4 = (NT + 3) / 4;
+    constexpr bool PACKED = NSM > 0;
     const size_t n = (size_t)D.n;
     const int4 pi = posq[s];
-    float G[NCH][NEP_NUM_S];
+    float2 G2[NCH][NEP_NUM_S / 2];                          // G_nk in pairs (k, k+1): see NEP_AB
     {
         const float* fpa = fp + (size_t)D.NR * n + s;          // angular blocks: fpa[(blk * NA + nn) * n]
         const size_t blk = (size_t)D.NA * n;
@@ -843,7 +862,7 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
             }
 #pragma unroll
             for (int k = 0; k < NEP_NUM_S; ++k) {
-                if (a < NCH) G[a < NCH ? a : 0][k] = Gt[k];
+                if (a < NCH) { if (k & 1) G2[a < NCH ? a : 0][k >> 1].y = Gt[k]; else G2[a < NCH ? a : 0][k >> 1].x = Gt[k]; }
                 else myG[((a - NCH) * NEP_NUM_S + k) * 128] = Gt[k];
             }
         }
@@ -859,17 +878,23 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         const float* c4 = tab_i + w.pj.w * tab_stride;
         float g[4 * N4], dg[NT];
         load_row<NT>(c4, g);                              // csum'
-#pragma unroll
-        for (int a = 0; a < NT; ++a) dg[a] = 0.0f;
         {
+            // (G0_n, G1_n) += c_nk (T_k, T_k'): one FFMA2 per channel and k (scalar c broadcast)
+            float2 gd[NT];
+#pragma unroll
+            for (int a = 0; a < NT; ++a) gd[a] = make_float2(g[a], 0.0f);
             float Tkm1 = 1.0f, Tk = h.x, Dkm1 = 0.0f, Dk = 1.0f;      // T_0,T_1 ; T_0',T_1'
             for (int r0 = 1; r0 < D.KAR; r0 += 4) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     float c[4 * N4];
                     load_row<NT>(c4 + (r0 + u) * (4 * N4), c);
+                    const float2 td = make_float2(Tk, Dk);
 #pragma unroll
-                    for (int a = 0; a < NT; ++a) { g[a] = fmaf(c[a], Tk, g[a]); dg[a] = fmaf(c[a], Dk, dg[a]); }
+                    for (int a = 0; a < NT; ++a) {
+                        if (PACKED) gd[a] = __ffma2_rn(make_float2(c[a], c[a]), td, gd[a]);
+                        else { gd[a].x = fmaf(c[a], td.x, gd[a].x); gd[a].y = fmaf(c[a], td.y, gd[a].y); }
+                    }
                     const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1));
                     const float Tn = fmaf(h.two_x, Tk, -Tkm1);
                     Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
@@ -877,9 +902,9 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
             }
 #pragma unroll
             for (int a = 0; a < NT; ++a) {
-                const float G0 = g[a];
+                const float G0 = gd[a].x;
                 g[a] = G0 * h.hfc;
-                dg[a] = fmaf(G0, h.hdfc, dg[a] * h.hfc_dx);
+                dg[a] = fmaf(G0, h.hdfc, gd[a].y * h.hfc_dx);
             }
         }
         const float x = dx * rinv, y = dy * rinv, z = dz * rinv;
@@ -887,42 +912,70 @@ __device__ __forceinline__ void force_angular_atom(const NepDims& D, const NepCo
         angular_b(x, y, z, b);
         float cu = 0.0f, vx = 0.0f, vy = 0.0f, vz = 0.0f;
         const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z, xyz = xy * z;
-        // ACC(k, l, gradP_k(u)): A_k, B_k, then the two sums
-#define NEP_ACC(k, l, gx, gy, gz)                                                                  \
+        // NEP_AB(kp): (A_k, A_k+1) and (B_k, B_k+1) for k = 2 kp.  PACKED: A += g_n (G_nk, G_nk+1) as one FFMA2 with the
+        // scalar g_n broadcast (sm_100 packed fp32).  Measured: with all G in registers (NSM = 0, two warps
+        // per scheduler) the packed form is SLOWER (607 -> 645 us at 1M atoms: the kernel waits on dependent chains, not
+        // on issue slots); with channels in shared memory (NSM > 0) it is 3 % faster -- hence PACKED = NSM > 0.
+        // NEP_USE(k, l, A, B, gradP_k(u)): the two sums.
+#define NEP_AB_STEP(kp, a)                                                                         \
+            if (PACKED) {                                                                           \
+                A2_##kp = __ffma2_rn(make_float2(g[a], g[a]), G2[a][kp], A2_##kp);                  \
+                B2_##kp = __ffma2_rn(make_float2(dg[a], dg[a]), G2[a][kp], B2_##kp);                \
+            } else {                                                                                \
+                A2_##kp.x = fmaf(g[a], G2[a][kp].x, A2_##kp.x); A2_##kp.y = fmaf(g[a], G2[a][kp].y, A2_##kp.y);     \
+                B2_##kp.x = fmaf(dg[a], G2[a][kp].x, B2_##kp.x); B2_##kp.y = fmaf(dg[a], G2[a][kp].y, B2_##kp.y);   \
+            }
+#define NEP_AB(kp)                                                                                 \
+        float2 A2_##kp = make_float2(0.0f, 0.0f), B2_##kp = make_float2(0.0f, 0.0f);                \
+        _Pragma("unroll") for (int a = 0; a < NCH; ++a) { NEP_AB_STEP(kp, a) }                     \
+        _Pragma("unroll") for (int a = 0; a < NSM; ++a) {                                          \
+            const float2 Gs = make_float2(myG[(a * NEP_NUM_S + 2 * (kp)) * 128], myG[(a * NEP_NUM_S + 2 * (kp) + 1) * 128]); \
+            A2_##kp = __ffma2_rn(make_float2(g[NCH + a], g[NCH + a]), Gs, A2_##kp);                 \
+            B2_##kp = __ffma2_rn(make_float2(dg[NCH + a], dg[NCH + a]), Gs, B2_##kp); }
+#define NEP_USE(k, l, A, B, gx, gy, gz)                                                            \
         {                                                                                           \
-            float A = 0.0f, B = 0.0f;                                                               \
-            _Pragma("unroll") for (int a = 0; a < NCH; ++a) { A = fmaf(G[a][k], g[a], A); B = fmaf(G[a][k], dg[a], B); } \
-            _Pragma("unroll") for (int a = 0; a < NSM; ++a) {                                      \
-                const float Gs = myG[(a * NEP_NUM_S + (k)) * 128];                                  \
-                A = fmaf(Gs, g[NCH + a], A); B = fmaf(Gs, dg[NCH + a], B); }                        \
-            cu = fmaf(fmaf(-(float)(l) * rinv, A, B), b[k], cu);                                    \
-            vx = fmaf(A, (gx), vx); vy = fmaf(A, (gy), vy); vz = fmaf(A, (gz), vz);                 \
+            cu = fmaf(fmaf(-(float)(l) * rinv, (A), (B)), b[k], cu);                                \
+            vx = fmaf((A), (gx), vx); vy = fmaf((A), (gy), vy); vz = fmaf((A), (gz), vz);           \
         }
-        NEP_ACC(0, 1, 0.0f, 0.0f, 1.0f)
-        NEP_ACC(1, 1, 1.0f, 0.0f, 0.0f)
-        NEP_ACC(2, 1, 0.0f, 1.0f, 0.0f)
-        NEP_ACC(3, 2, -2.0f * x, -2.0f * y, 4.0f * z)
-        NEP_ACC(4, 2, z, 0.0f, x)
-        NEP_ACC(5, 2, 0.0f, z, y)
-        NEP_ACC(6, 2, 2.0f * x, -2.0f * y, 0.0f)
-        NEP_ACC(7, 2, 2.0f * y, 2.0f * x, 0.0f)
-        NEP_ACC(8, 3, -6.0f * xz, -6.0f * yz, -3.0f * (x2 + y2 - 2.0f * z2))
-        NEP_ACC(9, 3, -3.0f * x2 - y2 + 4.0f * z2, -2.0f * xy, 8.0f * xz)
-        NEP_ACC(10, 3, -2.0f * xy, -x2 - 3.0f * y2 + 4.0f * z2, 8.0f * yz)
-        NEP_ACC(11, 3, 2.0f * xz, -2.0f * yz, x2 - y2)
-        NEP_ACC(12, 3, 2.0f * yz, 2.0f * xz, 2.0f * xy)
-        NEP_ACC(13, 3, 3.0f * (x2 - y2), -6.0f * xy, 0.0f)
-        NEP_ACC(14, 3, 6.0f * xy, 3.0f * (x2 - y2), 0.0f)
-        NEP_ACC(15, 4, 12.0f * x * (x2 + y2 - 4.0f * z2), 12.0f * y * (x2 + y2 - 4.0f * z2), -16.0f * z * (3.0f * x2 + 3.0f * y2 - 2.0f * z2))
-        NEP_ACC(16, 4, -z * (9.0f * x2 + 3.0f * y2 - 4.0f * z2), -6.0f * xyz, -3.0f * x * (x2 + y2 - 4.0f * z2))
-        NEP_ACC(17, 4, -6.0f * xyz, -z * (3.0f * x2 + 9.0f * y2 - 4.0f * z2), -3.0f * y * (x2 + y2 - 4.0f * z2))
-        NEP_ACC(18, 4, -4.0f * x * (x2 - 3.0f * z2), 4.0f * y * (y2 - 3.0f * z2), 12.0f * z * (x2 - y2))
-        NEP_ACC(19, 4, -2.0f * y * (3.0f * x2 + y2 - 6.0f * z2), -2.0f * x * (x2 + 3.0f * y2 - 6.0f * z2), 24.0f * xyz)
-        NEP_ACC(20, 4, 3.0f * z * (x2 - y2), -6.0f * xyz, x * (x2 - 3.0f * y2))
-        NEP_ACC(21, 4, 6.0f * xyz, 3.0f * z * (x2 - y2), y * (3.0f * x2 - y2))
-        NEP_ACC(22, 4, 4.0f * x * (x2 - 3.0f * y2), -4.0f * y * (3.0f * x2 - y2), 0.0f)
-        NEP_ACC(23, 4, 4.0f * y * (3.0f * x2 - y2), 4.0f * x * (x2 - 3.0f * y2), 0.0f)
-#undef NEP_ACC
+        NEP_AB(0)
+        NEP_USE(0, 1, A2_0.x, B2_0.x, 0.0f, 0.0f, 1.0f)
+        NEP_USE(1, 1, A2_0.y, B2_0.y, 1.0f, 0.0f, 0.0f)
+        NEP_AB(1)
+        NEP_USE(2, 1, A2_1.x, B2_1.x, 0.0f, 1.0f, 0.0f)
+        NEP_USE(3, 2, A2_1.y, B2_1.y, -2.0f * x, -2.0f * y, 4.0f * z)
+        NEP_AB(2)
+        NEP_USE(4, 2, A2_2.x, B2_2.x, z, 0.0f, x)
+        NEP_USE(5, 2, A2_2.y, B2_2.y, 0.0f, z, y)
+        NEP_AB(3)
+        NEP_USE(6, 2, A2_3.x, B2_3.x, 2.0f * x, -2.0f * y, 0.0f)
+        NEP_USE(7, 2, A2_3.y, B2_3.y, 2.0f * y, 2.0f * x, 0.0f)
+        NEP_AB(4)
+        NEP_USE(8, 3, A2_4.x, B2_4.x, -6.0f * xz, -6.0f * yz, -3.0f * (x2 + y2 - 2.0f * z2))
+        NEP_USE(9, 3, A2_4.y, B2_4.y, -3.0f * x2 - y2 + 4.0f * z2, -2.0f * xy, 8.0f * xz)
+        NEP_AB(5)
+        NEP_USE(10, 3, A2_5.x, B2_5.x, -2.0f * xy, -x2 - 3.0f * y2 + 4.0f * z2, 8.0f * yz)
+        NEP_USE(11, 3, A2_5.y, B2_5.y, 2.0f * xz, -2.0f * yz, x2 - y2)
+        NEP_AB(6)
+        NEP_USE(12, 3, A2_6.x, B2_6.x, 2.0f * yz, 2.0f * xz, 2.0f * xy)
+        NEP_USE(13, 3, A2_6.y, B2_6.y, 3.0f * (x2 - y2), -6.0f * xy, 0.0f)
+        NEP_AB(7)
+        NEP_USE(14, 3, A2_7.x, B2_7.x, 6.0f * xy, 3.0f * (x2 - y2), 0.0f)
+        NEP_USE(15, 4, A2_7.y, B2_7.y, 12.0f * x * (x2 + y2 - 4.0f * z2), 12.0f * y * (x2 + y2 - 4.0f * z2), -16.0f * z * (3.0f * x2 + 3.0f * y2 - 2.0f * z2))
+        NEP_AB(8)
+        NEP_USE(16, 4, A2_8.x, B2_8.x, -z * (9.0f * x2 + 3.0f * y2 - 4.0f * z2), -6.0f * xyz, -3.0f * x * (x2 + y2 - 4.0f * z2))
+        NEP_USE(17, 4, A2_8.y, B2_8.y, -6.0f * xyz, -z * (3.0f * x2 + 9.0f * y2 - 4.0f * z2), -3.0f * y * (x2 + y2 - 4.0f * z2))
+        NEP_AB(9)
+        NEP_USE(18, 4, A2_9.x, B2_9.x, -4.0f * x * (x2 - 3.0f * z2), 4.0f * y * (y2 - 3.0f * z2), 12.0f * z * (x2 - y2))
+        NEP_USE(19, 4, A2_9.y, B2_9.y, -2.0f * y * (3.0f * x2 + y2 - 6.0f * z2), -2.0f * x * (x2 + 3.0f * y2 - 6.0f * z2), 24.0f * xyz)
+        NEP_AB(10)
+        NEP_USE(20, 4, A2_10.x, B2_10.x, 3.0f * z * (x2 - y2), -6.0f * xyz, x * (x2 - 3.0f * y2))
+        NEP_USE(21, 4, A2_10.y, B2_10.y, 6.0f * xyz, 3.0f * z * (x2 - y2), y * (3.0f * x2 - y2))
+        NEP_AB(11)
+        NEP_USE(22, 4, A2_11.x, B2_11.x, 4.0f * x * (x2 - 3.0f * y2), -4.0f * y * (3.0f * x2 - y2), 0.0f)
+        NEP_USE(23, 4, A2_11.y, B2_11.y, 4.0f * y * (3.0f * x2 - y2), 4.0f * x * (x2 - 3.0f * y2), 0.0f)
+#undef NEP_AB
+#undef NEP_AB_STEP
+#undef NEP_USE
         float4 out = make_float4(fmaf(cu, x, rinv * vx), fmaf(cu, y, rinv * vy), fmaf(cu, z, rinv * vz), 0.0f);
         sx += out.x; sy += out.y; sz += out.z;
         // delivered to the receiver: row (slot of i in j's column) of atom j -- a fire-and-forget store
