@@ -25,6 +25,12 @@
  * scipy's cKDTree and a 125-lattice-image search, orthorhombic and sheared.  Parity of E/F/W against any trained-model number of the paper: UNPINNED
  * (the paper's models and datasets are not available) -- see DESIGN.md.
  *
+ * Cells of any size (onep_compute_images, reading A18; the small cells of a training batch, Eq. (33),
+ * PAPER.md:267-283): neighbours are all lattice images within the cutoffs.  Pins (tests/test_oracle_derived.py): equals
+ * the pinned minimum-image path on a supercell of the same crystal, atom by atom (orthorhombic, sheared, and 4-atom
+ * cells where atoms see their own images); entry counts vs a numpy lattice-image search; F = -dE/dr and
+ * sum W = -dE/d(eps) by central differences in a cell with self-images.
+ *
  * Compile: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC nep_oracle.c -o libnep_oracle.so -lm
  * (-ffp-contract=off so that the neighbour predicate is the literal IEEE expression of reading A8).
  */
@@ -396,10 +402,107 @@ static pair_t* build_pairs(int64_t n, const double* pos, const double box[9], co
     return pairs;
 }
 
+/* Cells of any size (reading A18): the sums of Eqs. (2) and (12) run over ALL atoms of the periodic
+ * structure within r_c, i.e. over every lattice image (j, N) with |r_j + N_a a + N_b b + N_c c - r_i| < r_c,
+ * (j, N) != (i, 0) -- in a cell thinner than 2 r_c several images of the same j (and images of i itself) count.
+ * Plain loop over image shifts: t = r_j - r_i; N0_k = rint((t Hinv)_k); for m in [-M_k, M_k]^3: N = N0 + m,
+ * d = ((t - N_a a) - N_b b) - N_c c; neighbour iff (dx dx + dy dy) + dz dz < rc rc (strict), with
+ * M_k = floor(rc / width_k + 1/2) + 1 and width_k the distance between the cell faces k.                     */
+static pair_t* build_pairs_images(int64_t n, const double* pos, const double box[9], double rc, int64_t** first_out)
+{
+    double inv[9];
+    inverse3(box, inv);
+    int M[3];
+    for (int k = 0; k < 3; ++k) {
+        const double w = 1.0 / sqrt(inv[k] * inv[k] + inv[3 + k] * inv[3 + k] + inv[6 + k] * inv[6 + k]);
+        M[k] = (int)floor(rc / w + 0.5) + 1;
+    }
+    int64_t* first = (int64_t*)malloc(sizeof(int64_t) * (size_t)(n + 1));
+    if (!first) return NULL;
+    const double rc2 = rc * rc;
+    pair_t* pairs = NULL;
+    for (int pass = 0; pass < 2; ++pass) {              /* count, then fill */
+        int64_t p = 0;
+        for (int64_t i = 0; i < n; ++i) {
+            if (pass == 0) first[i] = p;
+            for (int64_t j = 0; j < n; ++j) {
+                double t[3], n0[3];
+                for (int a = 0; a < 3; ++a) t[a] = pos[3 * j + a] - pos[3 * i + a];
+                for (int k = 0; k < 3; ++k) n0[k] = rint((t[0] * inv[k] + t[1] * inv[3 + k]) + t[2] * inv[6 + k]);
+                for (int ma = -M[0]; ma <= M[0]; ++ma)
+                    for (int mb = -M[1]; mb <= M[1]; ++mb)
+                        for (int mc = -M[2]; mc <= M[2]; ++mc) {
+                            const double N[3] = {n0[0] + ma, n0[1] + mb, n0[2] + mc};
+                            if (j == i && N[0] == 0.0 && N[1] == 0.0 && N[2] == 0.0) continue;
+                            double d[3];
+                            for (int a = 0; a < 3; ++a) d[a] = ((t[a] - N[0] * box[a]) - N[1] * box[3 + a]) - N[2] * box[6 + a];
+                            const double d2 = dist2(d);
+                            if (d2 < rc2) {
+                                if (pass == 1) {
+                                    pairs[p].j = (int32_t)j;
+                                    pairs[p].d[0] = d[0]; pairs[p].d[1] = d[1]; pairs[p].d[2] = d[2];
+                                    pairs[p].r = sqrt(d2);
+                                }
+                                ++p;
+                            }
+                        }
+            }
+        }
+        if (pass == 0) {
+            first[n] = p;
+            pairs = (pair_t*)malloc(sizeof(pair_t) * (size_t)(p > 0 ? p : 1));
+            if (!pairs) { free(first); return NULL; }
+        }
+    }
+    *first_out = first;
+    return pairs;
+}
+
+static int compute_impl(const onep_hyper* h,
+                 const double* c_radial, const double* c_angular,
+                 const double* w0, const double* b0, const double* w1, const double* b1,
+                 int64_t n, const double* pos, const int32_t* type, const double box[9], const int32_t pbc[3], int images,
+                 double* energy, double* force, double* virial,
+                 double* q_out, double* fp_out, double* S_out);
+
 int onep_compute(const onep_hyper* h,
                  const double* c_radial, const double* c_angular,
                  const double* w0, const double* b0, const double* w1, const double* b1,
                  int64_t n, const double* pos, const int32_t* type, const double box[9], const int32_t pbc[3],
+                 double* energy, double* force, double* virial,
+                 double* q_out, double* fp_out, double* S_out)
+{
+    return compute_impl(h, c_radial, c_angular, w0, b0, w1, b1, n, pos, type, box, pbc, 0, energy, force, virial, q_out, fp_out, S_out);
+}
+
+/* the same for a fully periodic cell of ANY size: neighbours are all lattice images within the cutoffs
+ * (build_pairs_images; reading A18).  Everything after the pair lists is the code of onep_compute.        */
+int onep_compute_images(const onep_hyper* h,
+                 const double* c_radial, const double* c_angular,
+                 const double* w0, const double* b0, const double* w1, const double* b1,
+                 int64_t n, const double* pos, const int32_t* type, const double box[9],
+                 double* energy, double* force, double* virial,
+                 double* q_out, double* fp_out, double* S_out)
+{
+    const int32_t pbc[3] = {1, 1, 1};
+    return compute_impl(h, c_radial, c_angular, w0, b0, w1, b1, n, pos, type, box, pbc, 1, energy, force, virial, q_out, fp_out, S_out);
+}
+
+/* number of ordered neighbour entries (j, N) within rc of each atom, lattice images counted (test hook)  */
+int onep_count_images(int64_t n, const double* pos, const double box[9], double rc, int32_t* count)
+{
+    int64_t* first = NULL;
+    pair_t* P = build_pairs_images(n, pos, box, rc, &first);
+    if (!P) return -1;
+    for (int64_t i = 0; i < n; ++i) count[i] = (int32_t)(first[i + 1] - first[i]);
+    free(P); free(first);
+    return 0;
+}
+
+static int compute_impl(const onep_hyper* h,
+                 const double* c_radial, const double* c_angular,
+                 const double* w0, const double* b0, const double* w1, const double* b1,
+                 int64_t n, const double* pos, const int32_t* type, const double box[9], const int32_t pbc[3], int images,
                  double* energy, double* force, double* virial,
                  double* q_out, double* fp_out, double* S_out)
 {
@@ -415,8 +518,8 @@ int onep_compute(const onep_hyper* h,
     if (has5 && nk_used < 3) nk_used = 3;
 
     int64_t *firstR = NULL, *firstA = NULL;
-    pair_t* PR = build_pairs(n, pos, box, pbc, h->rc_radial, &firstR);
-    pair_t* PA = build_pairs(n, pos, box, pbc, h->rc_angular, &firstA);
+    pair_t* PR = images ? build_pairs_images(n, pos, box, h->rc_radial, &firstR) : build_pairs(n, pos, box, pbc, h->rc_radial, &firstR);
+    pair_t* PA = images ? build_pairs_images(n, pos, box, h->rc_angular, &firstA) : build_pairs(n, pos, box, pbc, h->rc_angular, &firstA);
     double* q = (double*)calloc((size_t)(n * D + 1), sizeof(double));
     double* fp = (double*)calloc((size_t)(n * D + 1), sizeof(double));
     double* S = (double*)calloc((size_t)(n * NA * NUM_B + 1), sizeof(double));

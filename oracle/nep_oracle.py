@@ -76,6 +76,11 @@ def lib():
         L.onep_compute.restype = C.c_int
         L.onep_compute.argtypes = [C.POINTER(OracleHyper), _dp, _dp, _dp, _dp, _dp, _dp,
                                    C.c_int64, _dp, _ip, _dp, _ip, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.onep_compute_images.restype = C.c_int
+        L.onep_compute_images.argtypes = [C.POINTER(OracleHyper), _dp, _dp, _dp, _dp, _dp, _dp,
+                                          C.c_int64, _dp, _ip, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.onep_count_images.restype = C.c_int
+        L.onep_count_images.argtypes = [C.c_int64, _dp, _dp, C.c_double, _ip]
         L.onep_md.restype = C.c_int
         L.onep_md.argtypes = [C.POINTER(OracleHyper), _dp, _dp, _dp, _dp, _dp, _dp,
                               C.c_int64, _dp, _dp, _ip, _dp, _dp, _ip, C.c_double, C.c_int32, _dp, _dp]
@@ -210,6 +215,37 @@ def compute(hyper, params, pos, types, box, pbc=(1, 1, 1), want_internals: bool 
     if rc != 0:
         raise MemoryError("oracle allocation failed")
     return (e, f, w, q, fp, S) if want_internals else (e, f, w)
+
+
+def compute_images(hyper, params, pos, types, box, want_internals: bool = False):
+    """compute() for a fully periodic cell of ANY size (reading A18): the neighbours of an atom are all
+    lattice images (j, N) within the cutoffs, (j, N) != (i, 0) -- what Eqs. (2), (12) mean for the small cells of a
+    training set.  Same outputs as compute()."""
+    h = OracleHyper.from_hyper(hyper)
+    pos, box = _d(pos), _box9(box)
+    types = np.ascontiguousarray(types, dtype=np.int32)
+    n = pos.shape[0]
+    cr, ca, w0, b0, w1, b1 = map(_d, (params.c_radial, params.c_angular, params.w0, params.b0, params.w1, params.b1))
+    D = int(lib().onep_num_descriptors(C.byref(h)))
+    NA = hyper.n_max_angular + 1
+    e, f, w = np.zeros(n), np.zeros((n, 3)), np.zeros((n, 9))
+    q = np.zeros((n, D)) if want_internals else None
+    fp = np.zeros((n, D)) if want_internals else None
+    S = np.zeros((n, NA, 24)) if want_internals else None
+    rc = lib().onep_compute_images(C.byref(h), _p(cr), _p(ca), _p(w0), _p(b0), _p(w1), _p(b1),
+                                   n, _p(pos), _p(types, _ip), _p(box), _p(e), _p(f), _p(w), _p(q), _p(fp), _p(S))
+    if rc != 0:
+        raise MemoryError("oracle allocation failed")
+    return (e, f, w, q, fp, S) if want_internals else (e, f, w)
+
+
+def count_images(pos, box, rc: float):
+    """Ordered neighbour entries (j, N) within rc of each atom, lattice images counted separately."""
+    pos, box = _d(pos), _box9(box)
+    cnt = np.zeros(pos.shape[0], dtype=np.int32)
+    if lib().onep_count_images(pos.shape[0], _p(pos), _p(box), rc, _p(cnt, _ip)) != 0:
+        raise MemoryError("oracle allocation failed")
+    return cnt
 
 
 def md(hyper, params, pos, vel, types, masses, box, dt_fs: float, n_steps: int, pbc=(1, 1, 1)):
@@ -363,6 +399,30 @@ def loss_terms(energy, force, virial, u_target: float, f_target, w_target6):
     six = np.array([wtot[0], wtot[4], wtot[8], wtot[1], wtot[5], wtot[6]])
     lv = float(np.sqrt(((six - wt) ** 2).sum() / 6.0))
     return float(le), lf, lv
+
+
+def loss_terms_batch(energies, forces, virials, u_targets, f_targets, w_targets6):
+    """The three RMSE terms of Eq. (33) for a batch of N_str structures; per structure s with
+    N_s atoms: energies[s][N_s], forces[s][N_s][3], virials[s][N_s][9] (W[3a+b]), targets u_targets[s] (eV/atom),
+    f_targets[s][N_s][3], w_targets6[s][6] (eV/atom; xx, yy, zz, xy, yz, zx).  With N = sum_s N_s:
+      L_e = sqrt( 1/N_str sum_s (sum_i U_i / N_s - u_tar(s))^2 )
+      L_f = sqrt( 1/(3N) sum_s sum_i |F_i - F_i^tar|^2 )
+      L_v = sqrt( 1/(6 N_str) sum_s sum_{mu nu} (sum_i W_i^{mu nu} / N_s - w_tar(s)[mu nu])^2 )
+    (U^NEP(n, z) and W^NEP(n, z) are per-atom energy and virial of structure n.)"""
+    n_str = len(energies)
+    se, sf, sv, n_tot = 0.0, 0.0, 0.0, 0
+    for s in range(n_str):
+        e, f, w = _d(energies[s]), _d(forces[s]), _d(virials[s])
+        ns = len(e)
+        n_tot += ns
+        se += (e.sum() / ns - float(u_targets[s])) ** 2
+        df = f - _d(f_targets[s])
+        sf += float((df * df).sum())
+        wt = w.sum(axis=0) / ns
+        six = np.array([wt[0], wt[4], wt[8], wt[1], wt[5], wt[6]])
+        dv = six - _d(w_targets6[s])
+        sv += float((dv * dv).sum())
+    return float(np.sqrt(se / n_str)), float(np.sqrt(sf / (3.0 * n_tot))), float(np.sqrt(sv / (6.0 * n_str)))
 
 
 def regularisation_terms(params):

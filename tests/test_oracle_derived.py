@@ -314,3 +314,106 @@ def test_loss_terms_hand_case_and_zero(oracle_mod):
     flip = types.SimpleNamespace(**{k: -3.0 * v for k, v in vars(hand).items()})
     l1f, l2f = oracle_mod.regularisation_terms(flip)
     assert l1f == pytest.approx(10.285714285714286, rel=1e-15) and l2f == pytest.approx(15.793307805161383, rel=1e-15)
+
+
+# ------------------------------------------------------------------ cells of any size: lattice images (reading A18)
+def _image_counts(pos, H, rc, reach=3):
+    """the plain definition in numpy: ordered entries (j, N) != (i, 0) with |r_j + N H - r_i| < rc"""
+    shifts = np.array([[a, b, c] for a in range(-reach, reach + 1) for b in range(-reach, reach + 1)
+                       for c in range(-reach, reach + 1)], dtype=np.float64)
+    sv = shifts @ H
+    zero = int(np.flatnonzero((shifts == 0).all(axis=1))[0])
+    out = np.zeros(len(pos), dtype=np.int64)
+    for i in range(len(pos)):
+        d = pos[None, :, :] - pos[i][None, None, :] + sv[:, None, :]
+        close = (d * d).sum(axis=2) < rc * rc
+        close[zero, i] = False
+        out[i] = close.sum()
+    return out
+
+
+def _small_and_super(idx, cells, reps, tilt=None, kind="stress"):
+    """a small periodic cell and the (rx, ry, rz) supercell of the SAME infinite structure"""
+    cfg = W.get_config(idx, cells)
+    s, p = W.make_system(cfg), W.make_params(cfg, kind)
+    pos, H = (s.pos, np.diag(s.box)) if tilt is None else W.sheared(s, *tilt)
+    rx, ry, rz = reps
+    offs = np.array([[a, b, c] for a in range(rx) for b in range(ry) for c in range(rz)], dtype=np.float64) @ H
+    big = (pos[None, :, :] + offs[:, None, :]).reshape(-1, 3)
+    Hbig = H * np.array([[rx], [ry], [rz]], dtype=np.float64)
+    return cfg, p, pos, s.types, H, big, np.tile(s.types, len(offs)), Hbig, len(offs)
+
+
+@pytest.mark.parametrize("idx,cells,reps,tilt", [
+    (3, (2, 2, 2), (2, 2, 2), None),                   # fcc alloy, 32 atoms, 7.2 A cell: rc_R = 5 > L/2
+    (3, (1, 1, 1), (4, 3, 3), None),                   # 4 atoms in a 3.6 A cell: every atom sees images of itself
+    (2, (1, 1, 2), (2, 2, 1), None),                   # rock salt, rc_R = 6, 6.46 x 6.46 x 12.92 A
+    (3, (2, 2, 1), (2, 2, 4), (0.21, -0.13, 0.17)),    # sheared small cell
+])
+def test_image_sum_equals_the_supercell(oracle_mod, idx, cells, reps, tilt):
+    """A cell thinner than 2 r_c evaluated with lattice images == the same crystal described by a supercell that
+    the pinned minimum-image path can handle: every atom's U_i, F_i, W_i and q, Fp, S equal those of its copies."""
+    cfg, p, pos, types, H, big, tbig, Hbig, ncopy = _small_and_super(idx, cells, reps, tilt)
+    hy = cfg.hyper
+    assert W.perpendicular_widths(H).min() < 2 * hy.rc_radial <= W.perpendicular_widths(Hbig).min()
+    e, f, w, q, fp, S = oracle_mod.compute_images(hy, p, pos, types, H, want_internals=True)
+    eb, fb, wb, qb, fpb, Sb = oracle_mod.compute(hy, p, big, tbig, Hbig, want_internals=True)
+    n = len(pos)
+    for c in range(ncopy):
+        sl = slice(c * n, (c + 1) * n)
+        np.testing.assert_allclose(eb[sl], e, rtol=1e-12, atol=1e-13)
+        np.testing.assert_allclose(fb[sl], f, rtol=1e-10, atol=1e-12)
+        np.testing.assert_allclose(wb[sl], w, rtol=1e-10, atol=1e-12)
+        np.testing.assert_allclose(qb[sl], q, rtol=1e-12, atol=1e-14)
+        np.testing.assert_allclose(Sb[sl], S, rtol=1e-11, atol=1e-13)
+    assert np.abs(f).max() > 1e-3 and np.abs(w).max() > 1e-3
+    # neighbour entries, images counted: the numpy definition
+    for rc in (hy.rc_radial, hy.rc_angular):
+        assert np.array_equal(oracle_mod.count_images(pos, H, rc), _image_counts(pos, H, rc))
+    # a cell wide enough for the minimum image: both paths are the same function
+    e2, f2, w2 = oracle_mod.compute_images(hy, p, big, tbig, Hbig)
+    np.testing.assert_allclose(e2, eb, rtol=1e-13, atol=1e-14)
+    np.testing.assert_allclose(f2, fb, rtol=1e-11, atol=1e-13)
+    np.testing.assert_allclose(w2, wb, rtol=1e-11, atol=1e-13)
+
+
+def test_image_sum_forces_and_virial_by_finite_differences(oracle_mod):
+    """F = -dE/dr (moving an atom moves all its images) and sum_i W_i = -dE/d(strain) in a cell with self-images."""
+    cfg = W.get_config(3, (1, 1, 2))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    pos, H = W.sheared(s, 0.12, -0.07, 0.05)
+    hy = cfg.hyper
+    etot = lambda x, h: oracle_mod.compute_images(hy, p, x, s.types, h)[0].sum()
+    e, f, w = oracle_mod.compute_images(hy, p, pos, s.types, H)
+    hstep = 1e-5
+    for i, a in ((0, 0), (3, 1), (5, 2)):
+        xp, xm = pos.copy(), pos.copy()
+        xp[i, a] += hstep; xm[i, a] -= hstep
+        assert f[i, a] == pytest.approx(-(etot(xp, H) - etot(xm, H)) / (2 * hstep), rel=2e-6, abs=1e-8)
+    assert np.abs(f.sum(axis=0)).max() < 1e-10
+    wsum = w.sum(axis=0).reshape(3, 3)
+    for a, b in ((0, 0), (1, 1), (2, 2), (0, 1), (1, 2), (2, 0)):
+        eps = np.zeros((3, 3)); eps[a, b] = hstep
+        Fp_, Fm_ = np.eye(3) + eps, np.eye(3) - eps          # r -> r F (row vectors): r^b picks up eps * r^a
+        de = (etot(pos @ Fp_, H @ Fp_) - etot(pos @ Fm_, H @ Fm_)) / (2 * hstep)
+        assert wsum[a, b] == pytest.approx(-de, rel=2e-6, abs=1e-8)
+
+
+def test_loss_terms_batch_hand_case(oracle_mod):
+    """Eq. (33) with N_str = 2, numbers worked by hand."""
+    e = [np.array([1.0, 3.0]), np.array([2.0, 2.0, 5.0])]                 # per-atom energies 2 and 3
+    f = [np.array([[1.0, 0.0, 0.0], [0.0, 2.0, 0.0]]), np.array([[0.0, 0.0, 2.0], [0.0, 0.0, 0.0], [1.0, 1.0, 0.0]])]
+    w = [np.zeros((2, 9)), np.zeros((3, 9))]
+    w[0][0, 0] = 2.0; w[0][1, 0] = 4.0; w[0][0, 1] = 1.0            # structure 0 per atom: xx 3, xy 0.5
+    w[1][0, 4] = 3.0; w[1][2, 5] = -6.0; w[1][1, 6] = 9.0           # structure 1 per atom: yy 1, yz -2, zx 3
+    ft = [np.zeros((2, 3)), np.zeros((3, 3))]
+    le, lf, lv = oracle_mod.loss_terms_batch(e, f, w, [1.5, 3.5], ft, [np.zeros(6), np.zeros(6)])
+    assert le == pytest.approx(np.sqrt((0.25 + 0.25) / 2))                      # (2 - 1.5)^2, (3 - 3.5)^2
+    assert lf == pytest.approx(np.sqrt((1 + 4 + 4 + 1 + 1) / (3 * 5)))          # N = 5 atoms
+    assert lv == pytest.approx(np.sqrt((9 + 0.25 + 1 + 4 + 9) / (6 * 2)))
+    # one structure: the N_str = 1 function (pinned above)
+    one = oracle_mod.loss_terms(e[1], f[1], w[1], 3.5, ft[1], np.zeros(6))
+    assert oracle_mod.loss_terms_batch(e[1:], f[1:], w[1:], [3.5], ft[1:], [np.zeros(6)]) == pytest.approx(one)
+    # exact targets: zero
+    tw = [np.array([3.0, 0, 0, 0.5, 0, 0]), np.array([0, 1.0, 0, 0, -2.0, 3.0])]
+    assert oracle_mod.loss_terms_batch(e, f, w, [2.0, 3.0], f, tw) == (0.0, 0.0, 0.0)
