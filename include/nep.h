@@ -222,6 +222,38 @@ int nep_compute_population(nep_t* nep, const double* pos_dev, int32_t n_pop,
 int nep_loss_terms(nep_t* nep, double u_target_per_atom, const double* f_target_dev,
                    const double w_target_per_atom[6], double terms_host[3]);
 
+/* ---- batched evaluation for training: many small structures x a population of parameter sets ------------------
+ * (SURVEY.md section 8(f) row 4.)  SNES evaluates every member of a population on every structure of a (mini-)batch
+ * and reduces the loss of Eq. (33).  Independent of nep_neighbors()/md_step(): the batch has its
+ * own storage in the handle.
+ * nep_batch_neighbors: n_str structures concatenated; structure s owns atoms atom_offset_host[s] .. [s+1]-1 (HOST,
+ *   [n_str+1], starting at 0, at least one atom each); pos_dev [N][3] fp64 and type_dev [N] int32 (DEVICE), N =
+ *   atom_offset_host[n_str]; boxes_host [n_str][9] (HOST): lattice vectors a, b, c of each cell as rows, det > 0.
+ *   The cells may be of ANY size > rc_radial / 6.5 per perpendicular width (NEP_ERR_BOX_TOO_SMALL below that):
+ *   the neighbours of atom i are all lattice images (j, N) != (i, 0) of the atoms of its own structure with
+ *   |r_j + N_a a + N_b b + N_c c - r_i| < rc_radial (angular: < rc_angular), evaluated in fp64 (DESIGN.md reading
+ *   A18); positions need not be wrapped.  Synchronises (sizes the storage from the longest list).
+ * nep_batch_compute: evaluates n_pop parameter sets (HOST arrays stacked member-major, layouts of nep_create as in
+ *   nep_compute_population) on every structure of the batch in one launch sequence over atoms x members; the
+ *   parameters are copied to the device once, there is no per-member synchronisation.  energy_dev [n_pop][N]
+ *   (required), force_dev [n_pop][N][3], virial_dev [n_pop][N][9] (either may be NULL), fp64, batch atom order.
+ *   Does not touch the handle's own model.  Synchronises before returning (the host arrays may then be reused).
+ * nep_batch_loss: the three data terms of Eq. (33) for every member, from the outputs of nep_batch_compute and the
+ *   targets u_target_dev [n_str] (eV/atom), f_target_dev [N][3] (eV/Angstrom), w_target_dev [n_str][6] (eV/atom;
+ *   xx, yy, zz, xy, yz, zx of W[3a+b]):  loss_dev [n_pop][3] = { sqrt(1/n_str sum_s (sum_i U_i/N_s - u_tar_s)^2),
+ *   sqrt(1/(3N) sum_i |F_i - F_i^tar|^2), sqrt(1/(6 n_str) sum_s sum_{mu nu} (sum_i W_i/N_s - w_tar_s)^2) },
+ *   reduced on the device per (member, structure) and then per member in a fixed order (bitwise reproducible).
+ *   The weights lambda and the regularisation terms of Eq. (33) are the caller's.  Does not synchronise.
+ * NEP_ERR_STATE before nep_batch_neighbors.                                                                      */
+int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_host, const double* pos_dev,
+                        const int32_t* type_dev, const double* boxes_host);
+int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const float* c_angular,
+                      const float* w0, const float* b0, const float* w1, const float* b1,
+                      double* energy_dev, double* force_dev, double* virial_dev);
+int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const double* force_dev,
+                   const double* virial_dev, const double* u_target_dev, const double* f_target_dev,
+                   const double* w_target_dev, double* loss_dev);
+
 /* ---- heat current, Eqs. (25)-(26) ------------------------------------------------
  * J_i = W_i . v_i with the per-atom virial W_i of the last evaluation (Eq. (24), layout W[3a+b]):
  * j_atom_dev [n][3] gets J_i^a = sum_b W_i^{ab} v_i^b, j_total_dev [3] gets J = sum_i J_i (reduced in a

@@ -21,7 +21,7 @@ exported_symbols = (
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
     "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
-    "nep_compute_population", "nep_loss_terms",
+    "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
@@ -104,6 +104,12 @@ def load_library():
     L.nep_compute_population.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.nep_loss_terms.restype = C.c_int
     L.nep_loss_terms.argtypes = [vp, dbl, vp, dp, dp]
+    L.nep_batch_neighbors.restype = C.c_int
+    L.nep_batch_neighbors.argtypes = [vp, i32, ip, vp, vp, dp]
+    L.nep_batch_compute.restype = C.c_int
+    L.nep_batch_compute.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.nep_batch_loss.restype = C.c_int
+    L.nep_batch_loss.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     L.nep_get_latent.restype = C.c_int
     L.nep_get_latent.argtypes = [vp, vp]
     L.nep_heat_current.restype = C.c_int
@@ -325,6 +331,43 @@ class NEP:
         out = (C.c_double * 3)()
         self._check(self._L.nep_loss_terms(self._h_ptr, float(u_target), self._dev(f_target, torch.float64, 3 * self.n), wt, out))
         return out[0], out[1], out[2]
+
+    # ---- batched evaluation for training (include/nep.h "batched evaluation")
+    def nep_batch_neighbors(self, atom_offset, pos, types, boxes):
+        """atom_offset: [n_str+1] ints (host); pos [N][3] f64 / types [N] i32 CUDA tensors; boxes [n_str][9] or [n_str][3][3] (host)."""
+        torch = self._torch
+        off = np.ascontiguousarray(atom_offset, dtype=np.int32)
+        n_str, N = len(off) - 1, int(off[-1])
+        bx = np.ascontiguousarray(np.asarray(boxes, dtype=np.float64).reshape(n_str, 9))
+        self._check(self._L.nep_batch_neighbors(self._h_ptr, n_str, off.ctypes.data_as(C.POINTER(C.c_int32)),
+                                                self._dev(pos, torch.float64, 3 * N), self._dev(types, torch.int32, N),
+                                                bx.ctypes.data_as(C.POINTER(C.c_double))))
+        self.batch_n, self.batch_n_str = N, n_str
+
+    def nep_batch_compute(self, members, want_forces: bool = True):
+        """E [n_pop][N], F [n_pop][N][3], W [n_pop][N][9] of a list of parameter sets on the whole batch."""
+        torch = self._torch
+        N, dev, P = self.batch_n, f"cuda:{self.device}", len(members)
+        stack = [np.ascontiguousarray(np.stack([_f32(getattr(m, k)).reshape(-1) for m in members]))
+                 for k in ("c_radial", "c_angular", "w0", "b0", "w1", "b1")]
+        e = torch.empty((P, N), dtype=torch.float64, device=dev)
+        f = torch.empty((P, N, 3), dtype=torch.float64, device=dev) if want_forces else None
+        w = torch.empty((P, N, 9), dtype=torch.float64, device=dev) if want_forces else None
+        self._check(self._L.nep_batch_compute(self._h_ptr, P, *[C.c_void_p(a.ctypes.data) for a in stack],
+                                              C.c_void_p(e.data_ptr()), C.c_void_p(f.data_ptr()) if want_forces else None,
+                                              C.c_void_p(w.data_ptr()) if want_forces else None))
+        return e, f, w
+
+    def nep_batch_loss(self, e, f, w, u_target, f_target, w_target6):
+        """[n_pop][3] = (L_e, L_f, L_v) of Eq. (33) per member; targets are CUDA f64 tensors [n_str], [N][3], [n_str][6]."""
+        torch = self._torch
+        P, N, S = e.shape[0], self.batch_n, self.batch_n_str
+        out = torch.empty((P, 3), dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._L.nep_batch_loss(self._h_ptr, P, self._dev(e, torch.float64, P * N), self._dev(f, torch.float64, 3 * P * N),
+                                           self._dev(w, torch.float64, 9 * P * N), self._dev(u_target, torch.float64, S),
+                                           self._dev(f_target, torch.float64, 3 * N), self._dev(w_target6, torch.float64, 6 * S),
+                                           C.c_void_p(out.data_ptr())))
+        return out
 
     def nep_get_latent(self):
         """[n][H] latent-space vectors of the last evaluation."""

@@ -9,6 +9,7 @@
 #include "nep_common.cuh"
 #include "nep_neighbor.cuh"
 #include "nep_kernels.cuh"
+#include "nep_batch.cuh"
 #include "nep_probe.cuh"
 
 namespace {
@@ -1140,6 +1141,162 @@ int nep_heat_current(nep_t* nep, const double* vel_dev, double* j_atom_dev, doub
     return NEP_OK;
 }
 
+// ---- batched evaluation for training (nep_batch.cuh) --------------------------
+int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_host, const double* pos_dev,
+                        const int32_t* type_dev, const double* boxes_host)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (n_str < 1 || !atom_offset_host || !pos_dev || !type_dev || !boxes_host) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n_str < 1");
+    if (atom_offset_host[0] != 0) return nep_fail(nep, NEP_ERR_INVALID_ARG, "atom_offset[0] must be 0");
+    for (int s = 0; s < n_str; ++s)
+        if (atom_offset_host[s + 1] <= atom_offset_host[s]) return nep_fail(nep, NEP_ERR_INVALID_ARG, "every structure needs at least one atom");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const int N = atom_offset_host[n_str];
+    std::vector<double> H(9 * (size_t)n_str), Hinv(9 * (size_t)n_str);
+    std::vector<int> M(3 * (size_t)n_str), sid((size_t)N);
+    for (int s = 0; s < n_str; ++s) {
+        const double* h = boxes_host + 9 * (size_t)s;
+        for (int a = 0; a < 9; ++a)
+            if (!(h[a] == h[a]) || fabs(h[a]) > 1e12) return nep_fail(nep, NEP_ERR_INVALID_ARG, "bad box");
+        const double c00 = h[4] * h[8] - h[5] * h[7], c01 = h[5] * h[6] - h[3] * h[8], c02 = h[3] * h[7] - h[4] * h[6];
+        const double det = (h[0] * c00 + h[1] * c01) + h[2] * c02;
+        if (!(det > 0.0)) return nep_fail(nep, NEP_ERR_UNSUPPORTED_BOX, "the cell vectors a, b, c must form a right-handed, non-degenerate cell");
+        double* inv = Hinv.data() + 9 * (size_t)s;
+        inv[0] = c00 / det; inv[1] = (h[2] * h[7] - h[1] * h[8]) / det; inv[2] = (h[1] * h[5] - h[2] * h[4]) / det;
+        inv[3] = c01 / det; inv[4] = (h[0] * h[8] - h[2] * h[6]) / det; inv[5] = (h[2] * h[3] - h[0] * h[5]) / det;
+        inv[6] = c02 / det; inv[7] = (h[1] * h[6] - h[0] * h[7]) / det; inv[8] = (h[0] * h[4] - h[1] * h[3]) / det;
+        for (int k = 0; k < 3; ++k) {
+            const double width = 1.0 / sqrt(inv[k] * inv[k] + inv[3 + k] * inv[3 + k] + inv[6 + k] * inv[6 + k]);
+            const int m = (int)floor(nep->h.rc_radial / width + 0.5) + 1;       // reading A18
+            if (m > NEP_BATCH_MAX_SHIFT) return nep_fail(nep, NEP_ERR_BOX_TOO_SMALL, "a cell of the batch is thinner than rc_radial / 6.5");
+            M[3 * (size_t)s + k] = m;
+        }
+        for (int a = 0; a < 9; ++a) H[9 * (size_t)s + a] = h[a];
+        for (int i = atom_offset_host[s]; i < atom_offset_host[s + 1]; ++i) sid[(size_t)i] = s;
+    }
+    auto& b = nep->b;
+    b.n_str = 0;                                          // invalid until everything below succeeds
+    NEP_TRY(dev_alloc(nep, &b.off, (size_t)n_str + 1));
+    NEP_TRY(dev_alloc(nep, &b.sid, (size_t)N));
+    NEP_TRY(dev_alloc(nep, &b.M, 3 * (size_t)n_str));
+    NEP_TRY(dev_alloc(nep, &b.H, 9 * (size_t)n_str));
+    NEP_TRY(dev_alloc(nep, &b.Hinv, 9 * (size_t)n_str));
+    NEP_TRY(dev_alloc(nep, &b.type, (size_t)N));
+    NEP_TRY(dev_alloc(nep, &b.cnt, (size_t)N));
+    if (!b.bad) NEP_TRY(dev_alloc(nep, &b.bad, 1));
+    cudaStream_t st = nep->stream;
+    NEP_CUDA(cudaMemcpyAsync(b.off, atom_offset_host, sizeof(int) * ((size_t)n_str + 1), cudaMemcpyHostToDevice, st));
+    NEP_CUDA(cudaMemcpyAsync(b.sid, sid.data(), sizeof(int) * (size_t)N, cudaMemcpyHostToDevice, st));
+    NEP_CUDA(cudaMemcpyAsync(b.M, M.data(), sizeof(int) * M.size(), cudaMemcpyHostToDevice, st));
+    NEP_CUDA(cudaMemcpyAsync(b.H, H.data(), sizeof(double) * H.size(), cudaMemcpyHostToDevice, st));
+    NEP_CUDA(cudaMemcpyAsync(b.Hinv, Hinv.data(), sizeof(double) * Hinv.size(), cudaMemcpyHostToDevice, st));
+    NEP_CUDA(cudaMemcpyAsync(b.type, type_dev, sizeof(int) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    NEP_CUDA(cudaMemsetAsync(b.bad, 0, sizeof(int), st));
+    // count, size the storage from the longest list, fill, reverse slots
+    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, 0, 0,
+                                                                          b.cnt, nullptr, nullptr, nullptr, b.bad));
+    std::vector<int> cnt((size_t)N);
+    int bad = 0;
+    NEP_CUDA(cudaMemcpyAsync(cnt.data(), b.cnt, sizeof(int) * (size_t)N, cudaMemcpyDeviceToHost, st));
+    NEP_CUDA(cudaMemcpyAsync(&bad, b.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NEP_CUDA(cudaStreamSynchronize(st));                  // the host vectors above are temporaries, too
+    if (bad & 2) return nep_fail(nep, NEP_ERR_INVALID_ARG, "an atom type is outside [0, n_types)");
+    int cap = 1;
+    for (int i = 0; i < N; ++i) if (cnt[(size_t)i] > cap) cap = cnt[(size_t)i];
+    if (cap > 65535) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 65535 neighbour entries per atom");
+    NEP_TRY(dev_alloc(nep, &b.nbr, (size_t)N * cap));
+    NEP_TRY(dev_alloc(nep, &b.d, (size_t)N * cap));
+    NEP_TRY(dev_alloc(nep, &b.code, (size_t)N * cap));
+    NEP_TRY(dev_alloc(nep, &b.rev, (size_t)N * cap));
+    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, 1, cap,
+                                                                          b.cnt, b.nbr, b.d, b.code, b.bad));
+    NEP_LAUNCH(NEP_K_BATCH, kb_reverse<<<div_up(N, 128), 128, 0, st>>>(N, cap, b.cnt, b.nbr, b.code, b.rev, b.bad));
+    NEP_CUDA(cudaMemcpyAsync(&bad, b.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NEP_CUDA(cudaStreamSynchronize(st));
+    if (bad & 1) return nep_fail(nep, NEP_ERR_CUDA, "batch neighbours: an entry has no reverse entry (internal error)");
+    b.N = N; b.cap = cap; b.n_str = n_str; b.scratch_rows = 0;
+    return NEP_OK;
+}
+
+int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const float* c_angular, const float* w0, const float* b0,
+                      const float* w1, const float* b1, double* energy_dev, double* force_dev, double* virial_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (n_pop < 1 || !c_radial || !c_angular || !w0 || !b0 || !w1 || !b1 || !energy_dev) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n_pop < 1");
+    auto& b = nep->b;
+    if (b.n_str < 1) return nep_fail(nep, NEP_ERR_STATE, "nep_batch_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    static const NepCoef C = make_coef();
+    const NepDims& d = nep->d;
+    cudaStream_t st = nep->stream;
+    const size_t N = (size_t)b.N;
+    // parameters of ALL members: six copies, no per-member synchronisation
+    const size_t per[6] = {(size_t)d.T * d.T * d.NR * d.KR, (size_t)d.T * d.T * d.NA * d.KA, (size_t)d.H * d.D, (size_t)d.H, (size_t)d.H, 1};
+    const float* src[6] = {c_radial, c_angular, w0, b0, w1, b1};
+    for (int a = 0; a < 6; ++a) {
+        if (per[a] * n_pop > b.par_cap[a]) {
+            b.par_cap[a] = 0;
+            NEP_TRY(dev_alloc(nep, &b.par[a], per[a] * n_pop));
+            b.par_cap[a] = per[a] * n_pop;
+        }
+        NEP_CUDA(cudaMemcpyAsync(b.par[a], src[a], sizeof(float) * per[a] * n_pop, cudaMemcpyHostToDevice, st));
+    }
+    // scratch per (member, atom); members in chunks of at most ~4 GB
+    const size_t row_bytes = sizeof(float) * (2 * (size_t)d.D + (size_t)d.NA * NEP_NUM_S + d.H) + sizeof(float4) * b.cap;
+    size_t mchunk = (size_t)4e9 / (row_bytes * N);
+    if (mchunk < 1) mchunk = 1;
+    if (mchunk > (size_t)n_pop) mchunk = (size_t)n_pop;
+    if (mchunk > 65535) mchunk = 65535;                  // gridDim.y
+    if (mchunk * N > b.scratch_rows) {
+        b.scratch_rows = 0;
+        NEP_TRY(dev_alloc(nep, &b.q, mchunk * N * d.D));
+        NEP_TRY(dev_alloc(nep, &b.fp, mchunk * N * d.D));
+        NEP_TRY(dev_alloc(nep, &b.S, mchunk * N * d.NA * NEP_NUM_S));
+        NEP_TRY(dev_alloc(nep, &b.cf, mchunk * N * d.H));
+        NEP_TRY(dev_alloc(nep, &b.pf, mchunk * N * b.cap));
+        b.scratch_rows = mchunk * N;
+    }
+    for (size_t p0 = 0; p0 < (size_t)n_pop; p0 += mchunk) {
+        const int np = (int)((size_t)n_pop - p0 < mchunk ? (size_t)n_pop - p0 : mchunk);
+        BatchParams P = {b.par[0] + p0 * per[0], b.par[1] + p0 * per[1], b.par[2] + p0 * per[2], b.par[3] + p0 * per[3],
+                         b.par[4] + p0 * per[4], b.par[5] + p0 * per[5]};
+        const dim3 grid(div_up(b.N, 128), np);
+        NEP_LAUNCH(NEP_K_BATCH, kb_descriptors<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.fp, b.cf, energy_dev + p0 * N));
+        if (force_dev || virial_dev) {
+            NEP_LAUNCH(NEP_K_BATCH, kb_partial<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf));
+            NEP_LAUNCH(NEP_K_BATCH, kb_gather<<<grid, 128, 0, st>>>(b.N, b.cap, b.cnt, b.nbr, b.d, b.rev, b.pf, force_dev ? force_dev + 3 * p0 * N : nullptr,
+                                                                    virial_dev ? virial_dev + 9 * p0 * N : nullptr));
+        }
+    }
+    NEP_CUDA(cudaStreamSynchronize(st));                  // the caller may free or reuse its host parameter arrays
+    return NEP_OK;
+}
+
+int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const double* force_dev, const double* virial_dev,
+                   const double* u_target_dev, const double* f_target_dev, const double* w_target_dev, double* loss_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (n_pop < 1 || !energy_dev || !force_dev || !virial_dev || !u_target_dev || !f_target_dev || !w_target_dev || !loss_dev)
+        return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer or n_pop < 1");
+    auto& b = nep->b;
+    if (b.n_str < 1) return nep_fail(nep, NEP_ERR_STATE, "nep_batch_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    const size_t need = 3 * (size_t)n_pop * b.n_str;
+    if (need > b.loss_cap) {
+        b.loss_cap = 0;
+        NEP_TRY(dev_alloc(nep, &b.loss_part, need));
+        b.loss_cap = need;
+    }
+    for (int p0 = 0; p0 < n_pop; p0 += 65535) {
+        const int np = n_pop - p0 < 65535 ? n_pop - p0 : 65535;
+        const size_t o = (size_t)p0 * b.N;
+        NEP_LAUNCH(NEP_K_BATCH, kb_loss_partial<<<dim3(b.n_str, np), 128, 0, nep->stream>>>(b.N, b.n_str, b.off, energy_dev + o, force_dev + 3 * o, virial_dev + 9 * o,
+                                                                                          u_target_dev, f_target_dev, w_target_dev, b.loss_part + 3 * (size_t)p0 * b.n_str));
+    }
+    NEP_LAUNCH(NEP_K_BATCH, kb_loss_total<<<n_pop, 128, 0, nep->stream>>>(b.N, b.n_str, b.loss_part, loss_dev));
+    return NEP_OK;
+}
+
 // ---- host-buffer entry points ---------------------------------------------------------------------------
 static int stage_alloc(nep_t* nep, int64_t n)
 {
@@ -1221,7 +1378,7 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 // ---- measurement support ----------------------------------------------------------------------------------
 static const char* const kKernelNames[NEP_K_COUNT] = {
     "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
-    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export"};
+    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export", "batch"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
 

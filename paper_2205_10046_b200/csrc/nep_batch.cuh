@@ -1,0 +1,433 @@
+// nep_batch.cuh -- SURVEY.md section 8(f) row 4: population-batched evaluation for training.
+//
+// SNES evaluates, per generation, a POPULATION of parameter sets on a BATCH of small structures and reduces
+// the loss of Eq. (33).  The MD path is built for one large cell; this path is built for
+// many small ones:
+//   * structures are concatenated (atom_offset[s] .. atom_offset[s+1]); each has its own cell, which may be
+//     thinner than 2 r_c: the neighbours of an atom are ALL lattice images within the cutoffs (DESIGN.md reading
+//     A18), found once per batch -- the geometry does not depend on the parameters -- by a plain fp64 loop over
+//     image shifts, stored per entry as the fp32 pair vector (rounded from the fp64 difference) plus the slot of the
+//     reverse entry (j -> i, -N) in j's list;
+//   * one launch covers all structures x all members: grid.x runs over the atoms of the batch, grid.y over the
+//     members; member p reads its parameters at p * stride from device arrays uploaded once per call (no
+//     per-member synchronisation), so the blocks of one member share its coefficients through L1;
+//   * per member: descriptors + network (kb_descriptors), partial forces of every entry (kb_partial, Eq. (21)),
+//     F_i and W_i from the own and the reverse entries (kb_gather, Eqs. (22)-(24));
+//   * the data terms of Eq. (33) are reduced on the device per (member, structure) and then per member in a
+//     fixed order (kb_loss_partial, kb_loss_total).
+// fp32 arithmetic like the MD path, fp64 outputs.  One thread per (atom, member); loops over n, k
+// have run-time bounds (any hyper-parameters), the angular sums are held 4 channels at a time.
+#pragma once
+#include "nep_common.cuh"
+#include "nep_kernels.cuh"
+
+#define NEP_BATCH_MAX_SHIFT 7      // |image shift relative to the minimum image| per axis that fits the reverse-entry code
+
+struct BatchParams {               // device pointers to the parameters of ALL members, member-major
+    const float* cR;               // [n_pop][T][T][NR][KR]
+    const float* cA;               // [n_pop][T][T][NA][KA]
+    const float* w0;               // [n_pop][H][D]
+    const float* b0;               // [n_pop][H]
+    const float* w1;               // [n_pop][H]
+    const float* b1;               // [n_pop]
+};
+
+// ---- neighbour entries with lattice images (reading A18); count pass (fill = 0) and fill pass (fill = 1) --------
+__global__ void __launch_bounds__(128)
+kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, const double* __restrict__ Hs,
+             const double* __restrict__ Hinvs, const int* __restrict__ Ms, const double* __restrict__ pos,
+             const int* __restrict__ type, int n_types, double rcR,
+             int fill, int cap, int* __restrict__ cnt, int* __restrict__ nbr, float4* __restrict__ dvec,
+             unsigned short* __restrict__ code, int* __restrict__ bad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    if ((unsigned)type[i] >= (unsigned)n_types) atomicOr(bad, 2);
+    const int s = sid[i];
+    const double* H = Hs + 9 * s;
+    const double* inv = Hinvs + 9 * s;
+    const int Ma = Ms[3 * s], Mb = Ms[3 * s + 1], Mc = Ms[3 * s + 2];
+    const double rc2 = rcR * rcR;
+    const double xi = pos[3 * (size_t)i], yi = pos[3 * (size_t)i + 1], zi = pos[3 * (size_t)i + 2];
+    int c = 0;
+    for (int j = off[s]; j < off[s + 1]; ++j) {
+        const double tx = __dsub_rn(pos[3 * (size_t)j], xi), ty = __dsub_rn(pos[3 * (size_t)j + 1], yi), tz = __dsub_rn(pos[3 * (size_t)j + 2], zi);
+        double n0[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            n0[k] = rint(__dadd_rn(__dadd_rn(__dmul_rn(tx, inv[k]), __dmul_rn(ty, inv[3 + k])), __dmul_rn(tz, inv[6 + k])));
+        for (int ma = -Ma; ma <= Ma; ++ma)
+            for (int mb = -Mb; mb <= Mb; ++mb)
+                for (int mc = -Mc; mc <= Mc; ++mc) {
+                    const double Na = n0[0] + ma, Nb = n0[1] + mb, Nc = n0[2] + mc;
+                    if (j == i && Na == 0.0 && Nb == 0.0 && Nc == 0.0) continue;
+                    const double t[3] = {tx, ty, tz};
+                    double d[3];
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+                        d[a] = __dsub_rn(__dsub_rn(__dsub_rn(t[a], __dmul_rn(Na, H[a])), __dmul_rn(Nb, H[3 + a])), __dmul_rn(Nc, H[6 + a]));
+                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+                    if (d2 < rc2) {
+                        if (fill && c < cap) {
+                            const size_t e = (size_t)i * cap + c;
+                            nbr[e] = j;
+                            dvec[e] = make_float4((float)d[0], (float)d[1], (float)d[2], (float)sqrt(d2));
+                            code[e] = (unsigned short)((ma + 8) | ((mb + 8) << 4) | ((mc + 8) << 8));
+                        }
+                        ++c;
+                    }
+                }
+    }
+    cnt[i] = c;
+}
+
+// slot of the reverse entry (j -> i, -N): same atoms, opposite shift relative to the (odd-symmetric) minimum image
+__global__ void __launch_bounds__(128)
+kb_reverse(int N, int cap, const int* __restrict__ cnt, const int* __restrict__ nbr, const unsigned short* __restrict__ code,
+           unsigned short* __restrict__ rev, int* __restrict__ bad)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    for (int m = 0; m < cnt[i]; ++m) {
+        const size_t e = (size_t)i * cap + m;
+        const int j = nbr[e];
+        const unsigned cd = code[e];
+        const unsigned want = (16u - (cd & 15u)) | ((16u - ((cd >> 4) & 15u)) << 4) | ((16u - ((cd >> 8) & 15u)) << 8);
+        int found = -1;
+        for (int mm = 0; mm < cnt[j]; ++mm)
+            if (nbr[(size_t)j * cap + mm] == i && code[(size_t)j * cap + mm] == want) { found = mm; break; }
+        if (found < 0) { atomicOr(bad, 1); found = 0; }
+        rev[e] = (unsigned short)found;
+    }
+}
+
+// f_k and f_k' of Eqs. (3)-(5) for k = 0..K-1 from the shared basis head:  f_k = (T_k + 1) f_c / 2,
+// f_k' = T_k'(x) x'(r) f_c / 2 + (T_k + 1) f_c' / 2
+struct ChebWalk {
+    BasisHead h; float Tkm1, Tk, Dkm1, Dk; int k;
+    __device__ __forceinline__ ChebWalk(float r, float rc_inv) : h(basis_head<true>(r, rc_inv)), Tkm1(1.0f), Tk(1.0f), Dkm1(0.0f), Dk(0.0f), k(0) {}
+    __device__ __forceinline__ void get(float& f, float& df) const { f = (Tk + 1.0f) * h.hfc; df = fmaf(Dk, h.hfc_dx, (Tk + 1.0f) * h.hdfc); }
+    __device__ __forceinline__ void step()
+    {
+        if (k == 0) { Tkm1 = 1.0f; Tk = h.x; Dkm1 = 0.0f; Dk = 1.0f; }
+        else {
+            const float Dn = fmaf(h.two_x, Dk, fmaf(2.0f, Tk, -Dkm1)), Tn = fmaf(h.two_x, Tk, -Tkm1);
+            Dkm1 = Dk; Dk = Dn; Tkm1 = Tk; Tk = Tn;
+        }
+        ++k;
+    }
+};
+
+// ---- descriptors + network: q, S, Fp, U of one (atom, member) --------------------------------------------------
+// scratch per (member, atom): q [D] (also the network input), S [NA][24], fp [D]; row-major, one row per thread
+__global__ void __launch_bounds__(128)
+kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
+               const int* __restrict__ nbr, const float4* __restrict__ dvec,
+               float* __restrict__ qbuf, float* __restrict__ Sbuf, float* __restrict__ fpbuf, float* __restrict__ cfbuf,
+               double* __restrict__ energy)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y;
+    if (i >= N) return;
+    const size_t row = (size_t)p * N + i;
+    const int ti = type[i], T = D.T;
+    const float* cR = P.cR + (size_t)p * T * T * D.NR * D.KR;
+    const float* cA = P.cA + (size_t)p * T * T * D.NA * D.KA;
+    float* q = qbuf + row * D.D;
+    float* S = Sbuf + row * D.NA * NEP_NUM_S;
+    const int c = cnt[i];
+    // Eq. (2)-(3): q_n = sum_j sum_k c_nk f_k(r_ij)
+    for (int n0 = 0; n0 < D.NR; n0 += 4) {
+        float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+        for (int m = 0; m < c; ++m) {
+            const size_t e = (size_t)i * cap + m;
+            const float r = dvec[e].w;
+            const float* cc = cR + ((size_t)(ti * T + type[nbr[e]]) * D.NR + n0) * D.KR;
+            ChebWalk w(r, D.rcR_inv);
+            for (int k = 0; k < D.KR; ++k) {
+                float f, df; w.get(f, df);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) if (n0 + u < D.NR) acc[u] = fmaf(__ldg(cc + u * D.KR + k), f, acc[u]);
+                w.step();
+            }
+        }
+        for (int u = 0; u < 4; ++u) if (n0 + u < D.NR) q[n0 + u] = acc[u];
+    }
+    // Eq. (12) and Eqs. (13)-(19), four channels at a time
+    for (int n0 = 0; n0 < D.NA; n0 += 4) {
+        float Sa[4][NEP_NUM_S];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = 0.0f;
+        for (int m = 0; m < c; ++m) {
+            const size_t e = (size_t)i * cap + m;
+            const float4 d = dvec[e];
+            if (d.w >= D.rcA) continue;
+            const float rinv = 1.0f / d.w;
+            const float* cc = cA + ((size_t)(ti * T + type[nbr[e]]) * D.NA + n0) * D.KA;
+            float g[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            ChebWalk w(d.w, D.rcA_inv);
+            for (int k = 0; k < D.KA; ++k) {
+                float f, df; w.get(f, df);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) if (n0 + u < D.NA) g[u] = fmaf(__ldg(cc + u * D.KA + k), f, g[u]);
+                w.step();
+            }
+            float b[NEP_NUM_S];
+            angular_b(d.x * rinv, d.y * rinv, d.z * rinv, b);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = fmaf(g[u], b[k], Sa[u][k]);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int nn = n0 + u;
+            if (nn < D.NA) {
+                float out[6];
+                q_from_S(Sa[u], C, out);
+                for (int l = 0; l < 4; ++l) q[D.NR + l * D.NA + nn] = out[l];
+                if (D.has4) q[D.NR + 4 * D.NA + nn] = out[4];
+                if (D.has5) q[D.NR + (4 + D.has4) * D.NA + nn] = out[5];
+#pragma unroll
+                for (int k = 0; k < NEP_NUM_S; ++k) S[nn * NEP_NUM_S + k] = Sa[u][k];
+            }
+        }
+    }
+    // Eq. (1) / Listing 1: U and Fp = dU/dq
+    const float* w0 = P.w0 + (size_t)p * D.H * D.D;
+    const float* b0 = P.b0 + (size_t)p * D.H;
+    const float* w1 = P.w1 + (size_t)p * D.H;
+    float* cf = cfbuf + row * D.H;
+    float u_i = 0.0f;
+    for (int m = 0; m < D.H; ++m) {
+        float z = -__ldg(b0 + m);
+        for (int v = 0; v < D.D; ++v) z = fmaf(__ldg(w0 + (size_t)m * D.D + v), q[v], z);
+        const float x1 = tanhf(z), w1m = __ldg(w1 + m);
+        u_i = fmaf(w1m, x1, u_i);
+        cf[m] = w1m * (1.0f - x1 * x1);
+    }
+    float* fp = fpbuf + row * D.D;
+    for (int v = 0; v < D.D; ++v) {
+        float a = 0.0f;
+        for (int m = 0; m < D.H; ++m) a = fmaf(cf[m], __ldg(w0 + (size_t)m * D.D + v), a);
+        fp[v] = a;
+    }
+    energy[row] = (double)(u_i - __ldg(P.b1 + p));
+}
+
+// grad P_k(u) of the 24 polynomials on the unit vector (table of SURVEY.md section 8(c)), and the assembly of Eq. (21):
+//   pf = [sum_k (B_k - l_k A_k / r) b_k] u + (1/r) sum_k A_k grad P_k(u)
+__device__ __forceinline__ void angular_assemble(const float* A, const float* B, float x, float y, float z, float rinv, float* pf)
+{
+    float b[NEP_NUM_S];
+    angular_b(x, y, z, b);
+    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z, xyz = xy * z;
+    float cu = 0.0f, vx = 0.0f, vy = 0.0f, vz = 0.0f;
+#define KB_USE(k, l, gx, gy, gz)                                                                   \
+    { cu = fmaf(fmaf(-(float)(l) * rinv, A[k], B[k]), b[k], cu); vx = fmaf(A[k], (gx), vx); vy = fmaf(A[k], (gy), vy); vz = fmaf(A[k], (gz), vz); }
+    KB_USE(0, 1, 0.0f, 0.0f, 1.0f)
+    KB_USE(1, 1, 1.0f, 0.0f, 0.0f)
+    KB_USE(2, 1, 0.0f, 1.0f, 0.0f)
+    KB_USE(3, 2, -2.0f * x, -2.0f * y, 4.0f * z)
+    KB_USE(4, 2, z, 0.0f, x)
+    KB_USE(5, 2, 0.0f, z, y)
+    KB_USE(6, 2, 2.0f * x, -2.0f * y, 0.0f)
+    KB_USE(7, 2, 2.0f * y, 2.0f * x, 0.0f)
+    KB_USE(8, 3, -6.0f * xz, -6.0f * yz, -3.0f * (x2 + y2 - 2.0f * z2))
+    KB_USE(9, 3, -3.0f * x2 - y2 + 4.0f * z2, -2.0f * xy, 8.0f * xz)
+    KB_USE(10, 3, -2.0f * xy, -x2 - 3.0f * y2 + 4.0f * z2, 8.0f * yz)
+    KB_USE(11, 3, 2.0f * xz, -2.0f * yz, x2 - y2)
+    KB_USE(12, 3, 2.0f * yz, 2.0f * xz, 2.0f * xy)
+    KB_USE(13, 3, 3.0f * (x2 - y2), -6.0f * xy, 0.0f)
+    KB_USE(14, 3, 6.0f * xy, 3.0f * (x2 - y2), 0.0f)
+    KB_USE(15, 4, 12.0f * x * (x2 + y2 - 4.0f * z2), 12.0f * y * (x2 + y2 - 4.0f * z2), -16.0f * z * (3.0f * x2 + 3.0f * y2 - 2.0f * z2))
+    KB_USE(16, 4, -z * (9.0f * x2 + 3.0f * y2 - 4.0f * z2), -6.0f * xyz, -3.0f * x * (x2 + y2 - 4.0f * z2))
+    KB_USE(17, 4, -6.0f * xyz, -z * (3.0f * x2 + 9.0f * y2 - 4.0f * z2), -3.0f * y * (x2 + y2 - 4.0f * z2))
+    KB_USE(18, 4, -4.0f * x * (x2 - 3.0f * z2), 4.0f * y * (y2 - 3.0f * z2), 12.0f * z * (x2 - y2))
+    KB_USE(19, 4, -2.0f * y * (3.0f * x2 + y2 - 6.0f * z2), -2.0f * x * (x2 + 3.0f * y2 - 6.0f * z2), 24.0f * xyz)
+    KB_USE(20, 4, 3.0f * z * (x2 - y2), -6.0f * xyz, x * (x2 - 3.0f * y2))
+    KB_USE(21, 4, 6.0f * xyz, 3.0f * z * (x2 - y2), y * (3.0f * x2 - y2))
+    KB_USE(22, 4, 4.0f * x * (x2 - 3.0f * y2), -4.0f * y * (3.0f * x2 - y2), 0.0f)
+    KB_USE(23, 4, 4.0f * y * (3.0f * x2 - y2), 4.0f * x * (x2 - 3.0f * y2), 0.0f)
+#undef KB_USE
+    pf[0] = fmaf(cu, x, rinv * vx); pf[1] = fmaf(cu, y, rinv * vy); pf[2] = fmaf(cu, z, rinv * vz);
+}
+
+// ---- partial forces dU_i/dr_ij of every entry, Eq. (21) -----------------------------------------------------------
+__global__ void __launch_bounds__(128)
+kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
+           const int* __restrict__ nbr, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
+           const float* __restrict__ fpbuf, float4* __restrict__ pfbuf)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y;
+    if (i >= N) return;
+    const size_t row = (size_t)p * N + i;
+    const int ti = type[i], T = D.T;
+    const float* cR = P.cR + (size_t)p * T * T * D.NR * D.KR;
+    const float* cA = P.cA + (size_t)p * T * T * D.NA * D.KA;
+    const float* fp = fpbuf + row * D.D;
+    const float* S = Sbuf + row * D.NA * NEP_NUM_S;
+    float4* pf = pfbuf + row * cap;
+    const int c = cnt[i];
+    // first term of Eq. (21): sum_n Fp_n g_n'(r) u
+    for (int m = 0; m < c; ++m) {
+        const size_t e = (size_t)i * cap + m;
+        const float4 d = dvec[e];
+        const float rinv = 1.0f / d.w;
+        const int tp = ti * T + type[nbr[e]];
+        float s = 0.0f;
+        ChebWalk w(d.w, D.rcR_inv);
+        for (int k = 0; k < D.KR; ++k) {
+            float f, df; w.get(f, df);
+            float a = 0.0f;
+            for (int n = 0; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cR + ((size_t)tp * D.NR + n) * D.KR + k), a);
+            s = fmaf(a, df, s);
+            w.step();
+        }
+        pf[m] = make_float4(s * d.x * rinv, s * d.y * rinv, s * d.z * rinv, 0.0f);
+    }
+    // last three terms, four channels at a time (pf is linear in A_k = sum_n G_nk g_n and B_k = sum_n G_nk g_n')
+    for (int n0 = 0; n0 < D.NA; n0 += 4) {
+        float G[4][NEP_NUM_S];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int n = min(n0 + u, D.NA - 1);
+            float Sv[NEP_NUM_S], f3[4];
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S; ++k) Sv[k] = S[n * NEP_NUM_S + k];
+            for (int l = 0; l < 4; ++l) f3[l] = fp[D.NR + l * D.NA + n];
+            const float f4 = D.has4 ? fp[D.NR + 4 * D.NA + n] : 0.0f;
+            const float f5 = D.has5 ? fp[D.NR + (4 + D.has4) * D.NA + n] : 0.0f;
+            G_from_S(Sv, f3, f4, f5, C, G[u]);
+            if (n0 + u >= D.NA) {
+#pragma unroll
+                for (int k = 0; k < NEP_NUM_S; ++k) G[u][k] = 0.0f;
+            }
+        }
+        for (int m = 0; m < c; ++m) {
+            const size_t e = (size_t)i * cap + m;
+            const float4 d = dvec[e];
+            if (d.w >= D.rcA) continue;
+            const float rinv = 1.0f / d.w;
+            const int tp = ti * T + type[nbr[e]];
+            float g[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dg[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            ChebWalk w(d.w, D.rcA_inv);
+            for (int k = 0; k < D.KA; ++k) {
+                float f, df; w.get(f, df);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (n0 + u < D.NA) {
+                        const float cc = __ldg(cA + ((size_t)tp * D.NA + n0 + u) * D.KA + k);
+                        g[u] = fmaf(cc, f, g[u]); dg[u] = fmaf(cc, df, dg[u]);
+                    }
+                }
+                w.step();
+            }
+            float A[NEP_NUM_S], B[NEP_NUM_S];
+#pragma unroll
+            for (int k = 0; k < NEP_NUM_S; ++k) {
+                A[k] = G[0][k] * g[0]; B[k] = G[0][k] * dg[0];
+#pragma unroll
+                for (int u = 1; u < 4; ++u) { A[k] = fmaf(G[u][k], g[u], A[k]); B[k] = fmaf(G[u][k], dg[u], B[k]); }
+            }
+            float pa[3];
+            angular_assemble(A, B, d.x * rinv, d.y * rinv, d.z * rinv, rinv, pa);
+            float4 o = pf[m];
+            o.x += pa[0]; o.y += pa[1]; o.z += pa[2];
+            pf[m] = o;
+        }
+    }
+}
+
+// ---- F_i = sum (dU_i/dr_ij - dU_j/dr_ji), W_i = sum r_ij (x) dU_j/dr_ji over all entries (Eqs. 22-24) -----------------
+__global__ void __launch_bounds__(128)
+kb_gather(int N, int cap, const int* __restrict__ cnt, const int* __restrict__ nbr, const float4* __restrict__ dvec,
+          const unsigned short* __restrict__ rev, const float4* __restrict__ pfbuf, double* __restrict__ force, double* __restrict__ virial)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y;
+    if (i >= N) return;
+    const size_t row = (size_t)p * N + i;
+    float f[3] = {0.0f, 0.0f, 0.0f}, w[9];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) w[a] = 0.0f;
+    for (int m = 0; m < cnt[i]; ++m) {
+        const size_t e = (size_t)i * cap + m;
+        const float4 own = pfbuf[row * cap + m];
+        const float4 oth = pfbuf[((size_t)p * N + nbr[e]) * cap + rev[e]];     // dU_j/dr_ji
+        const float4 d = dvec[e];
+        f[0] += own.x - oth.x; f[1] += own.y - oth.y; f[2] += own.z - oth.z;
+        w[0] = fmaf(d.x, oth.x, w[0]); w[1] = fmaf(d.x, oth.y, w[1]); w[2] = fmaf(d.x, oth.z, w[2]);
+        w[3] = fmaf(d.y, oth.x, w[3]); w[4] = fmaf(d.y, oth.y, w[4]); w[5] = fmaf(d.y, oth.z, w[5]);
+        w[6] = fmaf(d.z, oth.x, w[6]); w[7] = fmaf(d.z, oth.y, w[7]); w[8] = fmaf(d.z, oth.z, w[8]);
+    }
+    if (force) { force[3 * row] = (double)f[0]; force[3 * row + 1] = (double)f[1]; force[3 * row + 2] = (double)f[2]; }
+    if (virial) {
+#pragma unroll
+        for (int a = 0; a < 9; ++a) virial[9 * row + a] = (double)w[a];
+    }
+}
+
+// ---- loss of Eq. (33): one block per (structure, member): squared per-structure terms {dU^2, sum |dF|^2, sum dW^2} ----
+__global__ void __launch_bounds__(128)
+kb_loss_partial(int N, int n_str, const int* __restrict__ off, const double* __restrict__ energy, const double* __restrict__ force,
+                const double* __restrict__ virial, const double* __restrict__ u_tar, const double* __restrict__ f_tar,
+                const double* __restrict__ w_tar, double* __restrict__ part)
+{
+    __shared__ double sh[11][128];
+    const int s = blockIdx.x, p = blockIdx.y;
+    const int a0 = off[s], a1 = off[s + 1];
+    double v[11];
+#pragma unroll
+    for (int a = 0; a < 11; ++a) v[a] = 0.0;
+    for (int i = a0 + threadIdx.x; i < a1; i += 128) {          // fixed assignment of atoms to threads: reproducible
+        const size_t row = (size_t)p * N + i;
+        v[0] += energy[row];
+        for (int a = 0; a < 3; ++a) { const double df = force[3 * row + a] - f_tar[3 * (size_t)i + a]; v[1] += df * df; }
+        for (int a = 0; a < 9; ++a) v[2 + a] += virial[9 * row + a];
+    }
+#pragma unroll
+    for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] = v[a];
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int a = 0; a < 11; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double ns = (double)(a1 - a0);
+        const double de = sh[0][0] / ns - u_tar[s];
+        const int six[6] = {0, 4, 8, 1, 5, 6};
+        double sv = 0.0;
+        for (int c = 0; c < 6; ++c) { const double dv = sh[2 + six[c]][0] / ns - w_tar[6 * s + c]; sv += dv * dv; }
+        double* o3 = part + 3 * ((size_t)p * n_str + s);
+        o3[0] = de * de; o3[1] = sh[1][0]; o3[2] = sv;
+    }
+}
+
+// one block per member: sums over the structures in a fixed order -> {L_e, L_f, L_v}
+__global__ void __launch_bounds__(128)
+kb_loss_total(int N, int n_str, const double* __restrict__ part, double* __restrict__ loss)
+{
+    __shared__ double sh[3][128];
+    const int p = blockIdx.x;
+    double v[3] = {0.0, 0.0, 0.0};
+    for (int s = threadIdx.x; s < n_str; s += 128)
+        for (int a = 0; a < 3; ++a) v[a] += part[3 * ((size_t)p * n_str + s) + a];
+    for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] = v[a];
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        loss[3 * p + 0] = sqrt(sh[0][0] / (double)n_str);
+        loss[3 * p + 1] = sqrt(sh[1][0] / (3.0 * (double)N));
+        loss[3 * p + 2] = sqrt(sh[2][0] / (6.0 * (double)n_str));
+    }
+}

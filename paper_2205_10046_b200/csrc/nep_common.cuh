@@ -19,7 +19,7 @@
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
     NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FORCE_RADIAL, NEP_K_FINAL,
-    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_COUNT
+    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_BATCH, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
 
@@ -147,8 +147,23 @@ struct nep_ctx {
     cudaStream_t copy_stream;   // md_run_host: second stream for the position download (created on first use)
     cudaEvent_t ev_pos;         // ... recorded when the positions of the last step are final
 
+    // batched evaluation for training (nep_batch.cuh): structures concatenated, lattice-image neighbour entries
+    struct {
+        int n_str, N, cap;                 // structures, atoms of the batch, storage slots per atom
+        int* off; int* sid; int* M;        // [n_str+1] atom offsets, [N] structure of an atom, [n_str][3] image reach
+        double* H; double* Hinv;           // [n_str][9]
+        int* type;                         // [N]
+        int* cnt; int* nbr;                // [N], [N][cap]
+        float4* d;                         // [N][cap] pair vector + distance
+        unsigned short* code; unsigned short* rev;   // [N][cap] image-shift code, slot of the reverse entry
+        int* bad;                          // [1] device flag
+        float* par[6]; size_t par_cap[6];  // parameters of all members of a call
+        float* q; float* S; float* fp; float* cf; float4* pf; size_t scratch_rows;   // per (member, atom) scratch of a chunk
+        double* loss_part; size_t loss_cap;
+    } b;
+
     // bookkeeping of owned device memory (nep_device_bytes)
-    struct { void* p; size_t bytes; } owned[96];
+    struct { void* p; size_t bytes; } owned[160];
     int n_owned;
 };
 
