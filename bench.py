@@ -45,6 +45,7 @@ METRIC = "atom-step/s (NEP force+MD step, 1 B200) and % of FP32/HBM roofline"
 UNIT = "atom-step/s"
 SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0     # B200_PROFILING.md "Nominal figures"
 L2_BYTES = 126e6
+PER_BUILD_IDS = ("build_rev", "scan")          # kernel ids whose cost entry is per list build, not per launch
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -79,6 +80,16 @@ def kernel_costs(h: W.Hyper, n_atoms: int, pairs_r: int, pairs_a: int, list_r: i
     # per-step filter of the skin lists to the in-cutoff lists (~12 flops per listed pair)
     out["filter"] = (list_r * 12, n * 32 + 4 * list_r + 4 * pairs_r)
     out["quantize"] = (n * 9, n * (24 + 4 + 4 + 16))
+    # a1, per build (every rebuild_every steps).  SURVEY.md 8(d): ~100 B/atom binning/reorder + 4 B x (L_R + L_A)
+    # list writes ~ 0.6 kB/atom and 300-500 candidate distance tests (~10 flops each) per atom.  The
+    # candidate count is the stencil's: 125 cells of edge (rc_R + skin)/2 = 3.73 x the sphere's volume.
+    cand = 3.73 * list_r
+    out["cell_hist"] = (n * 12, n * (24 + 4 + 4 + 4))
+    out["scatter"] = (0, n * (4 + 4 + 4 + 4))
+    out["sort_cells"] = (0, n * 8)
+    out["build_lists"] = (cand * 10, n * (16 + 8 + 4) + 4 * (list_r + list_a))
+    # reverse index: every listed pair needs the slot of i in j's list (one byte), found from j's list row
+    out["build_rev"] = (0, (4 + 1) * list_r)       # per build; divided by the launches of this id below
     out["kick_drift"] = (n * 3 * 5, n * (3 * 8 * 5 + 4))
     out["kick"] = (n * 3 * 3, n * (3 * 8 * 3 + 4))
     return out
@@ -199,13 +210,32 @@ def run_oracle_steps(cfg: W.Config, n_steps: int):
 
 
 def cpu_baseline(cfg: W.Config):
+    """The oracle on the host cores: its force evaluation GIVEN its neighbour lists, and
+    the O(N^2) brute-force search reported separately (oracle.last_timing: wall clock of the two parts of one
+    oracle.compute call).  cfg 0 and cfg 1 in full, cfg 2-4 on a 32,000-atom replica."""
     import oracle
-    scfg = oracle_sample_config(cfg, 32000)
-    secs, n, evals = run_oracle_steps(scfg, 2)
-    return {"value": n * evals / secs, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{n}-atom replica ({'x'.join(map(str, scfg.cells))} cells) of {cfg.name}, "
-                      f"{evals} fp64 force evaluations (oracle.md, 2 NVE steps) in {secs:.1f} s, "
-                      "O(N^2) neighbour search included"}
+    full = cfg.index in (0, 1)
+    scfg = cfg if full else oracle_sample_config(cfg, 32000)
+    s, p = W.make_system(scfg), W.make_params(scfg)
+    n = len(s.pos)
+    oracle.lib()
+    reps = 50 if n < 5000 else 1
+    t_search = t_eval = 0.0
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle.compute(scfg.hyper, p, s.pos, s.types, s.box)
+        a, b = oracle.last_timing()
+        t_search += a / reps
+        t_eval += b / reps
+    t_cmp = (time.perf_counter() - t0) / reps
+    what = (f"all {n} atoms of {cfg.name}" if full else
+            f"{n}-atom replica ({'x'.join(map(str, scfg.cells))} cells) of {cfg.name}")
+    return {"value": n / t_eval, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{what}: fp64 energy/force/virial evaluation given the neighbour lists, {t_eval:.3f} s of the "
+                      f"{t_cmp:.3f} s of one oracle.compute call (mean of {reps}); the rest is its O(N^2) search",
+            "search": {"seconds": t_search, "atoms_per_s": n / t_search,
+                       "what": "O(N^2) brute-force pair search of the same call (radial + angular lists)"},
+            "with_search_value": n / t_cmp}
 
 
 def config_dict(cfg: W.Config, n_atoms: int, extra=None):
@@ -307,12 +337,34 @@ def run_ours(args):
     nep.nep_profile(True)
     l0 = nep.nep_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    nep.md_step(pos, vel, cfg.dt_fs, K, cfg.rebuild_every, cfg.skin)
-    ev1.record()
-    barrier()
-    ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
+    windows = None
+    if args.windows and args.windows > 1:
+        # --windows W: the K steps as W consecutive md_step calls, each bracketed by its own event pair and a
+        # synchronize; between two windows the pair counts are read back (untimed).  ms = sum of the windows.
+        # Shows how ms/step moves with the trajectory (the in-cutoff pair counts grow as the lattice disorders).
+        windows, ms = [], 0.0
+        edges = [round(K * w / args.windows) for w in range(args.windows + 1)]
+        for w in range(args.windows):
+            kw = edges[w + 1] - edges[w]
+            if kw <= 0:
+                continue
+            barrier()
+            ev0.record()
+            nep.md_step(pos, vel, cfg.dt_fs, kw, cfg.rebuild_every, cfg.skin)
+            ev1.record()
+            barrier()
+            ms_w = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
+            ms += ms_w
+            pr, pa = nep.nep_pair_counts()
+            windows.append({"steps": [edges[w], edges[w + 1]], "ms_per_step": ms_w / kw,
+                            "pairs_in_rc_per_atom": [pr / n, pa / n]})
+    else:
+        barrier()
+        ev0.record()
+        nep.md_step(pos, vel, cfg.dt_fs, K, cfg.rebuild_every, cfg.skin)
+        ev1.record()
+        barrier()
+        ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
     clocks = sampler.stop()
     launches = nep.nep_launch_count() - l0
     prof = nep.nep_profile_read()
@@ -357,11 +409,16 @@ def run_ours(args):
     traffic = ncu_traffic(cfg.name)
     t_sum = sum(v[0] for v in prof.values())
     kernels = []
+    builds = prof.get("build_lists", (0.0, 0))[1]
     for name, (tot_ms, cnt) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
         avg_s = tot_ms / cnt * 1e-3
         entry = {"name": name, "launches": cnt, "avg_us": avg_s * 1e6, "share": tot_ms / t_sum}
         if name in costs and avg_s > 0:
             fl, by = costs[name]
+            if name in PER_BUILD_IDS and builds > 0 and cnt != builds:
+                # several launches share this id in one build: the cost stated is per build
+                fl, by = fl * builds / cnt, by * builds / cnt
+                costs[name] = (fl, by)
             entry.update({"tflops": fl / avg_s / 1e12, "alu_frac": fl / avg_s / 1e12 / alu_peak,
                           "gbs": by / avg_s / 1e9, "hbm_frac": by / avg_s / 1e9 / hbm_peak,
                           "flops_per_launch": fl, "bytes_per_launch": by})
@@ -394,6 +451,16 @@ def run_ours(args):
             "hbm_frac": step_bytes * K / (ms * 1e-3) / 1e9 / hbm_peak,
             "kernel_time_share_of_wall": t_sum / ms if world == 1 else None}
 
+    nb_ids = ("cell_hist", "scan", "scatter", "sort_cells", "build_lists", "build_rev")
+    nb_ms = sum(prof[k][0] for k in nb_ids if k in prof)
+    neighbour_pass = None
+    if builds > 0:
+        nb_bytes = sum(costs[k][1] * prof[k][1] for k in nb_ids if k in prof and k in costs) / builds
+        neighbour_pass = {"builds": builds, "us_per_build": nb_ms / builds * 1e3, "share_of_step": nb_ms / t_sum,
+                          "bytes_per_build": nb_bytes, "gbs": nb_bytes / (nb_ms / builds * 1e-3) / 1e9,
+                          "hbm_frac": nb_bytes / (nb_ms / builds * 1e-3) / 1e9 / hbm_peak,
+                          "note": "plus one k_quantize per build (counted under quantize)"}
+
     cpu = cpu_baseline(cfg) if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
 
     if rank == 0:
@@ -408,7 +475,8 @@ def run_ours(args):
                     "list_entries_per_atom": [list_r / n, list_a / n],
                     "max_displacement_since_build": disp}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-                "kernels": kernels, "step": step, "fp32_probe_tflops": fp32_probe,
+                "kernels": kernels, "step": step, "neighbour_pass": neighbour_pass, "windows": windows,
+                "fp32_probe_tflops": fp32_probe,
                 "cpu_baseline": cpu, "impl": "ours"}
         print(json.dumps(line), flush=True)
     nep.close()
@@ -425,6 +493,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: 1M atoms)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--windows", type=int, default=0,
+                    help="time the K steps as this many consecutive windows (ms/step and pair counts per window)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps

@@ -7,5 +7,5 @@ from .nep_oracle import (  # noqa: F401
     OracleHyper, build, lib, num_threads, num_descriptors, fc, fk, bk, bk_grad, constants, q_from_S,
     ann, neighbors, neighbors_of, compute, md, latent, heat_current, kinetic_temperature, md_berendsen,
     ACC_CONV, KB_EV_PER_K, counter_normal, langevin_half_step, md_langevin, loss_terms, regularisation_terms,
-    compute_images, count_images, loss_terms_batch,
+    compute_images, count_images, loss_terms_batch, last_timing,
 )

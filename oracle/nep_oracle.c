@@ -465,6 +465,16 @@ static int compute_impl(const onep_hyper* h,
                  double* energy, double* force, double* virial,
                  double* q_out, double* fp_out, double* S_out);
 
+static double g_last_search_s = 0.0, g_last_eval_s = 0.0;    /* see onep_last_timing */
+static double wall_seconds(void)
+{
+#ifdef _OPENMP
+    return omp_get_wtime();
+#else
+    return 0.0;
+#endif
+}
+
 int onep_compute(const onep_hyper* h,
                  const double* c_radial, const double* c_angular,
                  const double* w0, const double* b0, const double* w1, const double* b1,
@@ -518,8 +528,10 @@ static int compute_impl(const onep_hyper* h,
     if (has5 && nk_used < 3) nk_used = 3;
 
     int64_t *firstR = NULL, *firstA = NULL;
+    const double t_begin = wall_seconds();
     pair_t* PR = images ? build_pairs_images(n, pos, box, h->rc_radial, &firstR) : build_pairs(n, pos, box, pbc, h->rc_radial, &firstR);
     pair_t* PA = images ? build_pairs_images(n, pos, box, h->rc_angular, &firstA) : build_pairs(n, pos, box, pbc, h->rc_angular, &firstA);
+    const double t_lists = wall_seconds();
     double* q = (double*)calloc((size_t)(n * D + 1), sizeof(double));
     double* fp = (double*)calloc((size_t)(n * D + 1), sizeof(double));
     double* S = (double*)calloc((size_t)(n * NA * NUM_B + 1), sizeof(double));
@@ -649,8 +661,15 @@ static int compute_impl(const onep_hyper* h,
     if (fp_out) memcpy(fp_out, fp, sizeof(double) * (size_t)(n * D));
     if (S_out) memcpy(S_out, S, sizeof(double) * (size_t)(n * NA * NUM_B));
     free(PR); free(PA); free(firstR); free(firstA); free(q); free(fp); free(S); free(pfR); free(pfA);
+    g_last_search_s = t_lists - t_begin;
+    g_last_eval_s = wall_seconds() - t_lists;
     return 0;
 }
+
+/* Wall-clock split of the last onep_compute / onep_compute_images call (bench.py's cpu_baseline: BASELINE.md
+ * section 3 wants the evaluation given the lists and the O(N^2) search reported separately):
+ * out[0] = seconds in the brute-force pair search, out[1] = seconds in O2-O6.  Timing only; no arithmetic.  */
+void onep_last_timing(double out[2]) { out[0] = g_last_search_s; out[1] = g_last_eval_s; }
 
 /* ---- O7: velocity-Verlet NVE -------------------------------------------------------------------
  * per step: v += (dt/2) F/m;  r += dt v;  F = F(r);  v += (dt/2) F/m.   Units: eV, Angstrom, amu, fs:

@@ -69,6 +69,8 @@ def lib():
         L.onep_q_from_S.argtypes = [_dp, _dp, _dp]
         L.onep_ann.restype = None
         L.onep_ann.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.onep_last_timing.restype = None
+        L.onep_last_timing.argtypes = [C.POINTER(C.c_double * 2)]
         L.onep_neighbors.restype = C.c_int64
         L.onep_neighbors.argtypes = [C.c_int64, _dp, _dp, _ip, C.c_double, _ip, _ip, C.c_int64]
         L.onep_neighbors_of.restype = C.c_int64
@@ -215,6 +217,14 @@ def compute(hyper, params, pos, types, box, pbc=(1, 1, 1), want_internals: bool 
     if rc != 0:
         raise MemoryError("oracle allocation failed")
     return (e, f, w, q, fp, S) if want_internals else (e, f, w)
+
+
+def last_timing():
+    """(seconds in the O(N^2) pair search, seconds in the evaluation given the lists) of the last compute /
+    compute_images call -- wall clock only (bench.py's cpu_baseline)."""
+    out = (C.c_double * 2)()
+    lib().onep_last_timing(C.byref(out))
+    return float(out[0]), float(out[1])
 
 
 def compute_images(hyper, params, pos, types, box, want_internals: bool = False):
