@@ -485,6 +485,82 @@ def run_ours(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------------
+def run_batch(args):
+    """--workload batch: SURVEY.md 8(f) row 4, one SNES generation's evaluation -- a population of parameter sets
+    x a batch of small structures (nep_batch_compute) + the data terms of Eq. (33) per member (nep_batch_loss).
+    Not BASELINE.json's metric (that is the MD step above): a second, separately named line for the widened row.
+    A "step" = one generation: parameters uploaded from the host, E/F/W of every (member, atom), loss [n_pop][3]
+    read back to the host.  Structures: seeded replicas of cfg 3's five-species fcc lattice, 16-108 atoms, a third
+    of them sheared, most thinner than 2 r_c (lattice-image neighbours, reading A18)."""
+    import torch
+    from paper_2205_10046_b200 import NEP
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the NEP path has no CPU fallback)")
+    cfg = W.get_config(3)
+    shapes = [(2, 2, 2), (2, 2, 1), (3, 2, 2), (3, 3, 2), (3, 3, 3), (2, 1, 1)]
+    tilts = [None, None, (0.21, -0.13, 0.17)]
+    specs = [(shapes[k % len(shapes)], tilts[k % len(tilts)], k) for k in range(args.structures)]
+    structs = W.make_batch(3, specs)
+    members = W.make_population(cfg, args.pop, sigma=0.3)
+    off = np.concatenate([[0], np.cumsum([len(p) for p, _, _ in structs])]).astype(np.int32)
+    N, S, P = int(off[-1]), len(structs), len(members)
+    pos = torch.tensor(np.concatenate([p for p, _, _ in structs]), device="cuda:0")
+    typ = torch.tensor(np.concatenate([t for _, t, _ in structs]), device="cuda:0")
+    boxes = np.stack([H for _, _, H in structs])
+    nep = NEP(cfg.hyper, members[0], cfg.masses, device=0)
+    nep.nep_batch_neighbors(off, pos, typ, boxes)
+    rng = np.random.default_rng(7)
+    u_t = torch.tensor(rng.normal(size=S), device="cuda:0")
+    f_t = torch.tensor(rng.normal(size=(N, 3)) * 0.1, device="cuda:0")
+    w_t = torch.tensor(rng.normal(size=(S, 6)) * 0.1, device="cuda:0")
+
+    def generation():
+        e, f, w = nep.nep_batch_compute(members)
+        return nep.nep_batch_loss(e, f, w, u_t, f_t, w_t).cpu()
+
+    for _ in range(max(3, args.warmup)):
+        loss = generation()
+    torch.cuda.synchronize()
+    l0 = nep.nep_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        loss = generation()
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    assert torch.isfinite(loss).all()
+    launches = nep.nep_launch_count() - l0
+    # oracle on the host cores: compute_images of a few structures with one member
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        t0, na = time.perf_counter(), 0
+        for k in range(min(S, 12)):
+            p_, t_, H_ = structs[k]
+            oracle.compute_images(cfg.hyper, members[0], p_, t_, H_)
+            na += len(p_)
+        dt = time.perf_counter() - t0
+        cpu = {"value": na / dt, "unit": "atom-member evaluation/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"oracle.compute_images of the first {min(S, 12)} structures ({na} atoms), one member, {dt:.2f} s"}
+    line = {"metric": "atom-member evaluation/s (batched training evaluation, SURVEY.md 8(f) row 4)",
+            "value": N * P * args.steps / (ms * 1e-3), "unit": "atom-member evaluation/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic (seeded small structures + a seeded population, workloads.py)",
+            "config": {"workload": "batch_cfg3_fcc_alloy_small_cells", "structures": S, "atoms": N, "population": P,
+                       "atoms_per_structure": [int(np.diff(off).min()), int(np.diff(off).max())],
+                       "neighbour_entries_per_atom": None,
+                       "step": "host parameters -> nep_batch_compute (E, F, W of every member) -> nep_batch_loss -> host [n_pop][3]"},
+            "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours"}
+    print(json.dumps(line), flush=True)
+    nep.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -493,6 +569,10 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3: 1M atoms)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", choices=["md", "batch"], default="md",
+                    help="md: BASELINE.json's metric (default); batch: the batched training evaluation of SURVEY 8(f) row 4")
+    ap.add_argument("--structures", type=int, default=600, help="--workload batch: structures in the batch")
+    ap.add_argument("--pop", type=int, default=50, help="--workload batch: parameter sets (PAPER.md:283: a population)")
     ap.add_argument("--windows", type=int, default=0,
                     help="time the K steps as this many consecutive windows (ms/step and pair counts per window)")
     args = ap.parse_args()
@@ -500,6 +580,8 @@ def main():
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "batch":
+        return run_batch(args)
     return run_ours(args)
 
 

@@ -1364,11 +1364,14 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
     const Thermostat none = {0, 0.0, 0.0, 0.0, 0ull, 0};
     NEP_TRY(md_loop(nep, nep->h_pos, nep->h_vel, dt_fs, n_steps, rebuild_every, skin, none, nep->ev_pos, true));
     unsigned disp_bits = 0;
-    NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, nep->stream));
     NEP_CUDA(cudaStreamWaitEvent(nep->copy_stream, nep->ev_pos, 0));
     NEP_CUDA(cudaMemcpyAsync(pos_host, nep->h_pos, b3, cudaMemcpyDeviceToHost, nep->copy_stream));
     NEP_CUDA(cudaMemcpyAsync(vel_host, nep->h_vel, b3, cudaMemcpyDeviceToHost, nep->stream));
     NEP_TRY(download_results(nep, energy_host, force_host, virial_host));
+    // last: &disp_bits is pageable memory, so this copy returns only when the stream has reached it -- enqueued
+    // before the downloads above it would hold the host back and the position download would no longer overlap
+    // the force evaluation
+    NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, nep->stream));
     NEP_CUDA(cudaStreamSynchronize(nep->stream));
     NEP_CUDA(cudaStreamSynchronize(nep->copy_stream));
     nep->h_run = true;

@@ -23,21 +23,7 @@ def pkg():
     return p
 
 
-def make_batch(idx, specs):
-    """specs: [(cells, tilt or None, displacement seed)]: structures of config `idx`'s lattice and species rule."""
-    structs = []
-    for k, (cells, tilt, seed) in enumerate(specs):
-        cfg = W.get_config(idx, cells)
-        s = W.make_system(cfg)
-        rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 930, idx, k, seed]))
-        pos = s.pos + rng.normal(0.0, 0.05, size=s.pos.shape)               # every structure its own displacements
-        H = np.diag(s.box)
-        if tilt is not None:
-            F = np.array([[1.0, 0.0, 0.0], [tilt[0], 1.0, 0.0], [tilt[1], tilt[2], 1.0]])
-            pos, H = pos @ F, H @ F
-        pos = pos + rng.integers(-1, 2, size=pos.shape).astype(np.float64) @ H   # unwrapped input
-        structs.append((np.ascontiguousarray(pos), s.types.copy(), H))
-    return structs
+make_batch = W.make_batch
 
 
 BATCHES = [

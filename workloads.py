@@ -233,6 +233,27 @@ def perpendicular_widths(box33) -> np.ndarray:
                      vol / np.linalg.norm(np.cross(a, b))])
 
 
+def make_batch(idx: int, specs):
+    """A batch of small structures for the training-evaluation path: specs =
+    [(cells, tilt or None, seed)], each a replica of config `idx`'s lattice and species rule with its own seeded
+    displacements (sigma 0.05 A), optionally sheared by the lower-triangular tilt (xy, xz, yz), positions shifted by
+    random lattice vectors (unwrapped input).  Returns [(pos [n][3], types [n], cell rows [3][3])].  They stand in
+    for the paper's DFT training structures, which are not available."""
+    structs = []
+    for k, (cells, tilt, seed) in enumerate(specs):
+        cfg = get_config(idx, cells)
+        s = make_system(cfg)
+        rng = np.random.default_rng(np.random.SeedSequence([2205, 10046, 930, idx, k, seed]))
+        pos = s.pos + rng.normal(0.0, 0.05, size=s.pos.shape)               # every structure its own displacements
+        H = np.diag(s.box)
+        if tilt is not None:
+            F = np.array([[1.0, 0.0, 0.0], [tilt[0], 1.0, 0.0], [tilt[1], tilt[2], 1.0]])
+            pos, H = pos @ F, H @ F
+        pos = pos + rng.integers(-1, 2, size=pos.shape).astype(np.float64) @ H   # unwrapped input
+        structs.append((np.ascontiguousarray(pos), s.types.copy(), H))
+    return structs
+
+
 def make_population(cfg: Config, n_pop: int, sigma: float = 0.1, kind: str = "stress"):
     """A seeded population of parameter sets around make_params(cfg, kind), as an evolution strategy draws
     them: member m = mean + sigma * N(0, 1) per parameter, rounded to fp32.  Member 0 is the
