@@ -101,3 +101,34 @@ def test_oracle_sample_config_keeps_minimum_image():
         s = bench.oracle_sample_config(cfg, 3000)
         assert all(c * cfg.a >= 2 * (cfg.hyper.rc_radial + cfg.skin) for c in s.cells)
         assert all(c <= full for c, full in zip(s.cells, cfg.cells))
+
+
+def test_cpu_baseline_reports_the_evaluation_and_the_search_separately():
+    """the oracle's force evaluation given its lists, the O(N^2) search beside it (the two
+    parts of one oracle.compute call, oracle.last_timing); cfg 0 is timed in full."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import oracle
+    import workloads as W
+    cfg = W.get_config(0)
+    c = bench.cpu_baseline(cfg)
+    assert c["kind"] == "oracle" and c["cores"] == oracle.num_threads() and "all 256 atoms" in c["sample"]
+    assert c["value"] > c["with_search_value"] > 0 and c["search"]["atoms_per_s"] > 0
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    oracle.compute(cfg.hyper, p, s.pos, s.types, s.box)
+    t_search, t_eval = oracle.last_timing()
+    assert t_search > 0 and t_eval > 0
+
+
+def test_neighbour_pass_has_cost_entries():
+    """~0.6 kB/atom and 300-500 candidate tests per atom per build."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as W
+    h = W.get_config(3).hyper
+    n, lr, la = 1000, 78000, 45000
+    c = bench.kernel_costs(h, n, 45000, 18000, lr, la)
+    per_atom = sum(c[k][1] for k in ("cell_hist", "scatter", "sort_cells", "build_lists")) / n
+    assert 500 <= per_atom <= 700
+    assert 250 <= c["build_lists"][0] / 10 / n <= 500          # 3.73 x 78 = 291 candidate tests per atom
+    assert c["build_rev"][1] == 5 * lr
