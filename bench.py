@@ -342,7 +342,7 @@ def run_ours(args):
         # --windows W: the K steps as W consecutive md_step calls, each bracketed by its own event pair and a
         # synchronize; between two windows the pair counts are read back (untimed).  ms = sum of the windows.
         # Shows how ms/step moves with the trajectory (the in-cutoff pair counts grow as the lattice disorders).
-        windows, ms = [], 0.0
+        windows, ms, prev = [], 0.0, {}
         edges = [round(K * w / args.windows) for w in range(args.windows + 1)]
         for w in range(args.windows):
             kw = edges[w + 1] - edges[w]
@@ -356,8 +356,17 @@ def run_ours(args):
             ms_w = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
             ms += ms_w
             pr, pa = nep.nep_pair_counts()
+            cum = nep.nep_profile_read()                      # cumulative since nep_profile(True): difference = this window
+            kus = {k: (v[0] - prev.get(k, (0.0, 0))[0]) / max(1, v[1] - prev.get(k, (0.0, 0))[1]) * 1e3
+                   for k, v in cum.items() if v[1] > prev.get(k, (0.0, 0))[1]}
+            prev = cum
             windows.append({"steps": [edges[w], edges[w + 1]], "ms_per_step": ms_w / kw,
-                            "pairs_in_rc_per_atom": [pr / n, pa / n]})
+                            "pairs_in_rc_per_atom": [pr / n, pa / n],
+                            "longest_skin_lists": [nep.nep_max_neighbors(0), nep.nep_max_neighbors(1)],
+                            "list_raggedness": nep.nep_list_raggedness(),
+                            "kernel_avg_us": {k: round(v, 2) for k, v in kus.items()},
+                            "force_angular_ns_per_pair": kus.get("force_angular", 0.0) * 1e3 / max(1, pa),
+                            "force_radial_ns_per_pair": kus.get("force_radial", 0.0) * 1e3 / max(1, pr)})
     else:
         barrier()
         ev0.record()
@@ -473,7 +482,8 @@ def run_ours(args):
                                  f"{dev_bytes / 1e6:.0f} MB of device memory vs 126 MB of L2",
                     "pairs_in_rc_per_atom": [pairs_r / n, pairs_a / n],
                     "list_entries_per_atom": [list_r / n, list_a / n],
-                    "max_displacement_since_build": disp}),
+                    "max_displacement_since_build": disp,
+                    "list_raggedness": nep.nep_list_raggedness()}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "kernels": kernels, "step": step, "neighbour_pass": neighbour_pass, "windows": windows,
                 "fp32_probe_tflops": fp32_probe,

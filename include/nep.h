@@ -165,6 +165,12 @@ int nep_get_last(nep_t* nep, double* energy_dev, double* force_dev, double* viri
  * evaluation; the lists are valid while it is below skin/2.  Synchronises.                            */
 int nep_max_displacement(nep_t* nep, double* disp_host);
 
+/* Measurement support: raggedness of the skin lists of the last build -- the sum over warps (32 consecutive atoms
+ * of the internal order) of 32 x the longest list, divided by the sum of all list lengths: the factor by which a
+ * pair loop is slowed by idle lanes when a warp's atoms have unequal lists (1.0 in a perfect crystal; it grows as a
+ * structure disorders).  NEP_ERR_STATE before nep_neighbors.                            */
+int nep_list_raggedness(nep_t* nep, double* raggedness_host);
+
 /* ---- host-buffer entry points (end-to-end path: H2D copies, kernels, D2H copies) -------------------
  * All *_host arrays are HOST memory (pageable or pinned; pinned makes the copies asynchronous DMA).
  * The device staging copies are owned by the handle and reused between calls.  Both synchronise.

@@ -18,7 +18,7 @@ _lib = None
 # every symbol include/nep.h declares
 exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
-    "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement",
+    "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement", "nep_list_raggedness",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
     "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
     "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss",
@@ -84,6 +84,8 @@ def load_library():
     L.nep_get_last.argtypes = [vp, vp, vp, vp]
     L.nep_max_displacement.restype = C.c_int
     L.nep_max_displacement.argtypes = [vp, dp]
+    L.nep_list_raggedness.restype = C.c_int
+    L.nep_list_raggedness.argtypes = [vp, dp]
     L.nep_compute_host.restype = C.c_int
     L.nep_compute_host.argtypes = [vp, i64, vp, vp, dp, dbl, vp, vp, vp]
     L.md_run_host.restype = C.c_int
@@ -286,6 +288,12 @@ class NEP:
         self._check(self._L.nep_get_last(self._h_ptr, C.c_void_p(e.data_ptr()), C.c_void_p(f.data_ptr()),
                                          C.c_void_p(w.data_ptr())))
         return e, f, w
+
+    def nep_list_raggedness(self) -> float:
+        """Sum over warps of 32 x the longest skin list / sum of all list lengths, last build (1.0 = no idle lanes)."""
+        v = C.c_double(0.0)
+        self._check(self._L.nep_list_raggedness(self._h_ptr, C.byref(v)))
+        return v.value
 
     def nep_max_displacement(self) -> float:
         v = C.c_double(0.0)

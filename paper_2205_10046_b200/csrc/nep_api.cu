@@ -202,7 +202,6 @@ int build_lists(nep_t* nep, const double* pos_dev)
     NEP_LAUNCH(NEP_K_SCATTER, k_scatter<<<div_up(n, TB), TB, 0, st>>>(n, nep->cell_of, nep->rank_in_cell, nep->cell_start, nep->perm));
     NEP_LAUNCH(NEP_K_SORT_CELLS, k_sort_cells<<<div_up(nep->n_cells, TB), TB, 0, st>>>(nep->n_cells, nep->cell_start, nep->perm));
     NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, TB), TB, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
-    NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
     NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, 2 * sizeof(unsigned), st));
 
     if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
@@ -215,29 +214,36 @@ int build_lists(nep_t* nep, const double* pos_dev)
     for (int attempt = 0; attempt < 4; ++attempt) {
         P.capA = nep->capA; P.capS = nep->capS;
         NEP_CUDA(cudaMemsetAsync(nep->flags, 0, sizeof(int) * 8, st));
+        NEP_CUDA(cudaMemsetAsync(nep->build_stat, 0, sizeof(unsigned long long) * 2, st));
         if (P.tri) {
             NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<true><<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
-                                                              nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
+                                                              nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags, nep->build_stat));
         } else {
             NEP_LAUNCH(NEP_K_BUILD_LISTS, k_build_lists<false><<<div_up(n, 128), 128, 0, st>>>(P, pos_dev, nep->perm, nep->posq, nep->cell_start,
-                                                               nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags));
+                                                               nep->listA, nep->cntA, nep->listS, nep->cntS, nep->flags, nep->build_stat));
         }
         int fl[8];
+        unsigned long long stat[2];
         NEP_CUDA(cudaMemcpyAsync(fl, nep->flags, sizeof(fl), cudaMemcpyDeviceToHost, st));
+        NEP_CUDA(cudaMemcpyAsync(stat, nep->build_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
         NEP_CUDA(cudaStreamSynchronize(st));
         nep->maxA_skin = fl[2];
         nep->maxR_skin = fl[3];
         nep->maxS_skin = fl[4];
+        nep->raggedness = stat[1] > 0 ? (double)stat[0] / (double)stat[1] : 1.0;
         if (fl[5]) return nep_fail(nep, NEP_ERR_INVALID_ARG, "an atom type is outside [0, n_types)");
         if (fl[2] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours inside rc_angular + skin");
         if (fl[4] > (1 << NEP_SLOT_BITS)) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "more than 256 neighbours between rc_angular + skin and rc_radial + skin");
         if (!fl[0] && !fl[1]) break;
         if (attempt == 3) return nep_fail(nep, NEP_ERR_NEIGHBOR_OVERFLOW, "neighbour lists kept overflowing");
+        // grow with a margin of a quarter: a re-allocation frees and allocates gigabytes and drains the device, so a
+        // structure whose longest list keeps creeping up (a melt, a cluster) must not trigger one every few builds
         int capA = nep->capA, capS = nep->capS;
-        if (fl[0]) capA = fl[2] + 8 > 256 ? 256 : fl[2] + 8;
-        if (fl[1]) capS = fl[4] + 8 > 256 ? 256 : fl[4] + 8;
+        if (fl[0]) capA = fl[2] + fl[2] / 4 + 8 > 256 ? 256 : fl[2] + fl[2] / 4 + 8;
+        if (fl[1]) capS = fl[4] + fl[4] / 4 + 8 > 256 ? 256 : fl[4] + fl[4] / 4 + 8;
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
+    NEP_CUDA(cudaMemcpyAsync(nep->posq_build, nep->posq, sizeof(int4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
     {
         const int row = nep->capA + nep->capS;
         NEP_LAUNCH(NEP_K_BUILD_REV, k_transpose_list<<<dim3(div_up(n, 32), div_up(nep->capA, 64)), 256, 0, st>>>(n, nep->capA, row, 0, nep->listA, nep->listT));
@@ -599,6 +605,7 @@ int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
         nc *= 4 * (int64_t)nep->ntile[a];
     }
     nep->n_cells = nc;
+    nep->raggedness = 1.0;
     if (!same_n || n > nep->atom_cap) {
         nep->n = n;
         nep->d.n = (int)n;
@@ -755,6 +762,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
     nep->smem_budget = 180 * 1024;
     nep->ann_fp32 = getenv("NEP_ANN_FP32") != nullptr;                // tests / comparison: the fp32-FMA network kernel
     nep->force_smem_radial = getenv("NEP_RADIAL_SMEM") != nullptr;    // tests: exercise the shared-memory variants
+    nep->raggedness = 1.0;
     if (const char* e = getenv("NEP_SMEM_KB")) { const int v = atoi(e); if (v >= 8 && v <= 227) nep->smem_budget = (size_t)v * 1024; }
     if (const char* e = getenv("NEP_NCH_MAX")) { const int v = atoi(e); if (v >= 1 && v <= NEP_NCH_MAX) { nep->nch_max = v; nch_forced = true; } }
     {   // angular passes: at most nch_max channels each, tables staged in shared memory; if a table would
@@ -790,6 +798,7 @@ int nep_create(nep_t** out, const nep_hyper_t* h, const float* c_radial, const f
         if (rc != NEP_OK) { nep_destroy(nep); return rc; }
     }
     rc = dev_alloc(nep, &nep->flags, 8);
+    if (rc == NEP_OK) rc = dev_alloc(nep, &nep->build_stat, 2);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->tile_ctr, 64);
     if (rc == NEP_OK) rc = dev_alloc(nep, &nep->disp_max, 2);
     if (rc != NEP_OK) { nep_destroy(nep); return rc; }
@@ -1016,6 +1025,14 @@ int nep_max_displacement(nep_t* nep, double* disp_host)
     float r2;
     memcpy(&r2, &bits, sizeof(r2));
     *disp_host = sqrt((double)r2);
+    return NEP_OK;
+}
+
+int nep_list_raggedness(nep_t* nep, double* raggedness_host)
+{
+    if (!nep || !raggedness_host) return NEP_ERR_INVALID_ARG;
+    if (!nep->have_lists) return nep_fail(nep, NEP_ERR_STATE, "nep_neighbors has not been called");
+    *raggedness_host = nep->raggedness;
     return NEP_OK;
 }
 

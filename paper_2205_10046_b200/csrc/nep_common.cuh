@@ -70,6 +70,7 @@ struct nep_ctx {
     int nch_max;            // angular n-values per pass (<= NEP_NCH_MAX)
     size_t smem_budget;     // shared memory per SM that the table-in-smem kernels may carve out of L1
     bool ann_fp32;          // NEP_ANN_FP32 set: the fp32-FMA network kernel instead of the tensor-core one
+    double raggedness;      // of the last build: sum over warps of 32 x longest list / sum of list lengths
     bool force_smem_radial; // NEP_RADIAL_SMEM set: use the shared-memory radial kernels even where a register variant exists
     float* w0p;      // [H][DP] rows padded with zeros to DP
     float* b0;       // [H]
@@ -97,6 +98,7 @@ struct nep_ctx {
     // per-atom (device); "sorted" = internal spatial order, "orig" = caller's order
     int* type_orig;          // [n]
     int* perm;               // [n] sorted -> orig
+    unsigned long long* build_stat;   // [2] device: raggedness sums of k_build_lists
     int4* posq;              // [n] sorted: quantised x,y,z (units of L/2^32) + type
     int4* posq_build;        // [n] copy at the last build (displacement check)
     unsigned* cell_of;       // [n] orig: cell id        (build scratch)

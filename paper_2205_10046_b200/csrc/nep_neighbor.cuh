@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(128)
 k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restrict__ perm,
               const int4* __restrict__ posq, const unsigned* __restrict__ cell_start,
               int* __restrict__ listA, int* __restrict__ cntA, int* __restrict__ listS, int* __restrict__ cntS,
-              int* __restrict__ flags)
+              int* __restrict__ flags, unsigned long long* __restrict__ stat)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
@@ -267,6 +267,15 @@ k_build_lists(BuildParams P, const double* __restrict__ pos, const int* __restri
     atomicMax(&flags[2], na);
     atomicMax(&flags[3], na + ns);
     atomicMax(&flags[4], ns);
+    {   // how ragged the lists of a warp's 32 atoms are: every pair loop of a warp runs to its longest list, so
+        // sum over warps of 32 x (longest) / sum of all lengths is the factor lost to idle lanes (nep_list_raggedness)
+        const unsigned am = __activemask();
+        const unsigned wmax = __reduce_max_sync(am, (unsigned)(na + ns)), wsum = __reduce_add_sync(am, (unsigned)(na + ns));
+        if ((threadIdx.x & 31) == (unsigned)(__ffs(am) - 1)) {
+            atomicAdd(&stat[0], (unsigned long long)wmax * (unsigned)__popc(am));
+            atomicAdd(&stat[1], (unsigned long long)wsum);
+        }
+    }
 }
 
 // ---- 4b. atom-major copy of a list: out[atom][base + slot] = in[slot][atom] (tiled transpose) -----------
