@@ -552,8 +552,13 @@ int evaluate(nep_t* nep, const double* pos_dev, bool reuse_geometry = false)
     if (!reuse_geometry) {   // else: same positions as the previous evaluation (another member of a population)
         NEP_LAUNCH(NEP_K_QUANTIZE, k_quantize<<<div_up(n, 256), 256, 0, st>>>(n, pos_dev, nep->type_orig, nep->perm, inv, nep->posq));
         NEP_CUDA(cudaMemsetAsync(nep->disp_max, 0, sizeof(unsigned), st));   // [0] only: [1] runs since the build
-        NEP_LAUNCH(NEP_K_FILTER, k_filter<<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
-                                                 nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
+        if (n <= (1 << 22)) {
+            NEP_LAUNCH(NEP_K_FILTER, k_filter<true><<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
+                                                           nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
+        } else {
+            NEP_LAUNCH(NEP_K_FILTER, k_filter<false><<<div_up(n, 256), 256, 0, st>>>(d, nep->posq, nep->posq_build, nep->listA, nep->cntA, nep->rev, nep->listS, nep->cntS,
+                                                            nep->revS, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->mask, nep->disp_max));
+        }
     }
     NEP_TRY(dispatch_radial(nep));
     NEP_TRY(dispatch_angular(nep, C, false));

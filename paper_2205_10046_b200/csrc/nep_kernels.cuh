@@ -122,6 +122,7 @@ struct PairWalk {
 //   pair W + w:   .x bit m: slot 64 w + m of listS is inside rcR;  .y: number of outer-shell bits of listA
 // The slot of i in j's COMPACT column -- where i delivers dU_i/dr_ij to j -- is the number of set bits
 // below rs in the matching mask of j (PairWalk::slot), so no per-step reverse list is built.
+template <bool PIPE>
 __global__ void __launch_bounds__(256)
 k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq_build,
          const int* __restrict__ listA, const int* __restrict__ cntA, const unsigned char* __restrict__ rev,
@@ -149,31 +150,43 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
     int na = 0, nb = 0;
     const size_t n4 = 4 * n;
     {
-        // the entries of the NEXT batch are requested before the gathers of this one are consumed: a batch then waits for
-        // the longer of the two round trips (list column from DRAM, neighbour positions from L1/L2), not for their sum
+        // PIPE: the entries of the NEXT batch are requested before the gathers of this one are consumed: a batch then
+        // waits for the longer of the two round trips (list column from DRAM, neighbour positions from L1/L2), not for
+        // their sum (303 -> 281 us at 1M atoms).  Not beyond ~4M atoms: there the extra rows in flight, each in a page
+        // of its own 4 n bytes apart, cost more than they hide (8.19M atoms: 3.52 -> 4.31 ms), and the host picks the
+        // plain order, entries of a batch first, then its gathers.
         const int ca = cntA[s];
         const int* lp = listA + s;
         const unsigned char* rp = rev + s;
         int jn[4], rsn[4];
+        if (PIPE) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { const bool ok = u < ca; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
-        lp += n4; rp += n4;
+            for (int u = 0; u < 4; ++u) { const bool ok = u < ca; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
+            lp += n4; rp += n4;
+        }
         for (int w = 0; w < D.maskW; ++w) {
             unsigned long long wa = 0ull, wb = 0ull, bit = 1ull;
             const int mend = min(ca, 64 * (w + 1));
             for (int m0 = 64 * w; m0 < mend; m0 += 4) {          // 4 independent gathers in flight
                 int j[4], rs[4]; int4 pj[4];
+                if (!PIPE) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { const bool ok = m0 + u < ca; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
+                    lp += n4; rp += n4;
+                }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) { j[u] = jn[u]; rs[u] = rsn[u]; }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+                if (PIPE) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const bool ok = m0 + 4 + u < ca;
-                    jn[u] = ok ? lp[u * n] : s;
-                    rsn[u] = ok ? rp[u * n] : 0;
+                    for (int u = 0; u < 4; ++u) {
+                        const bool ok = m0 + 4 + u < ca;
+                        jn[u] = ok ? lp[u * n] : s;
+                        rsn[u] = ok ? rp[u * n] : 0;
+                    }
+                    lp += n4; rp += n4;
                 }
-                lp += n4; rp += n4;
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
@@ -196,25 +209,34 @@ k_filter(NepDims D, const int4* __restrict__ posq, const int4* __restrict__ posq
         const int* lp = listS + s;
         const unsigned char* rp = revS + s;
         int jn[4], rsn[4];
+        if (PIPE) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { const bool ok = u < cs; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
-        lp += n4; rp += n4;
+            for (int u = 0; u < 4; ++u) { const bool ok = u < cs; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
+            lp += n4; rp += n4;
+        }
         for (int w = 0; w < D.maskW; ++w) {
             unsigned long long ws = 0ull, bit = 1ull;
             const int mend = min(cs, 64 * (w + 1));
             for (int m0 = 64 * w; m0 < mend; m0 += 4) {
                 int j[4], rs[4]; int4 pj[4];
+                if (!PIPE) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { const bool ok = m0 + u < cs; jn[u] = ok ? lp[u * n] : s; rsn[u] = ok ? rp[u * n] : 0; }
+                    lp += n4; rp += n4;
+                }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) { j[u] = jn[u]; rs[u] = rsn[u]; }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) pj[u] = posq[j[u]];
+                if (PIPE) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const bool ok = m0 + 4 + u < cs;
-                    jn[u] = ok ? lp[u * n] : s;
-                    rsn[u] = ok ? rp[u * n] : 0;
+                    for (int u = 0; u < 4; ++u) {
+                        const bool ok = m0 + 4 + u < cs;
+                        jn[u] = ok ? lp[u * n] : s;
+                        rsn[u] = ok ? rp[u * n] : 0;
+                    }
+                    lp += n4; rp += n4;
                 }
-                lp += n4; rp += n4;
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     float dx, dy, dz, r2;
