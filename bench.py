@@ -12,8 +12,9 @@ alloy), the configuration north_star's throughput target is quoted on.  Seeded s
 
 Prints ONE JSON line (rank 0).  Keys beyond the base contract:
   roofline     the dominant kernel: algorithmic flops (or bytes) per launch / CUDA-event duration
-  kernels      the same for every kernel that ran in the timed region (events recorded by the library
-               on its own stream, nep_profile_*)
+  kernels      the same for every kernel of a step (events recorded by the library on its own stream,
+               nep_profile_*, over the K steps that directly follow the timed region: the instrumentation itself
+               costs 2.4 % of the step, so the timed region runs without it; --windows times and profiles together)
   cpu_baseline the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
   e2e          the same metric through md_run_host() with pinned HOST buffers: every step uploads
                positions + velocities and downloads positions, velocities, energies and forces
@@ -334,11 +335,12 @@ def run_ours(args):
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.15)
-    nep.nep_profile(True)
     l0 = nep.nep_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     windows = None
+    profiled_ms = None
     if args.windows and args.windows > 1:
+        nep.nep_profile(True)
         # --windows W: the K steps as W consecutive md_step calls, each bracketed by its own event pair and a
         # synchronize; between two windows the pair counts are read back (untimed).  ms = sum of the windows.
         # Shows how ms/step moves with the trajectory (the in-cutoff pair counts grow as the lattice disorders).
@@ -368,6 +370,10 @@ def run_ours(args):
                             "force_angular_ns_per_pair": kus.get("force_angular", 0.0) * 1e3 / max(1, pa),
                             "force_radial_ns_per_pair": kus.get("force_radial", 0.0) * 1e3 / max(1, pr)})
     else:
+        # the timed region runs WITHOUT the library's per-kernel events: an event pair around each of the ~13 launches
+        # of a step costs 2.4 % of the step at 1M atoms (2.61 -> 2.67 ms).  The per-kernel durations behind `roofline`
+        # and `kernels` are taken, still live and with CUDA events on the library's stream, over the K steps that
+        # follow directly (same workload, same cadence; `profiled_ms_per_step` is that pass's own wall time).
         barrier()
         ev0.record()
         nep.md_step(pos, vel, cfg.dt_fs, K, cfg.rebuild_every, cfg.skin)
@@ -376,6 +382,14 @@ def run_ours(args):
         ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
     clocks = sampler.stop()
     launches = nep.nep_launch_count() - l0
+    if windows is None:
+        nep.nep_profile(True)
+        barrier()
+        ev0.record()
+        nep.md_step(pos, vel, cfg.dt_fs, K, cfg.rebuild_every, cfg.skin)
+        ev1.record()
+        barrier()
+        profiled_ms = ev0.elapsed_time(ev1)
     prof = nep.nep_profile_read()
     nep.nep_profile(False)
     pairs_r, pairs_a = nep.nep_pair_counts()
@@ -458,7 +472,10 @@ def run_ours(args):
             "tflops": world * step_flops * K / (ms * 1e-3) / 1e12 / world,
             "alu_frac": step_flops * K / (ms * 1e-3) / 1e12 / alu_peak,
             "hbm_frac": step_bytes * K / (ms * 1e-3) / 1e9 / hbm_peak,
-            "kernel_time_share_of_wall": t_sum / ms if world == 1 else None}
+            "kernel_time_share_of_wall": t_sum / (profiled_ms if profiled_ms else ms) if world == 1 else None,
+            "kernel_timing": ("CUDA-event pair per launch over the K steps after the timed region" if profiled_ms
+                              else "CUDA-event pair per launch inside the timed windows"),
+            "profiled_ms_per_step": profiled_ms / K if profiled_ms else None}
 
     nb_ids = ("cell_hist", "scan", "scatter", "sort_cells", "build_lists", "build_rev")
     nb_ms = sum(prof[k][0] for k in nb_ids if k in prof)
