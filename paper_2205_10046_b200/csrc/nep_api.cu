@@ -124,7 +124,15 @@ int alloc_lists(nep_t* nep, int capA, int capS)
     NEP_TRY(dev_alloc(nep, &nep->pf, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->mA, (size_t)capA * n));
     NEP_TRY(dev_alloc(nep, &nep->listS, (size_t)capS * n));
-    NEP_TRY(dev_alloc(nep, &nep->listT, (size_t)(capA + capS) * n));
+    // the atom-major copy lives only during a build, when the per-step delivery buffers are free: it takes pf's storage
+    // (16 capA n bytes) whenever 4 (capA + capS) n bytes fit there, which saves 0.35 GB at 1M atoms and 3.6 GB at 8.19M
+    if ((size_t)(capA + capS) <= 4 * (size_t)capA) {
+        if (nep->listT_own) { disown(nep, nep->listT_own); cudaFree(nep->listT_own); nep->listT_own = nullptr; }
+        nep->listT = reinterpret_cast<int*>(nep->pf);
+    } else {
+        NEP_TRY(dev_alloc(nep, &nep->listT_own, (size_t)(capA + capS) * n));
+        nep->listT = nep->listT_own;
+    }
     NEP_TRY(dev_alloc(nep, &nep->revS, (size_t)capS * n));
     NEP_TRY(dev_alloc(nep, &nep->mB, (size_t)(capA + capS) * n));
     NEP_TRY(dev_alloc(nep, &nep->cB, (size_t)(capA + capS) * n));

@@ -112,7 +112,8 @@ struct nep_ctx {
     int capA, capS;          // allocated rows
     int* listA;  int* cntA;  // [capA][n] sorted indices with |r| < rcA + skin
     int* listS;  int* cntS;  // [capS][n] rcA + skin <= |r| < rcR + skin
-    int* listT;              // [n][capA+capS] atom-major copy of both lists (reverse-index search)
+    int* listT;              // [n][capA+capS] atom-major copy of both lists (reverse-index search): build scratch, in pf's storage if it fits
+    int* listT_own;          // ... its own allocation otherwise
     unsigned char* rev;      // [capA][n] slot of i in j's listA
     unsigned char* revS;     // [capS][n] slot of i in j's listS
     int* cA; int* ncA;       // [capA][n] per step: packed (j<<8)|(slot of i in j's skin list) with |r| < rcA
