@@ -551,6 +551,11 @@ def run_batch(args):
     for _ in range(max(3, args.warmup)):
         loss = generation()
     torch.cuda.synchronize()
+    nep.nep_profile(True)                                   # per-kernel times of one extra, untimed generation
+    generation()
+    prof = nep.nep_profile_read()
+    nep.nep_profile(False)
+    entries = int(nep.nep_batch_entries()) if hasattr(nep, "nep_batch_entries") else None
     l0 = nep.nep_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
@@ -582,7 +587,8 @@ def run_batch(args):
                        "atoms_per_structure": [int(np.diff(off).min()), int(np.diff(off).max())],
                        "neighbour_entries_per_atom": None,
                        "step": "host parameters -> nep_batch_compute (E, F, W of every member) -> nep_batch_loss -> host [n_pop][3]"},
-            "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours"}
+            "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours",
+            "kernels": [{"name": k, "launches": v[1], "avg_us": v[0] / v[1] * 1e3} for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])]}
     print(json.dumps(line), flush=True)
     nep.close()
     return 0

@@ -1213,6 +1213,7 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
     NEP_TRY(dev_alloc(nep, &b.Hinv, 9 * (size_t)n_str));
     NEP_TRY(dev_alloc(nep, &b.type, (size_t)N));
     NEP_TRY(dev_alloc(nep, &b.cnt, (size_t)N));
+    NEP_TRY(dev_alloc(nep, &b.cntA, (size_t)N));
     if (!b.bad) NEP_TRY(dev_alloc(nep, &b.bad, 1));
     cudaStream_t st = nep->stream;
     NEP_CUDA(cudaMemcpyAsync(b.off, atom_offset_host, sizeof(int) * ((size_t)n_str + 1), cudaMemcpyHostToDevice, st));
@@ -1223,8 +1224,8 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
     NEP_CUDA(cudaMemcpyAsync(b.type, type_dev, sizeof(int) * (size_t)N, cudaMemcpyDeviceToDevice, st));
     NEP_CUDA(cudaMemsetAsync(b.bad, 0, sizeof(int), st));
     // count, size the storage from the longest list, fill, reverse slots
-    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, 0, 0,
-                                                                          b.cnt, nullptr, nullptr, nullptr, b.bad));
+    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, nep->d.rcA, 0, 0,
+                                                                          b.cnt, b.cntA, nullptr, nullptr, nullptr, b.bad));
     std::vector<int> cnt((size_t)N);
     int bad = 0;
     NEP_CUDA(cudaMemcpyAsync(cnt.data(), b.cnt, sizeof(int) * (size_t)N, cudaMemcpyDeviceToHost, st));
@@ -1238,8 +1239,8 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
     NEP_TRY(dev_alloc(nep, &b.d, (size_t)N * cap));
     NEP_TRY(dev_alloc(nep, &b.code, (size_t)N * cap));
     NEP_TRY(dev_alloc(nep, &b.rev, (size_t)N * cap));
-    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, 1, cap,
-                                                                          b.cnt, b.nbr, b.d, b.code, b.bad));
+    NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, nep->d.rcA, 1, cap,
+                                                                          b.cnt, b.cntA, b.nbr, b.d, b.code, b.bad));
     NEP_LAUNCH(NEP_K_BATCH, kb_reverse<<<div_up(N, 128), 128, 0, st>>>(N, cap, b.cnt, b.nbr, b.code, b.rev, b.bad));
     NEP_CUDA(cudaMemcpyAsync(&bad, b.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
     NEP_CUDA(cudaStreamSynchronize(st));
@@ -1291,10 +1292,10 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
         BatchParams P = {b.par[0] + p0 * per[0], b.par[1] + p0 * per[1], b.par[2] + p0 * per[2], b.par[3] + p0 * per[3],
                          b.par[4] + p0 * per[4], b.par[5] + p0 * per[5]};
         const dim3 grid(div_up(b.N, 128), np);
-        NEP_LAUNCH(NEP_K_BATCH, kb_descriptors<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.fp, b.cf, energy_dev + p0 * N));
+        NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.fp, b.cf, energy_dev + p0 * N, b.cntA));
         if (force_dev || virial_dev) {
-            NEP_LAUNCH(NEP_K_BATCH, kb_partial<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf));
-            NEP_LAUNCH(NEP_K_BATCH, kb_gather<<<grid, 128, 0, st>>>(b.N, b.cap, b.cnt, b.nbr, b.d, b.rev, b.pf, force_dev ? force_dev + 3 * p0 * N : nullptr,
+            NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA));
+            NEP_LAUNCH(NEP_K_BATCH_GATHER, kb_gather<<<grid, 128, 0, st>>>(b.N, b.cap, b.cnt, b.nbr, b.d, b.rev, b.pf, force_dev ? force_dev + 3 * p0 * N : nullptr,
                                                                     virial_dev ? virial_dev + 9 * p0 * N : nullptr));
         }
     }
@@ -1320,10 +1321,10 @@ int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const do
     for (int p0 = 0; p0 < n_pop; p0 += 65535) {
         const int np = n_pop - p0 < 65535 ? n_pop - p0 : 65535;
         const size_t o = (size_t)p0 * b.N;
-        NEP_LAUNCH(NEP_K_BATCH, kb_loss_partial<<<dim3(b.n_str, np), 128, 0, nep->stream>>>(b.N, b.n_str, b.off, energy_dev + o, force_dev + 3 * o, virial_dev + 9 * o,
+        NEP_LAUNCH(NEP_K_BATCH_LOSS, kb_loss_partial<<<dim3(b.n_str, np), 128, 0, nep->stream>>>(b.N, b.n_str, b.off, energy_dev + o, force_dev + 3 * o, virial_dev + 9 * o,
                                                                                           u_target_dev, f_target_dev, w_target_dev, b.loss_part + 3 * (size_t)p0 * b.n_str));
     }
-    NEP_LAUNCH(NEP_K_BATCH, kb_loss_total<<<n_pop, 128, 0, nep->stream>>>(b.N, b.n_str, b.loss_part, loss_dev));
+    NEP_LAUNCH(NEP_K_BATCH_LOSS, kb_loss_total<<<n_pop, 128, 0, nep->stream>>>(b.N, b.n_str, b.loss_part, loss_dev));
     return NEP_OK;
 }
 
@@ -1411,7 +1412,8 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 // ---- measurement support ----------------------------------------------------------------------------------
 static const char* const kKernelNames[NEP_K_COUNT] = {
     "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
-    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export", "batch"};
+    "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export", "batch_neighbors",
+    "batch_descriptors", "batch_partial", "batch_gather", "batch_loss"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
 

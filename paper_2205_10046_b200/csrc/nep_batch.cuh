@@ -36,8 +36,8 @@ struct BatchParams {               // device pointers to the parameters of ALL m
 __global__ void __launch_bounds__(128)
 kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, const double* __restrict__ Hs,
              const double* __restrict__ Hinvs, const int* __restrict__ Ms, const double* __restrict__ pos,
-             const int* __restrict__ type, int n_types, double rcR,
-             int fill, int cap, int* __restrict__ cnt, int* __restrict__ nbr, float4* __restrict__ dvec,
+             const int* __restrict__ type, int n_types, double rcR, float rcA,
+             int fill, int cap, int* __restrict__ cnt, int* __restrict__ cntA, int* __restrict__ nbr, float4* __restrict__ dvec,
              unsigned short* __restrict__ code, int* __restrict__ bad)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -49,7 +49,9 @@ kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, co
     const int Ma = Ms[3 * s], Mb = Ms[3 * s + 1], Mc = Ms[3 * s + 2];
     const double rc2 = rcR * rcR;
     const double xi = pos[3 * (size_t)i], yi = pos[3 * (size_t)i + 1], zi = pos[3 * (size_t)i + 2];
-    int c = 0;
+    // entries inside the angular cutoff (the fp32 test the kernels apply: r < rcA) are stored first, so that the angular
+    // loops of a warp run over the angular entries only instead of skipping the others in place (no divergence)
+    int c = 0, ca = 0, cb = fill ? cntA[i] : 0;
     for (int j = off[s]; j < off[s + 1]; ++j) {
         const double tx = __dsub_rn(pos[3 * (size_t)j], xi), ty = __dsub_rn(pos[3 * (size_t)j + 1], yi), tz = __dsub_rn(pos[3 * (size_t)j + 2], zi);
         double n0[3];
@@ -68,8 +70,11 @@ kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, co
                         d[a] = __dsub_rn(__dsub_rn(__dsub_rn(t[a], __dmul_rn(Na, H[a])), __dmul_rn(Nb, H[3 + a])), __dmul_rn(Nc, H[6 + a]));
                     const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
                     if (d2 < rc2) {
-                        if (fill && c < cap) {
-                            const size_t e = (size_t)i * cap + c;
+                        const bool ang = (float)sqrt(d2) < rcA;
+                        const int slot = ang ? ca : cb;
+                        if (ang) ++ca; else ++cb;
+                        if (fill && slot < cap) {
+                            const size_t e = (size_t)i * cap + slot;
                             nbr[e] = j;
                             dvec[e] = make_float4((float)d[0], (float)d[1], (float)d[2], (float)sqrt(d2));
                             code[e] = (unsigned short)((ma + 8) | ((mb + 8) << 4) | ((mc + 8) << 8));
@@ -79,6 +84,7 @@ kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, co
                 }
     }
     cnt[i] = c;
+    if (!fill) cntA[i] = ca;
 }
 
 // slot of the reverse entry (j -> i, -N): same atoms, opposite shift relative to the (odd-symmetric) minimum image
@@ -124,7 +130,7 @@ __global__ void __launch_bounds__(128)
 kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
                const int* __restrict__ nbr, const float4* __restrict__ dvec,
                float* __restrict__ qbuf, float* __restrict__ Sbuf, float* __restrict__ fpbuf, float* __restrict__ cfbuf,
-               double* __restrict__ energy)
+               double* __restrict__ energy, const int* __restrict__ cntA)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int p = blockIdx.y;
@@ -135,7 +141,7 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
     const float* cA = P.cA + (size_t)p * T * T * D.NA * D.KA;
     float* q = qbuf + row * D.D;
     float* S = Sbuf + row * D.NA * NEP_NUM_S;
-    const int c = cnt[i];
+    const int c = cnt[i], ca = cntA[i];
     // Eq. (2)-(3): q_n = sum_j sum_k c_nk f_k(r_ij)
     for (int n0 = 0; n0 < D.NR; n0 += 4) {
         float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
@@ -160,10 +166,9 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
         for (int u = 0; u < 4; ++u)
 #pragma unroll
             for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = 0.0f;
-        for (int m = 0; m < c; ++m) {
+        for (int m = 0; m < ca; ++m) {
             const size_t e = (size_t)i * cap + m;
             const float4 d = dvec[e];
-            if (d.w >= D.rcA) continue;
             const float rinv = 1.0f / d.w;
             const float* cc = cA + ((size_t)(ti * T + type[nbr[e]]) * D.NA + n0) * D.KA;
             float g[4] = {0.0f, 0.0f, 0.0f, 0.0f};
@@ -259,7 +264,7 @@ __device__ __forceinline__ void angular_assemble(const float* A, const float* B,
 __global__ void __launch_bounds__(128)
 kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
            const int* __restrict__ nbr, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
-           const float* __restrict__ fpbuf, float4* __restrict__ pfbuf)
+           const float* __restrict__ fpbuf, float4* __restrict__ pfbuf, const int* __restrict__ cntA)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int p = blockIdx.y;
@@ -271,7 +276,7 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
     const float* fp = fpbuf + row * D.D;
     const float* S = Sbuf + row * D.NA * NEP_NUM_S;
     float4* pf = pfbuf + row * cap;
-    const int c = cnt[i];
+    const int c = cnt[i], ca = cntA[i];
     // first term of Eq. (21): sum_n Fp_n g_n'(r) u
     for (int m = 0; m < c; ++m) {
         const size_t e = (size_t)i * cap + m;
@@ -307,10 +312,9 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
                 for (int k = 0; k < NEP_NUM_S; ++k) G[u][k] = 0.0f;
             }
         }
-        for (int m = 0; m < c; ++m) {
+        for (int m = 0; m < ca; ++m) {
             const size_t e = (size_t)i * cap + m;
             const float4 d = dvec[e];
-            if (d.w >= D.rcA) continue;
             const float rinv = 1.0f / d.w;
             const int tp = ti * T + type[nbr[e]];
             float g[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dg[4] = {0.0f, 0.0f, 0.0f, 0.0f};

@@ -19,7 +19,8 @@
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
     NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FORCE_RADIAL, NEP_K_FINAL,
-    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_BATCH, NEP_K_COUNT
+    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_BATCH, NEP_K_BATCH_DESC, NEP_K_BATCH_PARTIAL,
+    NEP_K_BATCH_GATHER, NEP_K_BATCH_LOSS, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
 
@@ -156,7 +157,7 @@ struct nep_ctx {
         int* off; int* sid; int* M;        // [n_str+1] atom offsets, [N] structure of an atom, [n_str][3] image reach
         double* H; double* Hinv;           // [n_str][9]
         int* type;                         // [N]
-        int* cnt; int* nbr;                // [N], [N][cap]
+        int* cnt; int* cntA; int* nbr;     // [N] entries, [N] of which inside rc_angular (stored first), [N][cap]
         float4* d;                         // [N][cap] pair vector + distance
         unsigned short* code; unsigned short* rev;   // [N][cap] image-shift code, slot of the reverse entry
         int* bad;                          // [1] device flag
