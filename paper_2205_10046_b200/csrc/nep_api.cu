@@ -638,6 +638,30 @@ int setup_system(nep_t* nep, int64_t n, const double box[9], double skin)
 }
 
 template <int DP>
+int launch_batch_ann2(nep_t* nep, dim3 grid, const BatchParams& P, double* energy_dev)
+{
+    const NepDims& d = nep->d;
+    const size_t sm = sizeof(float) * ((size_t)d.H * DP + 2 * d.H + (size_t)d.H * 128);
+    NEP_TRY(allow_smem(nep, kb_ann<DP>, sm));
+    NEP_LAUNCH(NEP_K_BATCH_ANN, kb_ann<DP><<<grid, 128, sm, nep->stream>>>(d, nep->b.N, P, nep->b.q, nep->b.fp, energy_dev));
+    return NEP_OK;
+}
+
+int launch_batch_ann(nep_t* nep, dim3 grid, const BatchParams& P, double* energy_dev)
+{
+    switch (nep->DP) {
+        case 24: return launch_batch_ann2<24>(nep, grid, P, energy_dev);
+        case 40: return launch_batch_ann2<40>(nep, grid, P, energy_dev);
+        case 56: return launch_batch_ann2<56>(nep, grid, P, energy_dev);
+        case 72: return launch_batch_ann2<72>(nep, grid, P, energy_dev);
+        case 88: return launch_batch_ann2<88>(nep, grid, P, energy_dev);
+        case 104: return launch_batch_ann2<104>(nep, grid, P, energy_dev);
+        case 120: return launch_batch_ann2<120>(nep, grid, P, energy_dev);
+    }
+    return nep_fail(nep, NEP_ERR_INVALID_ARG, "descriptor too long");
+}
+
+template <int DP>
 int launch_latent(nep_t* nep, float* latent_dev)
 {
     const NepDims& d = nep->d;
@@ -1273,7 +1297,7 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
         NEP_CUDA(cudaMemcpyAsync(b.par[a], src[a], sizeof(float) * per[a] * n_pop, cudaMemcpyHostToDevice, st));
     }
     // scratch per (member, atom); members in chunks of at most ~4 GB
-    const size_t row_bytes = sizeof(float) * (2 * (size_t)d.D + (size_t)d.NA * NEP_NUM_S + d.H) + sizeof(float4) * b.cap;
+    const size_t row_bytes = sizeof(float) * (2 * (size_t)d.D + (size_t)d.NA * NEP_NUM_S) + sizeof(float4) * b.cap;
     size_t mchunk = (size_t)4e9 / (row_bytes * N);
     if (mchunk < 1) mchunk = 1;
     if (mchunk > (size_t)n_pop) mchunk = (size_t)n_pop;
@@ -1283,7 +1307,6 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
         NEP_TRY(dev_alloc(nep, &b.q, mchunk * N * d.D));
         NEP_TRY(dev_alloc(nep, &b.fp, mchunk * N * d.D));
         NEP_TRY(dev_alloc(nep, &b.S, mchunk * N * d.NA * NEP_NUM_S));
-        NEP_TRY(dev_alloc(nep, &b.cf, mchunk * N * d.H));
         NEP_TRY(dev_alloc(nep, &b.pf, mchunk * N * b.cap));
         b.scratch_rows = mchunk * N;
     }
@@ -1292,9 +1315,22 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
         BatchParams P = {b.par[0] + p0 * per[0], b.par[1] + p0 * per[1], b.par[2] + p0 * per[2], b.par[3] + p0 * per[3],
                          b.par[4] + p0 * per[4], b.par[5] + p0 * per[5]};
         const dim3 grid(div_up(b.N, 128), np);
-        NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.fp, b.cf, energy_dev + p0 * N, b.cntA));
+        // angular channels per pass: all of them for five to seven channels (one pass), else four at a time
+#define NEP_KB_LAUNCH(NCHB)                                                                                     \
+        do {                                                                                                    \
+            NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<NCHB><<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.cntA)); \
+            NEP_TRY(launch_batch_ann(nep, grid, P, energy_dev + p0 * N));                                       \
+            if (force_dev || virial_dev)                                                                        \
+                NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<NCHB><<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA)); \
+        } while (0)
+        switch (d.NA) {
+            case 5: NEP_KB_LAUNCH(5); break;
+            case 6: NEP_KB_LAUNCH(6); break;
+            case 7: NEP_KB_LAUNCH(7); break;
+            default: NEP_KB_LAUNCH(4); break;
+        }
+#undef NEP_KB_LAUNCH
         if (force_dev || virial_dev) {
-            NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA));
             NEP_LAUNCH(NEP_K_BATCH_GATHER, kb_gather<<<grid, 128, 0, st>>>(b.N, b.cap, b.cnt, b.nbr, b.d, b.rev, b.pf, force_dev ? force_dev + 3 * p0 * N : nullptr,
                                                                     virial_dev ? virial_dev + 9 * p0 * N : nullptr));
         }
@@ -1413,7 +1449,7 @@ int md_run_host(nep_t* nep, int64_t n, double* pos_host, double* vel_host, const
 static const char* const kKernelNames[NEP_K_COUNT] = {
     "cell_hist", "scan", "scatter", "sort_cells", "quantize", "build_lists", "build_rev", "filter", "radial",
     "angular", "ann", "force_angular", "force_radial", "final", "kick_drift", "kick", "thermostat", "export", "batch_neighbors",
-    "batch_descriptors", "batch_partial", "batch_gather", "batch_loss"};
+    "batch_descriptors", "batch_ann", "batch_partial", "batch_gather", "batch_loss"};
 
 int nep_profile_num_kernels(void) { return NEP_K_COUNT; }
 

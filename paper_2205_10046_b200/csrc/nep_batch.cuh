@@ -23,6 +23,10 @@
 
 #define NEP_BATCH_MAX_SHIFT 7      // |image shift relative to the minimum image| per axis that fits the reverse-entry code
 
+#ifndef NEP_KB_RG
+#define NEP_KB_RG 4                // radial n per group in kb_descriptors
+#endif
+
 struct BatchParams {               // device pointers to the parameters of ALL members, member-major
     const float* cR;               // [n_pop][T][T][NR][KR]
     const float* cA;               // [n_pop][T][T][NA][KA]
@@ -126,11 +130,11 @@ struct ChebWalk {
 
 // ---- descriptors + network: q, S, Fp, U of one (atom, member) --------------------------------------------------
 // scratch per (member, atom): q [D] (also the network input), S [NA][24], fp [D]; row-major, one row per thread
+template <int NCHB>
 __global__ void __launch_bounds__(128)
 kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
                const int* __restrict__ nbr, const float4* __restrict__ dvec,
-               float* __restrict__ qbuf, float* __restrict__ Sbuf, float* __restrict__ fpbuf, float* __restrict__ cfbuf,
-               double* __restrict__ energy, const int* __restrict__ cntA)
+               float* __restrict__ qbuf, float* __restrict__ Sbuf, const int* __restrict__ cntA)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int p = blockIdx.y;
@@ -142,9 +146,9 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
     float* q = qbuf + row * D.D;
     float* S = Sbuf + row * D.NA * NEP_NUM_S;
     const int c = cnt[i], ca = cntA[i];
-    // Eq. (2)-(3): q_n = sum_j sum_k c_nk f_k(r_ij)
-    for (int n0 = 0; n0 < D.NR; n0 += 4) {
-        float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    // Eq. (2)-(3): q_n = sum_j sum_k c_nk f_k(r_ij); eight n at a time, one Chebyshev walk per pair and group
+    for (int n0 = 0; n0 < D.NR; n0 += NEP_KB_RG) {
+        float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
         for (int m = 0; m < c; ++m) {
             const size_t e = (size_t)i * cap + m;
             const float r = dvec[e].w;
@@ -153,17 +157,18 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
             for (int k = 0; k < D.KR; ++k) {
                 float f, df; w.get(f, df);
 #pragma unroll
-                for (int u = 0; u < 4; ++u) if (n0 + u < D.NR) acc[u] = fmaf(__ldg(cc + u * D.KR + k), f, acc[u]);
+                for (int u = 0; u < NEP_KB_RG; ++u) if (n0 + u < D.NR) acc[u] = fmaf(__ldg(cc + u * D.KR + k), f, acc[u]);
                 w.step();
             }
         }
-        for (int u = 0; u < 4; ++u) if (n0 + u < D.NR) q[n0 + u] = acc[u];
-    }
-    // Eq. (12) and Eqs. (13)-(19), four channels at a time
-    for (int n0 = 0; n0 < D.NA; n0 += 4) {
-        float Sa[4][NEP_NUM_S];
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int u = 0; u < NEP_KB_RG; ++u) if (n0 + u < D.NR) q[n0 + u] = acc[u];
+    }
+    // Eq. (12) and Eqs. (13)-(19), NCHB channels at a time (NCHB = N_A for 5..7 channels: one pass)
+    for (int n0 = 0; n0 < D.NA; n0 += NCHB) {
+        float Sa[NCHB][NEP_NUM_S];
+#pragma unroll
+        for (int u = 0; u < NCHB; ++u)
 #pragma unroll
             for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = 0.0f;
         for (int m = 0; m < ca; ++m) {
@@ -171,23 +176,25 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
             const float4 d = dvec[e];
             const float rinv = 1.0f / d.w;
             const float* cc = cA + ((size_t)(ti * T + type[nbr[e]]) * D.NA + n0) * D.KA;
-            float g[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            float g[NCHB];
+#pragma unroll
+            for (int u = 0; u < NCHB; ++u) g[u] = 0.0f;
             ChebWalk w(d.w, D.rcA_inv);
             for (int k = 0; k < D.KA; ++k) {
                 float f, df; w.get(f, df);
 #pragma unroll
-                for (int u = 0; u < 4; ++u) if (n0 + u < D.NA) g[u] = fmaf(__ldg(cc + u * D.KA + k), f, g[u]);
+                for (int u = 0; u < NCHB; ++u) if (n0 + u < D.NA) g[u] = fmaf(__ldg(cc + u * D.KA + k), f, g[u]);
                 w.step();
             }
             float b[NEP_NUM_S];
             angular_b(d.x * rinv, d.y * rinv, d.z * rinv, b);
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < NCHB; ++u)
 #pragma unroll
                 for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = fmaf(g[u], b[k], Sa[u][k]);
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < NCHB; ++u) {
             const int nn = n0 + u;
             if (nn < D.NA) {
                 float out[6];
@@ -200,38 +207,85 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
             }
         }
     }
-    // Eq. (1) / Listing 1: U and Fp = dU/dq
+}
+
+// ---- network of one (atom, member): U and Fp = dU/dq, Eq. (1) / Listing 1 -----------------------------------------
+// The member's weights are staged once per block in shared memory (rows padded to DP, warp-uniform reads), q sits in
+// registers, cf_m = w1_m (1 - tanh^2) in this thread's shared-memory column; as k_ann of the MD path, with the
+// per-thread rows of the batch scratch ([row][D]) as input and output.
+template <int DP>
+__global__ void __launch_bounds__(128)
+kb_ann(NepDims D, int N, BatchParams P, const float* __restrict__ qbuf, float* __restrict__ fpbuf, double* __restrict__ energy)
+{
+    extern __shared__ float sw[];                       // w0 [H][DP], b0 [H], w1 [H], cf [H][128]
+    const int p = blockIdx.y;
     const float* w0 = P.w0 + (size_t)p * D.H * D.D;
-    const float* b0 = P.b0 + (size_t)p * D.H;
-    const float* w1 = P.w1 + (size_t)p * D.H;
-    float* cf = cfbuf + row * D.H;
-    float u_i = 0.0f;
-    for (int m = 0; m < D.H; ++m) {
-        float z = -__ldg(b0 + m);
-        for (int v = 0; v < D.D; ++v) z = fmaf(__ldg(w0 + (size_t)m * D.D + v), q[v], z);
-        const float x1 = tanhf(z), w1m = __ldg(w1 + m);
-        u_i = fmaf(w1m, x1, u_i);
-        cf[m] = w1m * (1.0f - x1 * x1);
+    for (int t = threadIdx.x; t < D.H * DP; t += 128) { const int m = t / DP, v = t - m * DP; sw[t] = v < D.D ? w0[(size_t)m * D.D + v] : 0.0f; }
+    float* sb0 = sw + D.H * DP;
+    float* sw1 = sb0 + D.H;
+    float* mycf = sw1 + D.H + threadIdx.x;
+    for (int t = threadIdx.x; t < D.H; t += 128) { sb0[t] = P.b0[(size_t)p * D.H + t]; sw1[t] = P.w1[(size_t)p * D.H + t]; }
+    __syncthreads();
+    const int i = blockIdx.x * 128 + threadIdx.x;
+    if (i >= N) return;
+    const size_t row = (size_t)p * N + i;
+    const float* q = qbuf + row * D.D;
+    float e = 0.0f;
+    {
+        float qv[DP];
+#pragma unroll
+        for (int d = 0; d < DP; ++d) qv[d] = d < D.D ? q[d] : 0.0f;
+        for (int m = 0; m < D.H; ++m) {
+            const float4* w = reinterpret_cast<const float4*>(sw + m * DP);
+            float a0 = -sb0[m], a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+#pragma unroll
+            for (int d4 = 0; d4 < DP / 4; ++d4) {
+                const float4 ww = w[d4];
+                a0 = fmaf(ww.x, qv[4 * d4 + 0], a0); a1 = fmaf(ww.y, qv[4 * d4 + 1], a1);
+                a2 = fmaf(ww.z, qv[4 * d4 + 2], a2); a3 = fmaf(ww.w, qv[4 * d4 + 3], a3);
+            }
+            const float x1 = tanhf((a0 + a1) + (a2 + a3));
+            const float w1m = sw1[m];
+            e = fmaf(w1m, x1, e);
+            mycf[m * 128] = w1m * (1.0f - x1 * x1);
+        }
     }
     float* fp = fpbuf + row * D.D;
-    for (int v = 0; v < D.D; ++v) {
-        float a = 0.0f;
-        for (int m = 0; m < D.H; ++m) a = fmaf(cf[m], __ldg(w0 + (size_t)m * D.D + v), a);
-        fp[v] = a;
+#pragma unroll
+    for (int d0 = 0; d0 < DP; d0 += 8) {
+        float acc[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc[u] = 0.0f;
+        const float4* w = reinterpret_cast<const float4*>(sw + d0);
+        for (int m = 0; m < D.H; ++m) {
+            const float cf = mycf[m * 128];
+            const float4 wa = w[m * (DP / 4)], wb = w[m * (DP / 4) + 1];
+            acc[0] = fmaf(cf, wa.x, acc[0]); acc[1] = fmaf(cf, wa.y, acc[1]);
+            acc[2] = fmaf(cf, wa.z, acc[2]); acc[3] = fmaf(cf, wa.w, acc[3]);
+            acc[4] = fmaf(cf, wb.x, acc[4]); acc[5] = fmaf(cf, wb.y, acc[5]);
+            acc[6] = fmaf(cf, wb.z, acc[6]); acc[7] = fmaf(cf, wb.w, acc[7]);
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) if (d0 + u < D.D) fp[d0 + u] = acc[u];
     }
-    energy[row] = (double)(u_i - __ldg(P.b1 + p));
+    energy[row] = (double)(e - P.b1[p]);
 }
 
 // grad P_k(u) of the 24 polynomials on the unit vector (table of SURVEY.md section 8(c)), and the assembly of Eq. (21):
 //   pf = [sum_k (B_k - l_k A_k / r) b_k] u + (1/r) sum_k A_k grad P_k(u)
-__device__ __forceinline__ void angular_assemble(const float* A, const float* B, float x, float y, float z, float rinv, float* pf)
+// A_k = sum_n G_nk g_n and B_k = sum_n G_nk g_n' are formed where they are used (no A[24], B[24] in registers).
+template <int NCHB>
+__device__ __forceinline__ void angular_assemble(const float (&G)[NCHB][NEP_NUM_S], const float* g, const float* dg,
+                                                 float x, float y, float z, float rinv, float* pf)
 {
     float b[NEP_NUM_S];
     angular_b(x, y, z, b);
     const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z, xyz = xy * z;
     float cu = 0.0f, vx = 0.0f, vy = 0.0f, vz = 0.0f;
 #define KB_USE(k, l, gx, gy, gz)                                                                   \
-    { cu = fmaf(fmaf(-(float)(l) * rinv, A[k], B[k]), b[k], cu); vx = fmaf(A[k], (gx), vx); vy = fmaf(A[k], (gy), vy); vz = fmaf(A[k], (gz), vz); }
+    { float Ak = G[0][k] * g[0], Bk = G[0][k] * dg[0];                                             \
+      _Pragma("unroll") for (int u = 1; u < NCHB; ++u) { Ak = fmaf(G[u][k], g[u], Ak); Bk = fmaf(G[u][k], dg[u], Bk); } \
+      cu = fmaf(fmaf(-(float)(l) * rinv, Ak, Bk), b[k], cu); vx = fmaf(Ak, (gx), vx); vy = fmaf(Ak, (gy), vy); vz = fmaf(Ak, (gz), vz); }
     KB_USE(0, 1, 0.0f, 0.0f, 1.0f)
     KB_USE(1, 1, 1.0f, 0.0f, 0.0f)
     KB_USE(2, 1, 0.0f, 1.0f, 0.0f)
@@ -261,6 +315,7 @@ __device__ __forceinline__ void angular_assemble(const float* A, const float* B,
 }
 
 // ---- partial forces dU_i/dr_ij of every entry, Eq. (21) -----------------------------------------------------------
+template <int NCHB>
 __global__ void __launch_bounds__(128)
 kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
            const int* __restrict__ nbr, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
@@ -277,28 +332,33 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
     const float* S = Sbuf + row * D.NA * NEP_NUM_S;
     float4* pf = pfbuf + row * cap;
     const int c = cnt[i], ca = cntA[i];
-    // first term of Eq. (21): sum_n Fp_n g_n'(r) u
+    // first term of Eq. (21): sum_n Fp_n g_n'(r) u; the first eight Fp_n stay in registers
+    float fpr[8];
+#pragma unroll
+    for (int n = 0; n < 8; ++n) fpr[n] = n < D.NR ? fp[n] : 0.0f;
     for (int m = 0; m < c; ++m) {
         const size_t e = (size_t)i * cap + m;
         const float4 d = dvec[e];
         const float rinv = 1.0f / d.w;
-        const int tp = ti * T + type[nbr[e]];
+        const float* cc = cR + (size_t)(ti * T + type[nbr[e]]) * D.NR * D.KR;
         float s = 0.0f;
         ChebWalk w(d.w, D.rcR_inv);
         for (int k = 0; k < D.KR; ++k) {
             float f, df; w.get(f, df);
             float a = 0.0f;
-            for (int n = 0; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cR + ((size_t)tp * D.NR + n) * D.KR + k), a);
+#pragma unroll
+            for (int n = 0; n < 8; ++n) if (n < D.NR) a = fmaf(fpr[n], __ldg(cc + n * D.KR + k), a);
+            for (int n = 8; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cc + n * D.KR + k), a);
             s = fmaf(a, df, s);
             w.step();
         }
         pf[m] = make_float4(s * d.x * rinv, s * d.y * rinv, s * d.z * rinv, 0.0f);
     }
-    // last three terms, four channels at a time (pf is linear in A_k = sum_n G_nk g_n and B_k = sum_n G_nk g_n')
-    for (int n0 = 0; n0 < D.NA; n0 += 4) {
-        float G[4][NEP_NUM_S];
+    // last three terms, NCHB channels at a time (pf is linear in A_k = sum_n G_nk g_n and B_k = sum_n G_nk g_n')
+    for (int n0 = 0; n0 < D.NA; n0 += NCHB) {
+        float G[NCHB][NEP_NUM_S];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < NCHB; ++u) {
             const int n = min(n0 + u, D.NA - 1);
             float Sv[NEP_NUM_S], f3[4];
 #pragma unroll
@@ -317,12 +377,14 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
             const float4 d = dvec[e];
             const float rinv = 1.0f / d.w;
             const int tp = ti * T + type[nbr[e]];
-            float g[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dg[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            float g[NCHB], dg[NCHB];
+#pragma unroll
+            for (int u = 0; u < NCHB; ++u) { g[u] = 0.0f; dg[u] = 0.0f; }
             ChebWalk w(d.w, D.rcA_inv);
             for (int k = 0; k < D.KA; ++k) {
                 float f, df; w.get(f, df);
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < NCHB; ++u) {
                     if (n0 + u < D.NA) {
                         const float cc = __ldg(cA + ((size_t)tp * D.NA + n0 + u) * D.KA + k);
                         g[u] = fmaf(cc, f, g[u]); dg[u] = fmaf(cc, df, dg[u]);
@@ -330,15 +392,8 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
                 }
                 w.step();
             }
-            float A[NEP_NUM_S], B[NEP_NUM_S];
-#pragma unroll
-            for (int k = 0; k < NEP_NUM_S; ++k) {
-                A[k] = G[0][k] * g[0]; B[k] = G[0][k] * dg[0];
-#pragma unroll
-                for (int u = 1; u < 4; ++u) { A[k] = fmaf(G[u][k], g[u], A[k]); B[k] = fmaf(G[u][k], dg[u], B[k]); }
-            }
             float pa[3];
-            angular_assemble(A, B, d.x * rinv, d.y * rinv, d.z * rinv, rinv, pa);
+            angular_assemble<NCHB>(G, g, dg, d.x * rinv, d.y * rinv, d.z * rinv, rinv, pa);
             float4 o = pf[m];
             o.x += pa[0]; o.y += pa[1]; o.z += pa[2];
             pf[m] = o;

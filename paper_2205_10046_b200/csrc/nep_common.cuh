@@ -19,7 +19,7 @@
 enum NepKernelId {
     NEP_K_CELL_HIST = 0, NEP_K_SCAN, NEP_K_SCATTER, NEP_K_SORT_CELLS, NEP_K_QUANTIZE, NEP_K_BUILD_LISTS,
     NEP_K_BUILD_REV, NEP_K_FILTER, NEP_K_RADIAL, NEP_K_ANGULAR, NEP_K_ANN, NEP_K_FORCE_ANGULAR, NEP_K_FORCE_RADIAL, NEP_K_FINAL,
-    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_BATCH, NEP_K_BATCH_DESC, NEP_K_BATCH_PARTIAL,
+    NEP_K_KICK_DRIFT, NEP_K_KICK, NEP_K_THERMOSTAT, NEP_K_EXPORT, NEP_K_BATCH, NEP_K_BATCH_DESC, NEP_K_BATCH_ANN, NEP_K_BATCH_PARTIAL,
     NEP_K_BATCH_GATHER, NEP_K_BATCH_LOSS, NEP_K_COUNT
 };
 #define NEP_PROF_PAIRS 32768     // event pairs kept before a forced drain
@@ -162,7 +162,7 @@ struct nep_ctx {
         unsigned short* code; unsigned short* rev;   // [N][cap] image-shift code, slot of the reverse entry
         int* bad;                          // [1] device flag
         float* par[6]; size_t par_cap[6];  // parameters of all members of a call
-        float* q; float* S; float* fp; float* cf; float4* pf; size_t scratch_rows;   // per (member, atom) scratch of a chunk
+        float* q; float* S; float* fp; float4* pf; size_t scratch_rows;   // per (member, atom) scratch of a chunk
         double* loss_part; size_t loss_cap;
     } b;
 
