@@ -1318,10 +1318,17 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
         // angular channels per pass: all of them for five to seven channels (one pass), else four at a time
 #define NEP_KB_LAUNCH(NCHB)                                                                                     \
         do {                                                                                                    \
-            NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<NCHB><<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.cntA)); \
+            int bs = 128;                                 /* per-thread sums / E table + the pass's coefficient table */ \
+            auto smem = [&](int b_) { return sizeof(float) * ((size_t)d.T * d.KR * b_ + (size_t)d.T * d.T * d.KA * NCHB); }; \
+            while (bs > 32 && smem(bs) > 100 * 1024) bs >>= 1;                                                   \
+            if (smem(bs) > 200 * 1024) return nep_fail(nep, NEP_ERR_INVALID_ARG, "n_types x basis too large for shared memory"); \
+            const dim3 gridb(div_up(b.N, bs), np);                                                               \
+            NEP_TRY(allow_smem(nep, kb_descriptors<NCHB>, smem(bs)));                                            \
+            NEP_TRY(allow_smem(nep, kb_partial<NCHB>, smem(bs)));                                                \
+            NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.cntA)); \
             NEP_TRY(launch_batch_ann(nep, grid, P, energy_dev + p0 * N));                                       \
             if (force_dev || virial_dev)                                                                        \
-                NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<NCHB><<<grid, 128, 0, st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA)); \
+                NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA)); \
         } while (0)
         switch (d.NA) {
             case 5: NEP_KB_LAUNCH(5); break;

@@ -130,42 +130,67 @@ struct ChebWalk {
 
 // ---- descriptors + network: q, S, Fp, U of one (atom, member) --------------------------------------------------
 // scratch per (member, atom): q [D] (also the network input), S [NA][24], fp [D]; row-major, one row per thread
+// Shared memory of kb_descriptors / kb_partial (dynamic): this thread's column of T x KR per-type sums (resp. its
+// E^i[t][k] table), [t * KR + k][blockDim.x], then the angular coefficients of the current pass, [tp][k][NCHB]
+// (zero beyond N_A) -- the member's coefficients are read from global memory once per block, not once per pair.
+template <int NCHB>
+__device__ __forceinline__ void kb_stage_angular(const NepDims& D, const float* __restrict__ cA, int n0, float* tab)
+{
+    const int TT = D.T * D.T;
+    __syncthreads();                                                     // the previous pass is done with the table
+    for (int t = threadIdx.x; t < TT * D.KA * NCHB; t += blockDim.x) {
+        const int u = t % NCHB, k = (t / NCHB) % D.KA, tp = t / (NCHB * D.KA);
+        tab[t] = (n0 + u < D.NA) ? cA[((size_t)tp * D.NA + n0 + u) * D.KA + k] : 0.0f;
+    }
+    __syncthreads();
+}
+
 template <int NCHB>
 __global__ void __launch_bounds__(128)
 kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
                const int* __restrict__ nbr, const float4* __restrict__ dvec,
                float* __restrict__ qbuf, float* __restrict__ Sbuf, const int* __restrict__ cntA)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    extern __shared__ float sm[];
+    const int BS = blockDim.x, T = D.T;
+    float* my = sm + threadIdx.x;
+    float* tab = sm + (size_t)T * D.KR * BS;
+    const int i0 = blockIdx.x * BS + threadIdx.x;
+    const bool valid = i0 < N;
+    const int i = valid ? i0 : N - 1;                                    // idle threads shadow the last atom, store nothing
     const int p = blockIdx.y;
-    if (i >= N) return;
     const size_t row = (size_t)p * N + i;
-    const int ti = type[i], T = D.T;
+    const int ti = type[i];
     const float* cR = P.cR + (size_t)p * T * T * D.NR * D.KR;
     const float* cA = P.cA + (size_t)p * T * T * D.NA * D.KA;
     float* q = qbuf + row * D.D;
     float* S = Sbuf + row * D.NA * NEP_NUM_S;
     const int c = cnt[i], ca = cntA[i];
-    // Eq. (2)-(3): q_n = sum_j sum_k c_nk f_k(r_ij); eight n at a time, one Chebyshev walk per pair and group
-    for (int n0 = 0; n0 < D.NR; n0 += NEP_KB_RG) {
-        float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
-        for (int m = 0; m < c; ++m) {
-            const size_t e = (size_t)i * cap + m;
-            const float r = dvec[e].w;
-            const float* cc = cR + ((size_t)(ti * T + type[nbr[e]]) * D.NR + n0) * D.KR;
-            ChebWalk w(r, D.rcR_inv);
-            for (int k = 0; k < D.KR; ++k) {
-                float f, df; w.get(f, df);
-#pragma unroll
-                for (int u = 0; u < NEP_KB_RG; ++u) if (n0 + u < D.NR) acc[u] = fmaf(__ldg(cc + u * D.KR + k), f, acc[u]);
-                w.step();
-            }
+    // Eq. (2)-(3) re-associated as in the MD path: q_n = sum_t sum_k c[ti][t][n][k] F_t,k with the per-type basis sums
+    // F_t,k = sum_{j of type t} f_k(r_ij): one Chebyshev walk and KR additions per pair, the contraction once per atom
+    for (int t = 0; t < T * D.KR; ++t) my[t * BS] = 0.0f;
+    for (int m = 0; m < c; ++m) {
+        const size_t e = (size_t)i * cap + m;
+        float* F = my + (size_t)type[nbr[e]] * D.KR * BS;
+        ChebWalk w(dvec[e].w, D.rcR_inv);
+        for (int k = 0; k < D.KR; ++k) {
+            float f, df; w.get(f, df);
+            F[k * BS] += f;
+            w.step();
         }
-#pragma unroll
-        for (int u = 0; u < NEP_KB_RG; ++u) if (n0 + u < D.NR) q[n0 + u] = acc[u];
+    }
+    for (int n = 0; n < D.NR; ++n) {
+        float acc = 0.0f;
+        for (int t = 0; t < T; ++t) {
+            const float* cc = cR + ((size_t)(ti * T + t) * D.NR + n) * D.KR;
+            const float* F = my + (size_t)t * D.KR * BS;
+            for (int k = 0; k < D.KR; ++k) acc = fmaf(__ldg(cc + k), F[k * BS], acc);
+        }
+        if (valid) q[n] = acc;
     }
     // Eq. (12) and Eqs. (13)-(19), NCHB channels at a time (NCHB = N_A for 5..7 channels: one pass)
     for (int n0 = 0; n0 < D.NA; n0 += NCHB) {
+        kb_stage_angular<NCHB>(D, cA, n0, tab);
         float Sa[NCHB][NEP_NUM_S];
 #pragma unroll
         for (int u = 0; u < NCHB; ++u)
@@ -175,7 +200,7 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
             const size_t e = (size_t)i * cap + m;
             const float4 d = dvec[e];
             const float rinv = 1.0f / d.w;
-            const float* cc = cA + ((size_t)(ti * T + type[nbr[e]]) * D.NA + n0) * D.KA;
+            const float* cc = tab + (size_t)(ti * T + type[nbr[e]]) * D.KA * NCHB;
             float g[NCHB];
 #pragma unroll
             for (int u = 0; u < NCHB; ++u) g[u] = 0.0f;
@@ -183,7 +208,8 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
             for (int k = 0; k < D.KA; ++k) {
                 float f, df; w.get(f, df);
 #pragma unroll
-                for (int u = 0; u < NCHB; ++u) if (n0 + u < D.NA) g[u] = fmaf(__ldg(cc + u * D.KA + k), f, g[u]);
+                for (int u = 0; u < NCHB; ++u) g[u] = fmaf(cc[u], f, g[u]);
+                cc += NCHB;
                 w.step();
             }
             float b[NEP_NUM_S];
@@ -196,7 +222,7 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
 #pragma unroll
         for (int u = 0; u < NCHB; ++u) {
             const int nn = n0 + u;
-            if (nn < D.NA) {
+            if (nn < D.NA && valid) {
                 float out[6];
                 q_from_S(Sa[u], C, out);
                 for (int l = 0; l < 4; ++l) q[D.NR + l * D.NA + nn] = out[l];
@@ -321,41 +347,47 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
            const int* __restrict__ nbr, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
            const float* __restrict__ fpbuf, float4* __restrict__ pfbuf, const int* __restrict__ cntA)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    extern __shared__ float sm[];
+    const int BS = blockDim.x, T = D.T;
+    float* my = sm + threadIdx.x;
+    float* tab = sm + (size_t)T * D.KR * BS;
+    const int i0 = blockIdx.x * BS + threadIdx.x;
+    const bool valid = i0 < N;
+    const int i = valid ? i0 : N - 1;
     const int p = blockIdx.y;
-    if (i >= N) return;
     const size_t row = (size_t)p * N + i;
-    const int ti = type[i], T = D.T;
+    const int ti = type[i];
     const float* cR = P.cR + (size_t)p * T * T * D.NR * D.KR;
     const float* cA = P.cA + (size_t)p * T * T * D.NA * D.KA;
     const float* fp = fpbuf + row * D.D;
     const float* S = Sbuf + row * D.NA * NEP_NUM_S;
     float4* pf = pfbuf + row * cap;
     const int c = cnt[i], ca = cntA[i];
-    // first term of Eq. (21): sum_n Fp_n g_n'(r) u; the first eight Fp_n stay in registers
-    float fpr[8];
-#pragma unroll
-    for (int n = 0; n < 8; ++n) fpr[n] = n < D.NR ? fp[n] : 0.0f;
+    // first term of Eq. (21) re-associated as in the MD path: m_ij = sum_k E^i[tj][k] f_k'(r_ij) with
+    // E^i[t][k] = sum_n Fp_n c[ti][t][n][k] formed once per atom (KR FMAs per pair instead of NR x KR)
+    for (int t = 0; t < T; ++t)
+        for (int k = 0; k < D.KR; ++k) {
+            float a = 0.0f;
+            for (int n = 0; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cR + ((size_t)(ti * T + t) * D.NR + n) * D.KR + k), a);
+            my[(t * D.KR + k) * BS] = a;
+        }
     for (int m = 0; m < c; ++m) {
         const size_t e = (size_t)i * cap + m;
         const float4 d = dvec[e];
         const float rinv = 1.0f / d.w;
-        const float* cc = cR + (size_t)(ti * T + type[nbr[e]]) * D.NR * D.KR;
+        const float* E = my + (size_t)type[nbr[e]] * D.KR * BS;
         float s = 0.0f;
         ChebWalk w(d.w, D.rcR_inv);
         for (int k = 0; k < D.KR; ++k) {
             float f, df; w.get(f, df);
-            float a = 0.0f;
-#pragma unroll
-            for (int n = 0; n < 8; ++n) if (n < D.NR) a = fmaf(fpr[n], __ldg(cc + n * D.KR + k), a);
-            for (int n = 8; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cc + n * D.KR + k), a);
-            s = fmaf(a, df, s);
+            s = fmaf(E[k * BS], df, s);
             w.step();
         }
-        pf[m] = make_float4(s * d.x * rinv, s * d.y * rinv, s * d.z * rinv, 0.0f);
+        if (valid) pf[m] = make_float4(s * d.x * rinv, s * d.y * rinv, s * d.z * rinv, 0.0f);
     }
     // last three terms, NCHB channels at a time (pf is linear in A_k = sum_n G_nk g_n and B_k = sum_n G_nk g_n')
     for (int n0 = 0; n0 < D.NA; n0 += NCHB) {
+        kb_stage_angular<NCHB>(D, cA, n0, tab);
         float G[NCHB][NEP_NUM_S];
 #pragma unroll
         for (int u = 0; u < NCHB; ++u) {
@@ -376,7 +408,7 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
             const size_t e = (size_t)i * cap + m;
             const float4 d = dvec[e];
             const float rinv = 1.0f / d.w;
-            const int tp = ti * T + type[nbr[e]];
+            const float* cc = tab + (size_t)(ti * T + type[nbr[e]]) * D.KA * NCHB;
             float g[NCHB], dg[NCHB];
 #pragma unroll
             for (int u = 0; u < NCHB; ++u) { g[u] = 0.0f; dg[u] = 0.0f; }
@@ -384,19 +416,17 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
             for (int k = 0; k < D.KA; ++k) {
                 float f, df; w.get(f, df);
 #pragma unroll
-                for (int u = 0; u < NCHB; ++u) {
-                    if (n0 + u < D.NA) {
-                        const float cc = __ldg(cA + ((size_t)tp * D.NA + n0 + u) * D.KA + k);
-                        g[u] = fmaf(cc, f, g[u]); dg[u] = fmaf(cc, df, dg[u]);
-                    }
-                }
+                for (int u = 0; u < NCHB; ++u) { g[u] = fmaf(cc[u], f, g[u]); dg[u] = fmaf(cc[u], df, dg[u]); }
+                cc += NCHB;
                 w.step();
             }
             float pa[3];
             angular_assemble<NCHB>(G, g, dg, d.x * rinv, d.y * rinv, d.z * rinv, rinv, pa);
-            float4 o = pf[m];
-            o.x += pa[0]; o.y += pa[1]; o.z += pa[2];
-            pf[m] = o;
+            if (valid) {
+                float4 o = pf[m];
+                o.x += pa[0]; o.y += pa[1]; o.z += pa[2];
+                pf[m] = o;
+            }
         }
     }
 }
