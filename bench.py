@@ -555,7 +555,7 @@ def run_batch(args):
     generation()
     prof = nep.nep_profile_read()
     nep.nep_profile(False)
-    entries = int(nep.nep_batch_entries()) if hasattr(nep, "nep_batch_entries") else None
+    ent_r, ent_a = nep.nep_batch_pair_counts()
     l0 = nep.nep_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
@@ -589,6 +589,17 @@ def run_batch(args):
                        "step": "host parameters -> nep_batch_compute (E, F, W of every member) -> nep_batch_loss -> host [n_pop][3]"},
             "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours",
             "kernels": [{"name": k, "launches": v[1], "avg_us": v[0] / v[1] * 1e3} for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])]}
+    # roofline of the dominant kernel (kb_partial: Eq. (21) of every entry and member), algorithmic flops as in
+    # kernel_costs (force_angular + force_radial per ordered pair), against the derived FP32 peak
+    h = cfg.hyper
+    fl = P * (ent_a * (4 * h.NA * h.KA + 4 * 24 * h.NA + 500) + N * 3 * 24 * h.NA + ent_r * (55 + 4 * h.KR + 2 * h.NR * h.KR))
+    if "batch_partial" in prof:
+        us = prof["batch_partial"][0] / prof["batch_partial"][1] * 1e3
+        alu_peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
+        line["roofline"] = {"kernel": "batch_partial", "bound": "alu", "achieved": fl / us / 1e6, "peak": alu_peak, "unit": "TFLOP/s",
+                            "frac": fl / us / 1e6 / alu_peak, "avg_us": us, "traffic": None,
+                            "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    line["config"]["neighbour_entries_per_atom"] = [ent_r / N, ent_a / N]
     print(json.dumps(line), flush=True)
     nep.close()
     return 0

@@ -256,6 +256,10 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
 int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const float* c_angular,
                       const float* w0, const float* b0, const float* w1, const float* b1,
                       double* energy_dev, double* force_dev, double* virial_dev);
+/* Measurement support: ordered neighbour entries of the batch inside rc_radial and inside rc_angular (lattice images
+ * counted), summed over all atoms.  Synchronises.  NEP_ERR_STATE before nep_batch_neighbors.                       */
+int nep_batch_pair_counts(nep_t* nep, int64_t* radial_entries_host, int64_t* angular_entries_host);
+
 int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const double* force_dev,
                    const double* virial_dev, const double* u_target_dev, const double* f_target_dev,
                    const double* w_target_dev, double* loss_dev);

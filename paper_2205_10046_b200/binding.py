@@ -21,7 +21,7 @@ exported_symbols = (
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement", "nep_list_raggedness",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
     "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
-    "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss",
+    "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss", "nep_batch_pair_counts",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
 )
@@ -112,6 +112,8 @@ def load_library():
     L.nep_batch_compute.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.nep_batch_loss.restype = C.c_int
     L.nep_batch_loss.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
+    L.nep_batch_pair_counts.restype = C.c_int
+    L.nep_batch_pair_counts.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     L.nep_get_latent.restype = C.c_int
     L.nep_get_latent.argtypes = [vp, vp]
     L.nep_heat_current.restype = C.c_int
@@ -365,6 +367,12 @@ class NEP:
                                               C.c_void_p(e.data_ptr()), C.c_void_p(f.data_ptr()) if want_forces else None,
                                               C.c_void_p(w.data_ptr()) if want_forces else None))
         return e, f, w
+
+    def nep_batch_pair_counts(self):
+        """(entries inside rc_radial, entries inside rc_angular) of the whole batch, lattice images counted."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._check(self._L.nep_batch_pair_counts(self._h_ptr, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def nep_batch_loss(self, e, f, w, u_target, f_target, w_target6):
         """[n_pop][3] = (L_e, L_f, L_v) of Eq. (33) per member; targets are CUDA f64 tensors [n_str], [N][3], [n_str][6]."""

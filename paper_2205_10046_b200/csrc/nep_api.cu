@@ -1346,6 +1346,23 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
     return NEP_OK;
 }
 
+int nep_batch_pair_counts(nep_t* nep, int64_t* radial_entries_host, int64_t* angular_entries_host)
+{
+    if (!nep || !radial_entries_host || !angular_entries_host) return NEP_ERR_INVALID_ARG;
+    auto& b = nep->b;
+    if (b.n_str < 1) return nep_fail(nep, NEP_ERR_STATE, "nep_batch_neighbors has not been called");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    std::vector<int> c((size_t)b.N), ca((size_t)b.N);
+    NEP_CUDA(cudaMemcpyAsync(c.data(), b.cnt, sizeof(int) * (size_t)b.N, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaMemcpyAsync(ca.data(), b.cntA, sizeof(int) * (size_t)b.N, cudaMemcpyDeviceToHost, nep->stream));
+    NEP_CUDA(cudaStreamSynchronize(nep->stream));
+    int64_t sr = 0, sa = 0;
+    for (int i = 0; i < b.N; ++i) { sr += c[(size_t)i]; sa += ca[(size_t)i]; }
+    *radial_entries_host = sr;
+    *angular_entries_host = sa;
+    return NEP_OK;
+}
+
 int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const double* force_dev, const double* virial_dev,
                    const double* u_target_dev, const double* f_target_dev, const double* w_target_dev, double* loss_dev)
 {
