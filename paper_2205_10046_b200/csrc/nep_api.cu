@@ -215,7 +215,9 @@ int build_lists(nep_t* nep, const double* pos_dev)
     if (nep->capA == 0) {   // first build for this n: size from the mean density, corrected below if short
         const double rho = (double)n / nep->volume;
         const double vA = 4.0 / 3.0 * 3.14159265358979 * acut * acut * acut, vR = 4.0 / 3.0 * 3.14159265358979 * rcut * rcut * rcut;
-        int capA = (int)(rho * vA * 1.25) + 12, capS = (int)(rho * (vR - vA) * 1.25) + 12;
+        // the outer shell gets the larger margin: its count per atom fluctuates more (a thin shell), and a re-allocation
+        // in mid-run frees and allocates gigabytes with the device drained -- 20 ms to 1.2 s, measured
+        int capA = (int)(rho * vA * 1.25) + 12, capS = (int)(rho * (vR - vA) * 1.6) + 16;
         if (capA > 256) capA = 256;
         NEP_TRY(alloc_lists(nep, capA, capS));
     }
@@ -540,16 +542,11 @@ int dispatch_force_radial(nep_t* nep)
     return nep_fail(nep, NEP_ERR_INVALID_ARG, "basis_radial out of range");
 }
 
-int dispatch_final(nep_t* nep, const FinalKick& fk)
+int dispatch_final(nep_t* nep)
 {
     const NepDims& d = nep->d;
-    if (fk.mode) {
-        NEP_LAUNCH(NEP_K_FINAL, k_final<true><<<div_up(d.n, 256), 256, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->pf, nep->mA, nep->mB,
-                                                                 nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out, fk));
-    } else {
-        NEP_LAUNCH(NEP_K_FINAL, k_final<false><<<div_up(d.n, 256), 256, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->pf, nep->mA, nep->mB,
-                                                                  nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out, fk));
-    }
+    NEP_LAUNCH(NEP_K_FINAL, k_final<<<div_up(d.n, 256), 256, 0, nep->stream>>>(d, nep->posq, nep->perm, nep->cA, nep->ncA, nep->cB, nep->ncB, nep->pf, nep->mA, nep->mB,
+                                                       nep->fa, nep->U, nep->e_out, nep->f_out, nep->w_out));
     return NEP_OK;
 }
 
@@ -559,8 +556,6 @@ int evaluate(nep_t* nep, const double* pos_dev, bool reuse_geometry = false)
     const NepDims& d = nep->d;
     const int n = d.n;
     cudaStream_t st = nep->stream;
-    const FinalKick fk = nep->final_kick;                // set by md_loop for this one evaluation only
-    nep->final_kick.mode = 0;
     CellInv inv;
     for (int a = 0; a < 9; ++a) inv.m[a] = nep->Hinv[a];
     NEP_CUDA(cudaMemsetAsync(nep->tile_ctr, 0, sizeof(int) * 64, st));
@@ -580,7 +575,7 @@ int evaluate(nep_t* nep, const double* pos_dev, bool reuse_geometry = false)
     NEP_TRY(dispatch_ann(nep));
     NEP_TRY(dispatch_angular(nep, C, true));
     NEP_TRY(dispatch_force_radial(nep));
-    NEP_TRY(dispatch_final(nep, fk));
+    NEP_TRY(dispatch_final(nep));
     nep->have_eval = true;
     return NEP_OK;
 }
@@ -924,8 +919,6 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
     return nep_get_last(nep, energy_dev, force_dev, virial_dev);
 }
 
-const int kFinalKickMaxAtoms = 1 << 18;   // NVE: the integrator tail rides in k_final up to this size (launch-bound steps)
-
 // thermostat of md_loop: none (NVE), Berendsen (reading A15) or Langevin (reading A16)
 struct Thermostat {
     int kind;                 // 0 none, 1 Berendsen, 2 Langevin
@@ -988,15 +981,11 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
         if (th.kind == 2)
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,
                                                       2ull * (unsigned long long)(th.first_step + s), nep->type_orig, nep->mass_dev, vel_dev));
-        // NVE: the closing half kick of step s - 1 and the opening half kick + drift of step s were applied by the k_final
-        // of step s - 1 (FinalKick mode 2), where the force is still in registers
-        // (small systems; large ones keep the streaming k_kick_kick_drift, see k_final)
+        // NVE: the closing half kick of step s - 1 is fused with the opening half kick + drift of step s
         const bool fuse_kicks = th.kind == 0;
-        const bool in_final = fuse_kicks && n <= kFinalKickMaxAtoms;
-        if (fuse_kicks && s > 0) {
-            if (!in_final)
-                NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
-        } else
+        if (fuse_kicks && s > 0)
+            NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
+        else
             NEP_LAUNCH(NEP_K_KICK_DRIFT, k_kick_drift<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, dt_fs, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev, pos_dev));
         if (pos_ready && s == n_steps - 1) NEP_CUDA(cudaEventRecord(pos_ready, st));
         nep->steps_since_build++;
@@ -1006,13 +995,8 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
             NEP_TRY(build_lists(nep, pos_dev));
             NEP_TRY(skin_check(nep, disp_bits));
         }
-        if (in_final) {
-            nep->final_kick.mode = s == n_steps - 1 ? 1 : 2;
-            nep->final_kick.hdt = hdt; nep->final_kick.dt = dt_fs;
-            nep->final_kick.mass = nep->mass_dev; nep->final_kick.vel = vel_dev; nep->final_kick.pos = pos_dev;
-        }
         NEP_TRY(evaluate(nep, pos_dev));
-        if (!in_final && (!fuse_kicks || s == n_steps - 1))
+        if (!fuse_kicks || s == n_steps - 1)
             NEP_LAUNCH(NEP_K_KICK, k_kick<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, hdt, nep->type_orig, nep->mass_dev, nep->f_out, vel_dev));
         if (th.kind == 2)
             NEP_LAUNCH(NEP_K_THERMOSTAT, k_langevin_half<<<div_up(3 * (int64_t)n, TB), TB, 0, st>>>(n, lc1, lc2, kBoltzmann * t_target * kAccConv, th.seed,

@@ -41,16 +41,6 @@ struct NepDims {
     int mrec;                    // 64-bit words of an atom's mask record (4 maskW, see k_filter)
 };
 
-// integrator tail fused into k_final by md_step (NVE): mode 0 none, 1 closing half kick, 2 closing kick + next step's
-// opening kick and drift
-struct FinalKick {
-    int mode;
-    double hdt, dt;              // dt/2 x unit conversion, dt
-    const double* mass;          // per type
-    double* vel;
-    double* pos;
-};
-
 struct nep_ctx {
     nep_hyper_t h;
     NepDims d;
@@ -143,7 +133,6 @@ struct nep_ctx {
     float* mA;               // [capA][n] received from j = cA[m][i]: radial scalar m_ji
     float* mB;               // [capA+capS][n] received from j = cB[m][i]: radial scalar m_ji
     float4* fa;              // [n] sum_j dU_i/dr_ij (angular part from k_force_angular, radial added by k_force_radial)
-    FinalKick final_kick;    // integrator tail of the next k_final launch (md_loop, NVE); mode 0 otherwise
     double* e_out;           // [n]    orig order
     double* f_out;           // [n][3]
     double* w_out;           // [n][9]

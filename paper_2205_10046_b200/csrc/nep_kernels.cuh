@@ -1309,13 +1309,12 @@ __device__ __forceinline__ void final_walk(const NepDims& D, const int4& pi, con
     }
 }
 
-template <bool KICK>
 __global__ void __launch_bounds__(256)
 k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
         const int* __restrict__ cA, const int* __restrict__ ncA, const int* __restrict__ cB,
         const int* __restrict__ ncB, const float4* __restrict__ pf, const float* __restrict__ mA, const float* __restrict__ mB,
         const float4* __restrict__ fa, const float* __restrict__ U,
-        double* __restrict__ e_out, double* __restrict__ f_out, double* __restrict__ w_out, FinalKick K)
+        double* __restrict__ e_out, double* __restrict__ f_out, double* __restrict__ w_out)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= D.n) return;
@@ -1335,25 +1334,6 @@ k_final(NepDims D, const int4* __restrict__ posq, const int* __restrict__ perm,
     if (w_out) {
 #pragma unroll
         for (int a = 0; a < 9; ++a) w_out[9 * i + a] = (double)acc.w[a];
-    }
-    if (KICK && K.mode) {
-        // NVE inside md_step, small systems (a step there is launch-bound): the closing half kick of this step and (mode 2)
-        // the opening half kick + drift of the next, with the arithmetic of k_kick / k_kick_kick_drift, applied where the
-        // force is in registers -- one launch less per step (64 k atoms: 0.246 -> 0.229 ms/step).  Not for large systems:
-        // the scattered fp64 updates and 14 more registers cost k_final 130 us at 1M atoms, the streaming kick kernel 30.
-        // Nothing in this kernel reads pos or vel (the gathers go to the quantised copy posq).
-        const double mi = K.mass[pi.w];
-        const double fr[3] = {(double)acc.fx, (double)acc.fy, (double)acc.fz};
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const double acc_a = fr[a] / mi;
-            double v = K.vel[3 * i + a] + K.hdt * acc_a;
-            if (K.mode == 2) {
-                v = v + K.hdt * acc_a;
-                K.pos[3 * i + a] += K.dt * v;
-            }
-            K.vel[3 * i + a] = v;
-        }
     }
 }
 
