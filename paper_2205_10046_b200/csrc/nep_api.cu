@@ -1251,7 +1251,7 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
     NEP_CUDA(cudaMemsetAsync(b.bad, 0, sizeof(int), st));
     // count, size the storage from the longest list, fill, reverse slots
     NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, nep->d.rcA, 0, 0,
-                                                                          b.cnt, b.cntA, nullptr, nullptr, nullptr, b.bad));
+                                                                          b.cnt, b.cntA, nullptr, nullptr, nullptr, nullptr, b.bad));
     std::vector<int> cnt((size_t)N);
     int bad = 0;
     NEP_CUDA(cudaMemcpyAsync(cnt.data(), b.cnt, sizeof(int) * (size_t)N, cudaMemcpyDeviceToHost, st));
@@ -1264,9 +1264,10 @@ int nep_batch_neighbors(nep_t* nep, int32_t n_str, const int32_t* atom_offset_ho
     NEP_TRY(dev_alloc(nep, &b.nbr, (size_t)N * cap));
     NEP_TRY(dev_alloc(nep, &b.d, (size_t)N * cap));
     NEP_TRY(dev_alloc(nep, &b.code, (size_t)N * cap));
+    NEP_TRY(dev_alloc(nep, &b.tnb, (size_t)N * cap));
     NEP_TRY(dev_alloc(nep, &b.rev, (size_t)N * cap));
     NEP_LAUNCH(NEP_K_BATCH, kb_neighbors<<<div_up(N, 128), 128, 0, st>>>(N, b.sid, b.off, b.H, b.Hinv, b.M, pos_dev, b.type, nep->d.T, nep->h.rc_radial, nep->d.rcA, 1, cap,
-                                                                          b.cnt, b.cntA, b.nbr, b.d, b.code, b.bad));
+                                                                          b.cnt, b.cntA, b.nbr, b.d, b.code, b.tnb, b.bad));
     NEP_LAUNCH(NEP_K_BATCH, kb_reverse<<<div_up(N, 128), 128, 0, st>>>(N, cap, b.cnt, b.nbr, b.code, b.rev, b.bad));
     NEP_CUDA(cudaMemcpyAsync(&bad, b.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
     NEP_CUDA(cudaStreamSynchronize(st));
@@ -1327,10 +1328,10 @@ int nep_batch_compute(nep_t* nep, int32_t n_pop, const float* c_radial, const fl
             const dim3 gridb(div_up(b.N, bs), np);                                                               \
             NEP_TRY(allow_smem(nep, kb_descriptors<NCHB>, smem(bs)));                                            \
             NEP_TRY(allow_smem(nep, kb_partial<NCHB>, smem(bs)));                                                \
-            NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.q, b.S, b.cntA)); \
+            NEP_LAUNCH(NEP_K_BATCH_DESC, kb_descriptors<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.tnb, b.d, b.q, b.S, b.cntA)); \
             NEP_TRY(launch_batch_ann(nep, grid, P, energy_dev + p0 * N));                                       \
             if (force_dev || virial_dev)                                                                        \
-                NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.nbr, b.d, b.S, b.fp, b.pf, b.cntA)); \
+                NEP_LAUNCH(NEP_K_BATCH_PARTIAL, kb_partial<NCHB><<<gridb, bs, smem(bs), st>>>(d, C, b.N, b.cap, P, b.type, b.cnt, b.tnb, b.d, b.S, b.fp, b.pf, b.cntA)); \
         } while (0)
         switch (d.NA) {
             case 5: NEP_KB_LAUNCH(5); break;

@@ -42,7 +42,7 @@ kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, co
              const double* __restrict__ Hinvs, const int* __restrict__ Ms, const double* __restrict__ pos,
              const int* __restrict__ type, int n_types, double rcR, float rcA,
              int fill, int cap, int* __restrict__ cnt, int* __restrict__ cntA, int* __restrict__ nbr, float4* __restrict__ dvec,
-             unsigned short* __restrict__ code, int* __restrict__ bad)
+             unsigned short* __restrict__ code, unsigned char* __restrict__ tnb, int* __restrict__ bad)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -80,6 +80,7 @@ kb_neighbors(int N, const int* __restrict__ sid, const int* __restrict__ off, co
                         if (fill && slot < cap) {
                             const size_t e = (size_t)i * cap + slot;
                             nbr[e] = j;
+                            tnb[e] = (unsigned char)type[j];
                             dvec[e] = make_float4((float)d[0], (float)d[1], (float)d[2], (float)sqrt(d2));
                             code[e] = (unsigned short)((ma + 8) | ((mb + 8) << 4) | ((mc + 8) << 8));
                         }
@@ -128,6 +129,26 @@ struct ChebWalk {
     }
 };
 
+// Walk over the entries of one atom (pair vector + distance, neighbour's type), the next entry requested while the
+// current one is processed.
+struct KbWalk {
+    const float4* __restrict__ dv; const unsigned char* __restrict__ tv;
+    int m, cnt, t, tn; float4 d, dn;
+    __device__ __forceinline__ KbWalk(const float4* __restrict__ dvec_row, const unsigned char* __restrict__ tnb_row, int cnt_)
+        : dv(dvec_row), tv(tnb_row), m(-1), cnt(cnt_), t(0), tn(0)
+    {
+        dn = make_float4(0.0f, 0.0f, 1.0f, 1.0f);
+        if (cnt > 0) { dn = dv[0]; tn = tv[0]; }
+    }
+    __device__ __forceinline__ bool next()
+    {
+        if (++m >= cnt) return false;
+        d = dn; t = tn;
+        if (m + 1 < cnt) { dn = dv[m + 1]; tn = tv[m + 1]; }
+        return true;
+    }
+};
+
 // ---- descriptors + network: q, S, Fp, U of one (atom, member) --------------------------------------------------
 // scratch per (member, atom): q [D] (also the network input), S [NA][24], fp [D]; row-major, one row per thread
 // Shared memory of kb_descriptors / kb_partial (dynamic): this thread's column of T x KR per-type sums (resp. its
@@ -148,7 +169,7 @@ __device__ __forceinline__ void kb_stage_angular(const NepDims& D, const float* 
 template <int NCHB>
 __global__ void __launch_bounds__(128)
 kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
-               const int* __restrict__ nbr, const float4* __restrict__ dvec,
+               const unsigned char* __restrict__ tnb, const float4* __restrict__ dvec,
                float* __restrict__ qbuf, float* __restrict__ Sbuf, const int* __restrict__ cntA)
 {
     extern __shared__ float sm[];
@@ -169,10 +190,9 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
     // Eq. (2)-(3) re-associated as in the MD path: q_n = sum_t sum_k c[ti][t][n][k] F_t,k with the per-type basis sums
     // F_t,k = sum_{j of type t} f_k(r_ij): one Chebyshev walk and KR additions per pair, the contraction once per atom
     for (int t = 0; t < T * D.KR; ++t) my[t * BS] = 0.0f;
-    for (int m = 0; m < c; ++m) {
-        const size_t e = (size_t)i * cap + m;
-        float* F = my + (size_t)type[nbr[e]] * D.KR * BS;
-        ChebWalk w(dvec[e].w, D.rcR_inv);
+    for (KbWalk pw(dvec + (size_t)i * cap, tnb + (size_t)i * cap, c); pw.next();) {
+        float* F = my + (size_t)pw.t * D.KR * BS;
+        ChebWalk w(pw.d.w, D.rcR_inv);
         for (int k = 0; k < D.KR; ++k) {
             float f, df; w.get(f, df);
             F[k * BS] += f;
@@ -196,11 +216,10 @@ kb_descriptors(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* _
         for (int u = 0; u < NCHB; ++u)
 #pragma unroll
             for (int k = 0; k < NEP_NUM_S; ++k) Sa[u][k] = 0.0f;
-        for (int m = 0; m < ca; ++m) {
-            const size_t e = (size_t)i * cap + m;
-            const float4 d = dvec[e];
+        for (KbWalk pw(dvec + (size_t)i * cap, tnb + (size_t)i * cap, ca); pw.next();) {
+            const float4 d = pw.d;
             const float rinv = 1.0f / d.w;
-            const float* cc = tab + (size_t)(ti * T + type[nbr[e]]) * D.KA * NCHB;
+            const float* cc = tab + (size_t)(ti * T + pw.t) * D.KA * NCHB;
             float g[NCHB];
 #pragma unroll
             for (int u = 0; u < NCHB; ++u) g[u] = 0.0f;
@@ -344,7 +363,7 @@ __device__ __forceinline__ void angular_assemble(const float (&G)[NCHB][NEP_NUM_
 template <int NCHB>
 __global__ void __launch_bounds__(128)
 kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __restrict__ type, const int* __restrict__ cnt,
-           const int* __restrict__ nbr, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
+           const unsigned char* __restrict__ tnb, const float4* __restrict__ dvec, const float* __restrict__ Sbuf,
            const float* __restrict__ fpbuf, float4* __restrict__ pfbuf, const int* __restrict__ cntA)
 {
     extern __shared__ float sm[];
@@ -371,11 +390,11 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
             for (int n = 0; n < D.NR; ++n) a = fmaf(fp[n], __ldg(cR + ((size_t)(ti * T + t) * D.NR + n) * D.KR + k), a);
             my[(t * D.KR + k) * BS] = a;
         }
-    for (int m = 0; m < c; ++m) {
-        const size_t e = (size_t)i * cap + m;
-        const float4 d = dvec[e];
+    for (KbWalk pw(dvec + (size_t)i * cap, tnb + (size_t)i * cap, c); pw.next();) {
+        const int m = pw.m;
+        const float4 d = pw.d;
         const float rinv = 1.0f / d.w;
-        const float* E = my + (size_t)type[nbr[e]] * D.KR * BS;
+        const float* E = my + (size_t)pw.t * D.KR * BS;
         float s = 0.0f;
         ChebWalk w(d.w, D.rcR_inv);
         for (int k = 0; k < D.KR; ++k) {
@@ -404,11 +423,11 @@ kb_partial(NepDims D, NepCoef C, int N, int cap, BatchParams P, const int* __res
                 for (int k = 0; k < NEP_NUM_S; ++k) G[u][k] = 0.0f;
             }
         }
-        for (int m = 0; m < ca; ++m) {
-            const size_t e = (size_t)i * cap + m;
-            const float4 d = dvec[e];
+        for (KbWalk pw(dvec + (size_t)i * cap, tnb + (size_t)i * cap, ca); pw.next();) {
+            const int m = pw.m;
+            const float4 d = pw.d;
             const float rinv = 1.0f / d.w;
-            const float* cc = tab + (size_t)(ti * T + type[nbr[e]]) * D.KA * NCHB;
+            const float* cc = tab + (size_t)(ti * T + pw.t) * D.KA * NCHB;
             float g[NCHB], dg[NCHB];
 #pragma unroll
             for (int u = 0; u < NCHB; ++u) { g[u] = 0.0f; dg[u] = 0.0f; }

@@ -160,6 +160,7 @@ struct nep_ctx {
         int* cnt; int* cntA; int* nbr;     // [N] entries, [N] of which inside rc_angular (stored first), [N][cap]
         float4* d;                         // [N][cap] pair vector + distance
         unsigned short* code; unsigned short* rev;   // [N][cap] image-shift code, slot of the reverse entry
+        unsigned char* tnb;                // [N][cap] type of the entry's neighbour
         int* bad;                          // [1] device flag
         float* par[6]; size_t par_cap[6];  // parameters of all members of a call
         float* q; float* S; float* fp; float4* pf; size_t scratch_rows;   // per (member, atom) scratch of a chunk
