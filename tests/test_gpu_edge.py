@@ -378,3 +378,38 @@ def test_bad_types_and_host_array_dtypes_are_rejected(pkg):
     nep.nep_compute_host(s.pos, s.types, s.box, 1.0, e, f, w)    # and the well-formed call still works
     assert np.isfinite(f).all() and np.abs(f).max() > 0.0
     nep.close()
+
+
+def test_list_raggedness_and_batch_pair_counts(pkg, oracle_mod):
+    """Measurement hooks: nep_list_raggedness = sum over warps of 32 x longest list / sum of lengths, recomputed here
+    from the exported lists in the internal order is not possible (the order is internal), so it is bracketed: >= 1,
+    = 1 when every atom has the same number of neighbours (perfect lattice), larger for a displaced one; and
+    nep_batch_pair_counts = the oracle's lattice-image entry counts."""
+    cfg = W.get_config(1, (6, 6, 6))
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    pos, typ = torch.tensor(s.pos, device="cuda:0"), torch.tensor(s.types, device="cuda:0")
+    with pytest.raises(pkg.NepError):
+        nep.nep_list_raggedness()
+    nep.nep_neighbors(pos, typ, s.box, cfg.skin)
+    r_disp = nep.nep_list_raggedness()
+    cnt, _ = nep.nep_get_neighbors(0)
+    assert 1.0 <= r_disp <= float(cnt.max()) / float(cnt.float().mean()) + 1e-9
+    lattice = (np.round(s.pos / (cfg.a / 4)) * (cfg.a / 4)) % s.box         # back onto the diamond sites
+    nep.nep_neighbors(torch.tensor(lattice, device="cuda:0"), typ, s.box, 0.3)
+    cnt, _ = nep.nep_get_neighbors(0)
+    if int(cnt.min()) == int(cnt.max()):
+        assert nep.nep_list_raggedness() == pytest.approx(1.0)
+    assert nep.nep_list_raggedness() <= r_disp + 1e-9
+    structs = W.make_batch(3, [((2, 2, 2), None, 0), ((2, 1, 1), (0.1, 0.05, -0.08), 1)])
+    cfg3 = W.get_config(3)
+    nep3 = pkg.NEP(cfg3.hyper, W.make_params(cfg3), cfg3.masses, device=0)
+    off = np.concatenate([[0], np.cumsum([len(q) for q, _, _ in structs])]).astype(np.int32)
+    nep3.nep_batch_neighbors(off, torch.tensor(np.concatenate([q for q, _, _ in structs]), device="cuda:0"),
+                             torch.tensor(np.concatenate([t for _, t, _ in structs]), device="cuda:0"), np.stack([H for _, _, H in structs]))
+    want_r = sum(int(oracle_mod.count_images(q, H, cfg3.hyper.rc_radial).sum()) for q, _, H in structs)
+    want_a = sum(int(oracle_mod.count_images(q, H, cfg3.hyper.rc_angular).sum()) for q, _, H in structs)
+    got_r, got_a = nep3.nep_batch_pair_counts()
+    assert got_r == want_r
+    assert abs(got_a - want_a) <= 2          # the angular split is the kernels' fp32 test r < rc_angular
+    nep.close(); nep3.close()
