@@ -10,22 +10,22 @@
 //     reverse entry (j -> i, -N) in j's list;
 //   * one launch covers all structures x all members: grid.x runs over the atoms of the batch, grid.y over the
 //     members; member p reads its parameters at p * stride from device arrays uploaded once per call (no
-//     per-member synchronisation), so the blocks of one member share its coefficients through L1;
-//   * per member: descriptors + network (kb_descriptors), partial forces of every entry (kb_partial, Eq. (21)),
-//     F_i and W_i from the own and the reverse entries (kb_gather, Eqs. (22)-(24));
+//     per-member synchronisation) and stages what a block needs in shared memory;
+//   * per member: descriptors (kb_descriptors), network (kb_ann), partial forces of every entry (kb_partial,
+//     Eq. (21)), F_i and W_i from the own and the reverse entries (kb_gather, Eqs. (22)-(24));
 //   * the data terms of Eq. (33) are reduced on the device per (member, structure) and then per member in a
 //     fixed order (kb_loss_partial, kb_loss_total).
 // fp32 arithmetic like the MD path, fp64 outputs.  One thread per (atom, member); loops over n, k
-// have run-time bounds (any hyper-parameters), the angular sums are held 4 channels at a time.
+// have run-time bounds (any hyper-parameters).  What the kernels take over from the MD path: the entries inside the
+// angular cutoff come first in an atom's list (no skipping in place); the radial parts use the per-type basis sums and
+// the E^i table (KR operations per pair) in a shared-memory column per thread; the angular coefficients of a pass
+// are staged per block as [type pair][k][channel]; five to seven angular channels go in one pass, A_k and B_k are
+// formed where they are used; the network has its own kernel with the member's weights in shared memory.
 #pragma once
 #include "nep_common.cuh"
 #include "nep_kernels.cuh"
 
 #define NEP_BATCH_MAX_SHIFT 7      // |image shift relative to the minimum image| per axis that fits the reverse-entry code
-
-#ifndef NEP_KB_RG
-#define NEP_KB_RG 4                // radial n per group in kb_descriptors
-#endif
 
 struct BatchParams {               // device pointers to the parameters of ALL members, member-major
     const float* cR;               // [n_pop][T][T][NR][KR]
