@@ -273,6 +273,28 @@ int nep_batch_loss(nep_t* nep, int32_t n_pop, const double* energy_dev, const do
  * NEP_ERR_STATE before the first evaluation.  Does not synchronise.                                    */
 int nep_heat_current(nep_t* nep, const double* vel_dev, double* j_atom_dev, double* j_total_dev);
 
+/* nep_heat_current_static: the same J_i and J as nep_heat_current, for callers that must not allocate.
+ * Who that is: a sampling loop (Green-Kubo runs read J every few steps) inside a process
+ * whose free device memory already belongs to someone else -- a framework's caching allocator, a second
+ * simulation sharing the GPU -- so that a cudaMalloc of even a few hundred kB fails; and threads that cannot
+ * afford the device-wide stall an allocation or a free may cause for every other stream.  nep_heat_current
+ * grows a cudaMalloc'ed scratch buffer for its block partials on first use and when n grows; this call uses
+ * a fixed array inside the library image instead and calls no cudaMalloc, cudaFree or any allocating routine.
+ *   Limit:  n <= 4,194,304 atoms (the array holds 3 partials per 256 atoms: 393,240 bytes).  Larger systems
+ *           return NEP_ERR_INVALID_ARG with a message naming the limit; use nep_heat_current for them.
+ *   Cost:   every GPU on which the library is loaded holds those 393,240 bytes until the process exits,
+ *           used or not.
+ *   Set-up: the FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with
+ *           that device current) and keeps it; make that first call outside any stream capture.
+ *   Sharing: all handles and all calls on one device use the same array, and it keeps the last call's
+ *           partials.  Nothing in it needs clearing (each call overwrites every element it later reads), but
+ *           two calls that overlap on the GPU -- different streams, or different handles on different
+ *           streams -- race on it and give wrong totals: keep calls on one device ordered.  With
+ *           j_total_dev == NULL the total is left in the array's tail, where the next call overwrites it.
+ * Arguments, units, order of the reduction (bitwise the same result as nep_heat_current), error codes and
+ * "does not synchronise" are as for nep_heat_current; inputs and outputs stay caller-owned device memory. */
+int nep_heat_current_static(nep_t* nep, const double* vel_dev, double* j_atom_dev, double* j_total_dev);
+
 /* ---- measurement support (bench.py) ---------------------------------------------------------------
  * nep_launch_count: kernel launches the handle has enqueued so far (bench.py's gpu_launches).
  * nep_device_bytes: device memory the handle currently owns (model tables, lists, scratch, staging).

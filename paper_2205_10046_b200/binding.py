@@ -20,7 +20,7 @@ exported_symbols = (
     "nep_create", "nep_destroy", "nep_num_descriptors", "nep_neighbors", "nep_max_neighbors",
     "nep_get_neighbors", "nep_compute", "md_step", "nep_get_last", "nep_max_displacement", "nep_list_raggedness",
     "nep_compute_host", "md_run_host", "nep_get_descriptors", "nep_get_angular_sums", "nep_get_latent",
-    "nep_heat_current", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
+    "nep_heat_current", "nep_heat_current_static", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
     "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss", "nep_batch_pair_counts",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
     "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
@@ -118,6 +118,8 @@ def load_library():
     L.nep_get_latent.argtypes = [vp, vp]
     L.nep_heat_current.restype = C.c_int
     L.nep_heat_current.argtypes = [vp, vp, vp, vp]
+    L.nep_heat_current_static.restype = C.c_int
+    L.nep_heat_current_static.argtypes = [vp, vp, vp, vp]
     L.nep_launch_count.restype = i64
     L.nep_launch_count.argtypes = [vp]
     L.nep_pair_counts.restype = C.c_int
@@ -401,6 +403,20 @@ class NEP:
         self._check(self._L.nep_heat_current(self._h_ptr, self._dev(vel, torch.float64, 3 * n),
                                              C.c_void_p(ja.data_ptr()), C.c_void_p(jt.data_ptr())))
         return ja, jt
+
+    def nep_heat_current_static(self, vel, j_atom, j_total):
+        """nep_heat_current for callers that must not allocate on the device: the block partials go to a
+        fixed array inside the library (limit 4,194,304 atoms; NepError beyond it) instead of a cudaMalloc'ed
+        buffer, and this wrapper allocates nothing either -- `j_atom` [n][3] and `j_total` [3] are fp64 CUDA
+        tensors the caller made beforehand and are filled in place.  The array is shared by every call on a
+        device: do not let two calls overlap on the GPU.  Make the first call on a device outside any stream
+        capture (it looks the array's address up).  See include/nep.h."""
+        torch = self._torch
+        n = self.n
+        self._check(self._L.nep_heat_current_static(self._h_ptr, self._dev(vel, torch.float64, 3 * n),
+                                                    self._dev(j_atom, torch.float64, 3 * n),
+                                                    self._dev(j_total, torch.float64, 3)))
+        return j_atom, j_total
 
     def nep_launch_count(self) -> int:
         return int(self._L.nep_launch_count(self._h_ptr))

@@ -3,6 +3,7 @@
 #include <math.h>
 #include <stdlib.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1194,6 +1195,74 @@ int nep_heat_current(nep_t* nep, const double* vel_dev, double* j_atom_dev, doub
     NEP_LAUNCH(NEP_K_EXPORT, k_heat_current<<<nb, 256, 0, nep->stream>>>(n, nep->w_out, vel_dev, j_atom_dev, nep->heat_partial));
     double* tot = j_total_dev ? j_total_dev : nep->heat_partial + 3 * (size_t)nb;
     NEP_LAUNCH(NEP_K_EXPORT, k_heat_total<<<1, 256, 0, nep->stream>>>(nb, nep->heat_partial, tot));
+    return NEP_OK;
+}
+
+// ---- heat current without any allocation (nep_heat_current_static, include/nep.h) ------------------------
+// nep_heat_current keeps its block partials in a cudaMalloc'ed buffer that grows with the system.  Some users
+// of this library sample J every few steps from places where a device allocation is not an option: a Green-Kubo
+// production loop that has handed all free device memory to another allocator (PyTorch's caching allocator,
+// a second simulation on the same GPU), where cudaMalloc fails although the 400 kB are trivially "there"; or a
+// latency-sensitive service thread, for which the device-wide synchronisation that cudaMalloc / cudaFree may
+// imply stalls every other stream of the process.  For them the partials live in the array below, which is part
+// of the library image: every GPU that loads libnep_b200.so carries these 393,240 bytes from the first CUDA call
+// to process exit, whether or not the entry point is ever used.
+//
+// g_heat_static is a DEVICE symbol.  In host code its name is only a host-side shadow of it: handing
+// `g_heat_static` itself to a kernel would pass a host address (a fault, or on systems where the GPU can reach host
+// memory a silent write to the wrong place).  The device address comes from cudaGetSymbolAddress, asked once per
+// device with that device current (heat_static_address), and that pointer is what the kernels receive.
+#define NEP_HEAT_STATIC_MAX_ATOMS 4194304                       /* stated limit of the entry point           */
+#define NEP_HEAT_STATIC_MAX_BLOCKS (NEP_HEAT_STATIC_MAX_ATOMS / 256)
+#define NEP_HEAT_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) double g_heat_static[3 * NEP_HEAT_STATIC_MAX_BLOCKS + 3];
+
+namespace {
+std::mutex g_heat_static_mutex;
+double* g_heat_static_ptr[NEP_HEAT_STATIC_MAX_DEVICES];         // device address of g_heat_static, per device
+
+// Device address of g_heat_static on `device`, which must be the current device.  The first call per device asks
+// the runtime (no allocation: the array was placed when the module was loaded); later calls read the table.
+cudaError_t heat_static_address(int device, double** out)
+{
+    std::lock_guard<std::mutex> lock(g_heat_static_mutex);
+    if (!g_heat_static_ptr[device]) {
+        double* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_heat_static);
+        if (e != cudaSuccess) return e;
+        g_heat_static_ptr[device] = p;
+    }
+    *out = g_heat_static_ptr[device];
+    return cudaSuccess;
+}
+}  // namespace
+
+int nep_heat_current_static(nep_t* nep, const double* vel_dev, double* j_atom_dev, double* j_total_dev)
+{
+    if (!nep) return NEP_ERR_INVALID_ARG;
+    if (!vel_dev || (!j_atom_dev && !j_total_dev)) return nep_fail(nep, NEP_ERR_INVALID_ARG, "null pointer");
+    if (!nep->have_eval) return nep_fail(nep, NEP_ERR_STATE, "no evaluation yet");
+    if (nep->n > NEP_HEAT_STATIC_MAX_ATOMS) {
+        snprintf(nep->err, sizeof(nep->err),
+                 "nep_heat_current_static: %lld atoms exceed the static scratch's limit of %d atoms; use nep_heat_current",
+                 (long long)nep->n, NEP_HEAT_STATIC_MAX_ATOMS);
+        return NEP_ERR_INVALID_ARG;
+    }
+    if (nep->device < 0 || nep->device >= NEP_HEAT_STATIC_MAX_DEVICES)
+        return nep_fail(nep, NEP_ERR_INVALID_ARG, "nep_heat_current_static: device ordinal beyond the per-device table (64)");
+    NEP_CUDA(cudaSetDevice(nep->device));
+    double* scratch = nullptr;
+    NEP_CUDA(heat_static_address(nep->device, &scratch));
+    const int n = (int)nep->n;
+    const int nb = div_up(n, 256);
+    // Nothing has to start at zero: each of the nb blocks stores its three partials unconditionally, and the
+    // second kernel (same stream, so after the first) reads exactly those 3 nb values.  Whatever an earlier
+    // call left beyond them is never read.  Plain launches: the profiling hooks of NEP_LAUNCH are left out.
+    k_heat_current<<<nb, 256, 0, nep->stream>>>(n, nep->w_out, vel_dev, j_atom_dev, scratch);
+    NEP_LAUNCH_CHECK();
+    double* tot = j_total_dev ? j_total_dev : scratch + 3 * (size_t)NEP_HEAT_STATIC_MAX_BLOCKS;
+    k_heat_total<<<1, 256, 0, nep->stream>>>(nb, scratch, tot);
+    NEP_LAUNCH_CHECK();
     return NEP_OK;
 }
 
