@@ -5,5 +5,5 @@ arguments (torch tensors -> device pointers).  There is no CPU fallback: importi
 the shared library is missing.
 """
 from .binding import (  # noqa: F401
-    NEP, NepError, NepHyper, lib_path, load_library, exported_symbols,
+    NEP, NepError, NepHyper, lib_path, lib_overridden, load_library, exported_symbols,
 )

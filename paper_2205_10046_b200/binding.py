@@ -51,6 +51,11 @@ def lib_path() -> str:
     return _LIB_PATH
 
 
+def lib_overridden() -> bool:
+    """True when NEP_B200_LIB redirected the binding to a library other than the in-tree build."""
+    return bool(os.environ.get("NEP_B200_LIB"))
+
+
 def load_library():
     """Loads libnep_b200.so; fails loudly if it has not been built (no fallback of any kind)."""
     global _lib
@@ -59,6 +64,10 @@ def load_library():
     if not os.path.exists(_LIB_PATH):
         raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2205_10046_b200.build` "
                           "(there is no CPU or PyTorch fallback for the NEP path)")
+    if lib_overridden():
+        import warnings
+        warnings.warn(f"NEP_B200_LIB is set: loading {_LIB_PATH} instead of the in-tree libnep_b200.so; tests and "
+                      "bench numbers of this process come from that build", RuntimeWarning, stacklevel=2)
     L = C.CDLL(_LIB_PATH)
     vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
     fp = C.POINTER(C.c_float)
