@@ -127,7 +127,12 @@ int nep_compute(nep_t* nep, const double* pos_dev, double* energy_dev, double* f
  * build.  The largest displacement of every evaluation is reduced on the device; it is read at every
  * scheduled rebuild and when the call ends, and NEP_ERR_SKIN_EXCEEDED is returned if it was ever above
  * skin/2 (pairs may then have been missed since that build: use a smaller rebuild_every or a larger skin;
- * the state in pos_dev / vel_dev is the one reached, not rolled back).
+ * the state in pos_dev / vel_dev is the one reached, not rolled back).  At a scheduled rebuild the check
+ * comes BEFORE the rebuild, so a skin error is never hidden by an error of that rebuild.
+ * The criterion is sufficient, not necessary: it bounds every atom's ABSOLUTE displacement, so a rigid
+ * translation or a net centre-of-mass drift larger than skin/2 per interval is reported although no pair
+ * distance changed (remove the centre-of-mass velocity, or rebuild more often).  nep_compute() with moved
+ * positions measures the same displacement but checks nothing: such callers poll nep_max_displacement().
  * Synchronises once per list rebuild (overflow check) and once before it returns (skin check).        */
 int md_step(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs,
             int32_t n_steps, int32_t rebuild_every, double skin);
@@ -303,8 +308,8 @@ int nep_heat_current_static(nep_t* nep, const double* vel_dev, double* j_atom_de
  *   drain every 32768 launches).  nep_profile_read: synchronises and returns, per kernel id
  *   k < nep_profile_num_kernels(), the summed device time in ms and the number of launches since the
  *   last nep_profile() call; nep_profile_kernel_name(k) names the id ("radial", "force_angular", ...).
- * nep_probe_fp32: runs an FP32 FMA throughput probe (independent 3-register FFMA chains, no memory
- *   traffic) on `device`/`cuda_stream` and returns the best of 5 timed launches in TFLOP/s: the measured
+ * nep_probe_fp32: runs an FP32 FMA throughput probe (16 independent a = fma(a, m, a) chains per thread, no memory
+ *   traffic) on `device`/`cuda_stream` at 2, 4, 6 and 8 blocks per SM and returns the best timed launch in TFLOP/s: the measured
  *   denominator of the ALU roofline.  Synchronises.                                                    */
 /* nep_pair_counts: ordered pairs inside r_c^R and inside r_c^A at the last evaluation (the sums of
  *   NN_i^R and NN_i^A without skin): the units of the per-kernel flop counts.  Synchronises. */

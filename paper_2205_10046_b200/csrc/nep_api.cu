@@ -991,10 +991,13 @@ static int md_loop(nep_t* nep, double* pos_dev, double* vel_dev, double dt_fs, i
         if (pos_ready && s == n_steps - 1) NEP_CUDA(cudaEventRecord(pos_ready, st));
         nep->steps_since_build++;
         if (nep->steps_since_build >= rebuild_every) {
-            // skin check of the interval that ends here: the copy completes with the build's own synchronisation
+            // skin check of the interval that ends here, BEFORE the rebuild: &disp_bits is pageable memory, so the
+            // copy has completed when the call returns; a run that lost pairs reports that, not whatever the
+            // rebuild of the broken state would have returned, and does not pay for that rebuild
             NEP_CUDA(cudaMemcpyAsync(&disp_bits, nep->disp_max + 1, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
-            NEP_TRY(build_lists(nep, pos_dev));
+            NEP_CUDA(cudaStreamSynchronize(st));
             NEP_TRY(skin_check(nep, disp_bits));
+            NEP_TRY(build_lists(nep, pos_dev));
         }
         NEP_TRY(evaluate(nep, pos_dev));
         if (!fuse_kicks || s == n_steps - 1)
