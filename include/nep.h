@@ -321,6 +321,12 @@ int nep_profile_num_kernels(void);
 const char* nep_profile_kernel_name(int k);
 int nep_profile_read(nep_t* nep, double* ms_total_host, int64_t* launches_host);
 int nep_probe_fp32(int device, void* cuda_stream, double* tflops_host);
+/* Unit-test probe: packs (j_host[a], slot_host[a]) into a list entry on the device exactly as the list kernels do
+ * ((j << 8) | slot, all 32 bits used) and unpacks it again; HOST arrays of `count` int32 each.  0 <= j < 2^24,
+ * 0 <= slot < 256, else NEP_ERR_INVALID_ARG.  Allocates and frees its own device buffer; synchronises.  Lets a cheap
+ * test cover j >= 2^23 (sign bit of the packed word) without a 2^24-atom system.                                  */
+int nep_probe_entry_roundtrip(int device, int32_t count, const int32_t* j_host, const int32_t* slot_host,
+                              int32_t* packed_host, int32_t* j_out_host, int32_t* slot_out_host);
 
 const char* nep_last_error(const nep_t* nep);
 const char* nep_status_string(int status);

@@ -23,7 +23,7 @@ exported_symbols = (
     "nep_heat_current", "nep_heat_current_static", "md_step_nvt_berendsen", "nep_last_temperature", "md_step_nvt_langevin", "nep_set_parameters",
     "nep_compute_population", "nep_loss_terms", "nep_batch_neighbors", "nep_batch_compute", "nep_batch_loss", "nep_batch_pair_counts",
     "nep_launch_count", "nep_pair_counts", "nep_device_bytes", "nep_profile", "nep_profile_num_kernels",
-    "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_last_error", "nep_status_string",
+    "nep_profile_kernel_name", "nep_profile_read", "nep_probe_fp32", "nep_probe_entry_roundtrip", "nep_last_error", "nep_status_string",
 )
 
 
@@ -145,6 +145,8 @@ def load_library():
     L.nep_profile_read.argtypes = [vp, dp, C.POINTER(i64)]
     L.nep_probe_fp32.restype = C.c_int
     L.nep_probe_fp32.argtypes = [C.c_int, vp, dp]
+    L.nep_probe_entry_roundtrip.restype = C.c_int
+    L.nep_probe_entry_roundtrip.argtypes = [C.c_int, i32, ip, ip, ip, ip, ip]
     L.nep_last_error.restype = C.c_char_p
     L.nep_last_error.argtypes = [vp]
     L.nep_status_string.restype = C.c_char_p
@@ -456,6 +458,17 @@ class NEP:
         if rc != 0:
             raise NepError(rc, self._L.nep_status_string(rc).decode())
         return v.value
+
+    def nep_probe_entry_roundtrip(self, j, slot):
+        """(packed, j_out, slot_out) of the device's list-entry packing for int32 host arrays `j`, `slot`."""
+        j = np.ascontiguousarray(j, dtype=np.int32)
+        slot = np.ascontiguousarray(slot, dtype=np.int32)
+        out = [np.empty_like(j) for _ in range(3)]
+        ptr = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32))
+        rc = self._L.nep_probe_entry_roundtrip(self.device, len(j), ptr(j), ptr(slot), *(ptr(o) for o in out))
+        if rc != 0:
+            raise NepError(rc, self._L.nep_status_string(rc).decode())
+        return tuple(out)
 
     # host-buffer entry points: numpy arrays or pinned CPU tensors (anything exposing a host pointer)
     @staticmethod

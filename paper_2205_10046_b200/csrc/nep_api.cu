@@ -480,7 +480,7 @@ int ann_tier(int D)
 
 int dispatch_ann(nep_t* nep)
 {
-    if (!nep->ann_fp32) {
+    if (!nep->ann_fp32 && !nep->ann_precise) {
         bool done = false;
         int rc = NEP_OK;
         switch (nep->DP) {
@@ -710,6 +710,12 @@ int upload_parameters(nep_t* nep, const float* c_radial, const float* c_angular,
         for (int v = 0; v < d.D; ++v) w0p[(size_t)m * nep->DP + v] = w0[(size_t)m * d.D + v];
     nep->b1 = b1[0];
     std::vector<float> vb0(b0, b0 + d.H), vw1(w1, w1 + d.H);
+    // k_ann_tc evaluates tanh with MUFU.EX2 / MUFU.RCP (tanh_fast: absolute error ~1e-7 per neuron), so its error in
+    // U_i is bounded by sum_m |w1_m| x 1e-7.  Up to sum |w1| = 5 that is 5e-7 eV, a twentieth of north_star's 1e-5 eV
+    // bar; wider or larger-weight output layers (trained |w1| > 1, up to 200 neurons) take the tanhf kernel instead.
+    double w1_abs = 0.0;
+    for (int m = 0; m < d.H; ++m) w1_abs += fabs((double)w1[m]);
+    nep->ann_precise = w1_abs > 5.0;
 #define UPLOAD(dst, vec)                                                                          \
     do {                                                                                          \
         if (!nep->dst) NEP_TRY(dev_alloc(nep, &nep->dst, (vec).size()));                          \
@@ -1615,23 +1621,47 @@ int nep_probe_fp32(int device, void* cuda_stream, double* tflops_host)
     if (cudaMalloc((void**)&sink, sizeof(float) * 1024) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_NOMEM; }
     cudaEvent_t a, b;
     cudaEventCreate(&a); cudaEventCreate(&b);
-    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
+    const int threads = 256, iters = 8192;
     double best = 0.0;
-    for (int rep = 0; rep < 6; ++rep) {
-        cudaEventRecord(a, st);
-        k_probe_ffma<<<blocks, threads, 0, st>>>(iters, 1.0f + 1e-7f * rep, sink);
-        cudaEventRecord(b, st);
-        cudaEventSynchronize(b);
-        float ms = 0.0f;
-        cudaEventElapsedTime(&ms, a, b);
-        const double tf = 2.0 * NEP_PROBE_CHAINS * (double)iters * blocks * threads / (ms * 1e-3) / 1e12;
-        if (rep > 0 && tf > best) best = tf;
+    const int per_sm[4] = {2, 4, 6, 8};                     // resident blocks per SM: the best of the sweep is reported
+    for (int sw = 0; sw < 4; ++sw) {
+        const int blocks = prop.multiProcessorCount * per_sm[sw];
+        for (int rep = 0; rep < 4; ++rep) {
+            cudaEventRecord(a, st);
+            k_probe_ffma<<<blocks, threads, 0, st>>>(iters, 1e-7f * (float)(rep + 1), sink);
+            cudaEventRecord(b, st);
+            cudaEventSynchronize(b);
+            float ms = 0.0f;
+            cudaEventElapsedTime(&ms, a, b);
+            const double tf = 2.0 * NEP_PROBE_CHAINS * (double)iters * blocks * threads / (ms * 1e-3) / 1e12;
+            if (rep > 0 && tf > best) best = tf;
+        }
     }
     cudaEventDestroy(a); cudaEventDestroy(b);
     cudaFree(sink);
     if (cudaGetLastError() != cudaSuccess) return NEP_ERR_CUDA;
     *tflops_host = best;
     return NEP_OK;
+}
+
+int nep_probe_entry_roundtrip(int device, int32_t count, const int32_t* j_host, const int32_t* slot_host,
+                              int32_t* packed_host, int32_t* j_out_host, int32_t* slot_out_host)
+{
+    if (count < 1 || !j_host || !slot_host || !packed_host || !j_out_host || !slot_out_host) return NEP_ERR_INVALID_ARG;
+    for (int32_t a = 0; a < count; ++a)
+        if (j_host[a] < 0 || j_host[a] >= NEP_MAX_ATOMS || slot_host[a] < 0 || slot_host[a] >= (1 << NEP_SLOT_BITS)) return NEP_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_CUDA; }
+    int32_t* buf = nullptr;
+    const size_t bytes = sizeof(int32_t) * (size_t)count;
+    if (cudaMalloc((void**)&buf, 5 * bytes) != cudaSuccess) { cudaGetLastError(); return NEP_ERR_NOMEM; }
+    cudaMemcpy(buf, j_host, bytes, cudaMemcpyHostToDevice);
+    cudaMemcpy(buf + count, slot_host, bytes, cudaMemcpyHostToDevice);
+    k_probe_entry<<<div_up(count, 128), 128>>>(count, buf, buf + count, buf + 2 * (size_t)count, buf + 3 * (size_t)count, buf + 4 * (size_t)count);
+    cudaMemcpy(packed_host, buf + 2 * (size_t)count, bytes, cudaMemcpyDeviceToHost);
+    cudaMemcpy(j_out_host, buf + 3 * (size_t)count, bytes, cudaMemcpyDeviceToHost);
+    cudaMemcpy(slot_out_host, buf + 4 * (size_t)count, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(buf);
+    return cudaGetLastError() == cudaSuccess ? NEP_OK : NEP_ERR_CUDA;
 }
 
 }  // extern "C"

@@ -71,6 +71,7 @@ struct nep_ctx {
     int nch_max;            // angular n-values per pass (<= NEP_NCH_MAX)
     size_t smem_budget;     // shared memory per SM that the table-in-smem kernels may carve out of L1
     bool ann_fp32;          // NEP_ANN_FP32 set: the fp32-FMA network kernel instead of the tensor-core one
+    bool ann_precise;       // sum_m |w1_m| too large for tanh_fast's absolute error (upload_parameters): k_ann with tanhf
     double raggedness;      // of the last build: sum over warps of 32 x longest list / sum of list lengths
     bool force_smem_radial; // NEP_RADIAL_SMEM set: use the shared-memory radial kernels even where a register variant exists
     float* w0p;      // [H][DP] rows padded with zeros to DP

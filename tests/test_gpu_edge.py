@@ -276,6 +276,62 @@ def test_network_kernel_variants_agree(pkg, oracle_mod, idx, cells):
     assert np.abs(out["tc"][1] - out["fp32"][1]).max() <= 4e-6 * np.abs(fpo).max()
 
 
+def test_wide_output_layer_takes_the_tanhf_kernel(pkg, oracle_mod):
+    """k_ann_tc's tanh (MUFU.EX2 / MUFU.RCP) has an absolute error of ~1e-7 per neuron, i.e. sum_m |w1_m| x 1e-7 in
+    U_i; nep_create / nep_set_parameters therefore send models with sum |w1| > 5 to the fp32 kernel with tanhf.
+    200 neurons with |w1| in [3, 5] (sum ~ 800): the default handle must give bitwise what NEP_ANN_FP32 gives (the
+    same kernel ran), and meet the oracle at the energy bar scaled with the output layer -- 1e-5 eV is north_star's
+    bar for O(1) output weights (sum |w1| <= 5, where the dispatch switches); every error source of U_i (the fp32
+    pre-activations, tanh, the fp32 sum) is linear in w1, so the bar is 1e-5 x sum |w1| / 5.  dU/dq likewise."""
+    cfg = W.get_config(0)
+    cfg = replace(cfg, hyper=replace(cfg.hyper, n_neurons=200))
+    s, p = W.make_system(cfg), W.make_params(cfg, "stress")
+    rng = np.random.default_rng(77)
+    p = replace(p, w1=(rng.uniform(3.0, 5.0, 200) * rng.choice([-1.0, 1.0], 200)).astype(np.float32))
+    out = {}
+    for variant in ("default", "fp32"):
+        if variant == "fp32":
+            os.environ["NEP_ANN_FP32"] = "1"
+        try:
+            nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+            dpos = torch.tensor(s.pos, device="cuda:0")
+            nep.nep_neighbors(dpos, torch.tensor(s.types, device="cuda:0"), s.box, 0.0)
+            e, f, w = nep.nep_compute(dpos)
+            q, fp = nep.nep_get_descriptors()
+            out[variant] = (e.cpu().numpy(), fp.cpu().numpy(), f.cpu().numpy())
+            nep.close()
+        finally:
+            os.environ.pop("NEP_ANN_FP32", None)
+    assert np.array_equal(out["default"][0], out["fp32"][0]) and np.array_equal(out["default"][1], out["fp32"][1])
+    eo, fo, wo, qo, fpo, So = oracle_mod.compute(cfg.hyper, p, s.pos, s.types, s.box, want_internals=True)
+    scale = float(np.abs(p.w1).sum()) / 5.0
+    assert scale > 100
+    assert np.abs(out["default"][0] - eo).max() <= 1e-5 * scale
+    assert np.abs(out["default"][1] - fpo).max() <= 2e-5 * np.abs(fpo).max()
+    assert np.abs(out["default"][2] - fo).max() <= 1e-4 * np.abs(fo).max()
+
+
+def test_packed_list_entry_round_trip_beyond_2_pow_23(pkg):
+    """A list entry is (j << 8) | slot with j < 2^24: bit 31 is set for every j >= 2^23, and a signed shift would
+    sign-extend it.  The device's own entry_pack / entry_j / slot mask, through nep_probe_entry_roundtrip -- the
+    regular-run stand-in for the 65 GB test_largest_atom_count_2_pow_24."""
+    cfg = W.get_config(0)
+    s, p = W.make_system(cfg), W.make_params(cfg)
+    nep = pkg.NEP(cfg.hyper, p, s.masses, device=0)
+    js = np.array([0, 1, 255, 256, 2**23 - 1, 2**23, 2**23 + 1, 2**24 - 2, 2**24 - 1], dtype=np.int32)
+    slots = np.array([0, 1, 63, 64, 127, 128, 255], dtype=np.int32)
+    j = np.repeat(js, len(slots))
+    slot = np.tile(slots, len(js))
+    packed, j_out, slot_out = nep.nep_probe_entry_roundtrip(j, slot)
+    assert np.array_equal(j_out, j) and np.array_equal(slot_out, slot)
+    expect = ((j.astype(np.uint32) << np.uint32(8)) | slot.astype(np.uint32)).view(np.int32)
+    assert np.array_equal(packed, expect)
+    assert (packed[j >= 2**23] < 0).all(), "the cases must reach the sign bit"
+    with pytest.raises(pkg.NepError):
+        nep.nep_probe_entry_roundtrip(np.array([2**24], dtype=np.int32), np.array([0], dtype=np.int32))
+    nep.close()
+
+
 def test_md_step_zero_steps_and_state_errors(pkg):
     cfg = W.get_config(0)
     s, p = W.make_system(cfg), W.make_params(cfg)
