@@ -4,7 +4,8 @@ Tolerances are BASELINE.json's north_star: neighbour lists bit-exact as sets; pe
 1e-5 eV absolute; each force component within max(1e-4 eV/A, 1e-4 |F|); virial within 1e-4 relative
 (reading A14: per atom ||dW_i||_F <= 1e-4 max(||W_i||_F, median_i ||W_i||_F); total ||dW||_F <= 1e-4 ||W||_F).
 Because the stated weight scale gives weak signals, the internals q, S, Fp are also compared
-component-wise, relative to the largest component of their block (1e-5), and every case is repeated with
+component-wise, relative to the largest component of their block (2e-5: DESIGN.md section 4 derives it from the fp32
+sums of up to ~50 pair terms; SURVEY 8(c) had proposed 1e-5), and every case is repeated with
 the amplified 'stress' parameter set where the 4-/5-body terms are O(0.1-1).
 """
 import numpy as np
