@@ -298,6 +298,45 @@ def whole_job_value(world: int, atoms_per_rank: int, steps: int, ms_max: float) 
     return world * atoms_per_rank * steps / (ms_max * 1e-3)
 
 
+def launch_replicas(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start N ranks of this same command, one
+    replica per GPU, under torch.distributed.run on 127.0.0.1 (the launch line the driver uses).  Replicas only:
+    the ranks share nothing but the barrier and the MAX-over-ranks time (north_star: no sharding, no collectives)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd).returncode
+
+
+def run_dry(args, rank: int, world: int) -> int:
+    """--dry: the multi-rank entry path without any CUDA work (CPU boxes, tests): rendezvous over gloo, a barrier,
+    a synthetic per-rank time through the same max_over_ranks / whole_job_value the timed arm uses, and rank 0's
+    ONE line.  Not a measurement: "dry": true, value from the synthetic times."""
+    import torch.distributed as dist
+    cfg = W.get_config(args.config)
+    n = int(np.prod(cfg.cells)) * len(W._BASIS[cfg.lattice])
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("gloo")
+        dist.barrier()
+    ms = max_over_ranks(10.0 + 5.0 * rank, world, "cpu")
+    value = whole_job_value(world, n, args.steps, ms)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f32", "dry": True,
+                          "data": "none: --dry runs the launch path only (synthetic per-rank times, no CUDA work)",
+                          "config": config_dict(cfg, n, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+                          "gpu_launches": 0, "impl": "ours"}), flush=True)
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -307,6 +346,8 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.dry:
+        return run_dry(args, rank, world)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the NEP path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -633,7 +674,11 @@ def main():
     ap.add_argument("--pop", type=int, default=50, help="--workload batch: parameter sets (PAPER.md:283: a population)")
     ap.add_argument("--windows", type=int, default=0,
                     help="time the K steps as this many consecutive windows (ms/step and pair counts per window)")
+    ap.add_argument("--dry", action="store_true",
+                    help="launch path only: ranks rendezvous over gloo and print the line from synthetic times (no CUDA)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.workload == "md":
+        return launch_replicas(args)                      # N replicas, one per GPU; this process only waits
     if args.warmup < 3:
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
     if args.impl == "reference":

@@ -77,6 +77,29 @@ def test_replica_aggregation_gloo_world2():
     assert out[0] == pytest.approx(want) and out[1] == pytest.approx(want)
 
 
+def test_bench_gpus_2_starts_two_ranks_dry():
+    """`python bench.py --gpus 2` must START two ranks (it used to run one and print n_gpus 1): the
+    same entry path as the timed arm -- re-exec under torch.distributed.run on 127.0.0.1, rendezvous, barrier,
+    MAX over ranks, one line from rank 0 -- with --dry standing in for the CUDA work (gloo, no GPU here)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry", "--steps", "7", "--config", "1"],
+                       capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["dry"] is True and d["scaling"] == "weak"
+    assert d["config"]["parallelism"] == "replicas only" and d["config"]["atoms"] == 64000
+    assert d["value"] == pytest.approx(2 * 64000 * 7 / 15.0e-3)      # the slow rank's 15 ms decides
+    # N = 1: no launcher, no process group, same line shape
+    r1 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--dry", "--steps", "7", "--config", "1"],
+                        capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    d1 = json.loads([l for l in r1.stdout.splitlines() if l.startswith("{")][0])
+    assert d1["n_gpus"] == 1 and d1["value"] == pytest.approx(64000 * 7 / 10.0e-3)
+
+
 def test_cost_model_matches_survey_table():
     """cfg 0/1/3 radial pair 161 + 307 flops, angular pair 420 + 1,160 + 30.  The 307
     are BOTH directions of a pair evaluated at one atom (Alg. 2); every direction is needed once, so the
