@@ -601,14 +601,24 @@ def run_batch(args):
     nep.nep_profile(False)
     ent_r, ent_a = nep.nep_batch_pair_counts()
     l0 = nep.nep_launch_count()
+    sampler = ClockSampler(0)                               # SM clock and throttle reasons DURING the timed region
+    sampler.start()
+    time.sleep(0.15)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for _ in range(args.steps):
         loss = generation()
     ev1.record()
     torch.cuda.synchronize()
+    clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
     assert torch.isfinite(loss).all()
+    # a generation IS end to end: every step uploads the population's parameters from host arrays (nep_batch_compute
+    # takes host pointers) and reads the loss back to the host; the structures are the fixed training set, resident
+    par_bytes = int(sum(getattr(m_, k_).nbytes for m_ in members for k_ in ("c_radial", "c_angular", "w0", "b0", "w1", "b1")))
+    e2e = {"value": N * P * args.steps / (ms * 1e-3), "unit": "atom-member evaluation/s",
+           "h2d_bytes_per_step": par_bytes, "d2h_bytes_per_step": int(loss.numel() * loss.element_size()),
+           "what": "same timed region: host parameter arrays in, loss [n_pop][3] back on the host, every generation"}
     launches = nep.nep_launch_count() - l0
     # oracle on the host cores: compute_images of a few structures with one member
     cpu = None
@@ -642,7 +652,7 @@ def run_batch(args):
                        "atoms_per_structure": [int(np.diff(off).min()), int(np.diff(off).max())],
                        "neighbour_entries_per_atom": None,
                        "step": "host parameters -> nep_batch_compute (E, F, W of every member) -> nep_batch_loss -> host [n_pop][3]"},
-            "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours",
+            "gpu_launches": launches, "cpu_baseline": cpu, "impl": "ours", "clocks": clocks, "e2e": e2e,
             "kernels": [{"name": k, "launches": v[1], "avg_us": v[0] / v[1] * 1e3} for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])]}
     # roofline of the dominant kernel (kb_partial: Eq. (21) of every entry and member), algorithmic flops as in
     # kernel_costs (force_angular + force_radial per ordered pair), against the derived FP32 peak
@@ -652,7 +662,8 @@ def run_batch(args):
         us = prof["batch_partial"][0] / prof["batch_partial"][1] * 1e3
         alu_peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
         line["roofline"] = {"kernel": "batch_partial", "bound": "alu", "achieved": fl / us / 1e6, "peak": alu_peak, "unit": "TFLOP/s",
-                            "frac": fl / us / 1e6 / alu_peak, "avg_us": us, "traffic": None,
+                            "frac": fl / us / 1e6 / alu_peak, "avg_us": us,
+                            "traffic": ncu_traffic("batch_cfg3_fcc_alloy_small_cells").get("batch_partial") if (S, P) == (600, 50) else None,
                             "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}
     line["config"]["neighbour_entries_per_atom"] = [ent_r / N, ent_a / N]
     print(json.dumps(line), flush=True)
