@@ -14,10 +14,13 @@ stated run goes through md_step FIRST, and only then
       clusters and compared with the GPU's E / F / W of the last step at north_star's tolerances;
   (c) sum_i F_i = 0 and the total energy is conserved over the run (NVE) to 2e-3 of the initial kinetic energy,
       the bar tests/test_gpu_parity.py uses for its 200-step run;
-  (d) the run did what it is meant to do to the lists: the longest lists grew (reported in the assertion text).
+  (d) the run did what it is meant to do to the lists: the longest lists grew (reported in the assertion text), and
+      in one extra cfg 3 run with a 1.2 A skin the longest angular-range list crosses the 64-entry mask-word limit.
 
 PAPER.md:240 (energy conservation validates the force expressions), PAPER.md:474 (speed runs are 100 steps).
 """
+from dataclasses import replace
+
 import numpy as np
 import pytest
 
@@ -76,12 +79,16 @@ def check_windows(nep, oracle_mod, cfg, p, s, snap, rng, half):
 
 
 # (config, sampled atoms for the set test, inner half edge of the oracle windows in A)
-RUNS = [(1, 2000, 9.0), (2, 2000, 9.0), (3, 1500, 8.0), (4, 400, 7.0)]
+# the last entry: cfg 3 with a 1.2 A skin, so that the longest angular-range list CROSSES 64 entries in mid-run (past 64 an
+# atom's mask record takes a second word); with the stated 1 A skin it ends at exactly 64.  cfg 4 is above 64 throughout.
+RUNS = [(1, 2000, 9.0, None), (2, 2000, 9.0, None), (3, 1500, 8.0, None), (4, 400, 7.0, None), (3, 1000, 8.0, 1.2)]
 
 
-@pytest.mark.parametrize("idx,n_sample,half", RUNS)
-def test_stated_run_length_nve(pkg, oracle_mod, idx, n_sample, half):
+@pytest.mark.parametrize("idx,n_sample,half,skin", RUNS)
+def test_stated_run_length_nve(pkg, oracle_mod, idx, n_sample, half, skin):
     cfg = W.get_config(idx)
+    if skin is not None:
+        cfg = replace(cfg, skin=skin)
     assert cfg.n_steps % cfg.rebuild_every == 0
     s, p = W.make_system(cfg), W.make_params(cfg)
     n = len(s.pos)
@@ -109,6 +116,8 @@ def test_stated_run_length_nve(pkg, oracle_mod, idx, n_sample, half):
     # (d) the run moved the atoms for real: a kinetic/potential exchange took place and the lists changed
     assert abs(k1 - k0) > 1e-4 * k0, "no kinetic / potential exchange: did the run run?"
     assert longest1 != longest0 or idx == 4, f"longest skin lists did not change: {longest0} -> {longest1}"
+    if skin is not None:
+        assert longest0[1] <= 64 < longest1[1], f"the one-word / two-word mask limit was not crossed: {longest0} -> {longest1}"
     snap = pos.cpu().numpy()
     check_final_lists(nep, oracle_mod, cfg, snap, s.box, rng, n_sample)
     check_windows(nep, oracle_mod, cfg, p, s, snap, rng, half)
